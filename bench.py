@@ -1,0 +1,317 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched GW log-likelihood hot path on B200.
+
+Metric (BASELINE.json): GW log-likelihood evaluations per second.  Workload at N=1: BASELINE.json configs[1] --
+TaylorF2 3.5PN aligned-spin, H1+L1, 4 s at 2048 Hz (4017 complex128 bins per detector), B = 65536 parameter rows drawn
+from the config-3 prior box; one "step" = one gw_loglike_batch call over the whole batch (set-up kernel + bin-sweep kernel).
+Extra objects report the lock-step walk (ns_walk_batch) and a full nested-sampling run on the same machine.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--batch B] [--quick]
+
+One JSON line on stdout (rank 0).  --impl reference times the CPU oracle (oracle/) on the host cores instead.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12   # 148 SMs x 64 DFMA/clk x 2 flop x 1.965 GHz = 37.2
+METRIC = "gw_loglike_evals_per_sec"
+UNIT = "evals/s"
+
+
+def alg_flops_per_bin(n_det, model="taylorf2"):
+    """Algorithmic fp64 flops per (particle, bin) of the minimal formulation: 9-FMA phase (18),
+    quarter-turn sincos (31), per detector: phasor advance (6) + complex product (6) + <d,h> accumulate (4)."""
+    assert model == "taylorf2"
+    return 18 + 31 + 16 * n_det
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+
+    def __init__(self, index=0):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self.index = index
+        self._t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip().splitlines()[0]
+                f = [x.strip() for x in out.split(",")]
+                self.samples.append(float(f[0]))
+                self.max_mhz = float(f[1])
+                for n, v in zip(names, f[2:]):
+                    if v.lower().startswith("active"):
+                        self.reasons.add(n)
+            except Exception:
+                pass
+            self._stop.wait(0.1)
+
+    def __enter__(self):
+        self._t.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._t.join(timeout=6)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    return json.load(open(p)) if os.path.exists(p) else {}
+
+
+# --------------------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle as it stands
+# --------------------------------------------------------------------------------------------------------------
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    from paper_2509_04336_b200 import workloads as W
+    spec = W.config2(lambda s, th: O.OracleProblem(s).waveform(th))
+    P = O.OracleProblem(spec)
+    cores = os.cpu_count()
+    B = args.ref_batch
+    theta = P.prior_transform(W.uniforms(B, 11, 2))
+    for _ in range(args.warmup):
+        P.gw_loglike(theta[: max(64, B // 8)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        P.gw_loglike(theta)
+    dt = time.perf_counter() - t0
+    val = args.steps * B / dt
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"config2 gw_loglike_batch TaylorF2 H1+L1 4017 bins, bounded sample of {B} rows per step (CPU oracle)"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"{B} rows per step x {args.steps} steps, OpenMP over rows"},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2509_04336_b200 import nsgw, workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- workload: config 2.  The injected signal comes from the CUDA library itself (gw_waveform).
+    def wf_cuda(spec, th):
+        tmp = dict(spec)
+        tmp["strain"] = np.zeros((spec["n_det"], spec["n_freq"], 2))
+        hh = nsgw.Handle(tmp)
+        out = hh.gw_waveform(torch.as_tensor(th).cuda()).cpu().numpy()
+        hh.close()
+        return out
+
+    spec = W.config2(wf_cuda)
+    h = nsgw.Handle(spec)
+    B = args.batch
+    n_det, n_freq = spec["n_det"], spec["n_freq"]
+    u = torch.as_tensor(W.uniforms(B, 11, 2 + rank)).cuda()       # each rank: its own B rows (weak scaling, no collective)
+    theta = h.prior_transform_batch(u)
+    logl = torch.empty(B, dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+    stream = torch.cuda.current_stream()
+
+    def step():
+        h.gw_loglike_batch(theta, out=logl)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    n0 = nsgw.launch_count()
+    h.profile_enable(True)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        barrier()
+        for a, b in ev:
+            flush.zero_()                       # L2 flush between timed iterations (outside the event pair)
+            a.record(stream)
+            step()
+            b.record(stream)
+        barrier()
+    h.profile_enable(False)
+    launches = nsgw.launch_count() - n0
+    ms = sum(a.elapsed_time(b) for a, b in ev)
+    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    value = world * B * args.steps / (ms * 1e-3)
+    kern_ms, kern_n = h.profile_read()
+
+    # ---- end to end through the binding with HOST buffers: pinned theta -> H2D -> gw_loglike_batch -> D2H logL
+    th_host = theta.cpu().pin_memory()
+    out_host = torch.empty(B, dtype=torch.float64).pin_memory()
+    th_dev = torch.empty_like(theta)
+
+    def e2e_step():
+        th_dev.copy_(th_host, non_blocking=True)
+        h.gw_loglike_batch(th_dev, out=logl)
+        out_host.copy_(logl, non_blocking=True)
+        torch.cuda.synchronize()
+
+    for _ in range(3):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_val = world * B * args.steps / float(t.item())
+    assert torch.equal(out_host, logl.cpu())
+
+    line = None
+    if rank == 0:
+        peaks = measured_peaks()
+        fp64_burst = nsgw.measure_fp64_peak(1 << 17)
+        flops_launch = float(B) * n_freq * alg_flops_per_bin(n_det)
+        ach = flops_launch / (kern_ms / kern_n * 1e-3) / 1e12
+        roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
+                "traffic": None, "kernel": "k_bins<TaylorF2,2det,P=2>", "kernel_ms": kern_ms / kern_n,
+                "flops_per_particle_bin": alg_flops_per_bin(n_det),
+                "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
+                "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,
+                "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+                "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"config2 gw_loglike_batch TaylorF2 H1+L1 {n_freq} bins x {n_det} det, B={B} rows per GPU",
+                           "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"rows sharded x{world}, no collective"},
+                "clocks": clk.summary(),
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": B * 11 * 8, "d2h_bytes_per_step": B * 8},
+                "gpu_launches": int(launches), "roofline": roof}
+
+    # ---- extras (rank 0, N=1 only): walk throughput and one full nested-sampling run
+    if rank == 0 and world == 1 and not args.quick:
+        extras = {}
+        # lock-step walk on the same data: B_w walkers, W steps
+        Bw, Wl = 16384, 20
+        P_u = torch.as_tensor(W.uniforms(2 * Bw, 11, 9)).cuda()
+        ll = h.loglike_u_batch(P_u)
+        order = torch.argsort(ll)
+        donors = P_u[order[Bw:]].contiguous()
+        lstar = float(ll[order[Bw - 1]])
+        uw = donors[torch.arange(Bw, device="cuda") % donors.shape[0]].clone()
+        lw = ll[order[Bw:]][torch.arange(Bw, device="cuda") % donors.shape[0]].clone()
+        for rep in range(2):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            cnt = h.walk_batch(donors, uw, lw, lstar, Wl, 1234, 7 + rep)
+            b.record(stream)
+            torch.cuda.synchronize()
+        ne = int(cnt["n_eval"].sum())
+        wms = a.elapsed_time(b)
+        extras["walk"] = {"workload": f"ns_walk_batch config2 data, B={Bw}, W={Wl}", "evals_per_s": ne / (wms * 1e-3), "ms": wms,
+                          "evals": ne, "accept_mean": float(cnt["n_accept"].double().mean()),
+                          "accept_min": int(cnt["n_accept"].min()), "accept_max": int(cnt["n_accept"].max()),
+                          "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl)}
+        # full run: config 3 (PhenomD-form, H1+L1, n_live 1000, k 500, naccept 60, dlogz < 0.1)
+        spec3, smp3 = W.config3(wf_cuda_for(nsgw, torch))
+        h3 = nsgw.Handle(spec3, smp3, seed=1)
+        t0 = time.perf_counter()
+        nit, st = h3.run(smp3["term_kind"], smp3["term_tol"], 4000)
+        logz, err, H = h3.finalize_evidence()
+        wall = time.perf_counter() - t0
+        extras["ns_run_config3"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz, "logz_err": err,
+                                    "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
+                                    "evals_per_s": st["n_eval_total"] / wall}
+        h3.close()
+        line["extras"] = extras
+
+    # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample of the same rows (rank 0, N=1)
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        Pc = O.OracleProblem(spec)
+        nb = args.cpu_rows
+        th_np = theta[:nb].cpu().numpy()
+        Pc.gw_loglike(th_np[:64])
+        t0 = time.perf_counter()
+        lo = Pc.gw_loglike(th_np)
+        dt = time.perf_counter() - t0
+        lg = logl[:nb].cpu().numpy()
+        line["cpu_baseline"] = {"value": nb / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": f"first {nb} of the {B} rows, OpenMP over rows, {dt:.1f} s",
+                                "max_abs_dlogl_vs_gpu": float(np.max(np.abs(lg - lo)))}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    h.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def wf_cuda_for(nsgw, torch):
+    def wf(spec, th):
+        tmp = dict(spec)
+        tmp["strain"] = np.zeros((spec["n_det"], spec["n_freq"], 2))
+        hh = nsgw.Handle(tmp)
+        out = hh.gw_waveform(torch.as_tensor(th).cuda()).cpu().numpy()
+        hh.close()
+        return out
+    return wf
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--batch", type=int, default=65536)
+    ap.add_argument("--ref-batch", type=int, default=1024)
+    ap.add_argument("--cpu-rows", type=int, default=16384)
+    ap.add_argument("--quick", action="store_true", help="skip the walk / full-run extras")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,146 @@
+/* nsgw.h -- C-ABI of libnsgw.so: the batched acceptance-walk nested-sampling hot path of arXiv 2509.04336
+ * (Prathaban et al.) as hand-written sm_100a CUDA.
+ *
+ * Citations: "P:NNN" = line NNN of the paper text; "R:Lnn" = reading Lnn in DESIGN.md section 3 (adopted where
+ * the paper is silent).  The hot path is: delete the k lowest-logL live points, accumulate logX/logZ with the
+ * saw-tooth live count (eq. 3-5), start k independent walkers, each doing a fixed number of
+ * differential-evolution proposals in the unit hypercube (footnote P:120) with periodic wrap for ra/psi/phase
+ * (P:196), a prior transform (Table 1), a frequency-domain GW log-likelihood ratio (P:153, P:174,
+ * use_ratio P:196) and accept iff logL > logL* (P:96); then adapt the walk length at batch level.
+ *
+ * Conventions
+ *  - All *_dev pointers are CUDA device pointers, fp64 (or int32 where typed), row-major, caller-owned.  The library copies
+ *    strain / PSD / live points into handle-owned device memory in ns_init and never keeps a caller pointer afterwards.
+ *  - *_host pointers are host memory.  `stream` is a cudaStream_t passed as void* (NULL = default stream).
+ *  - Calls enqueue work on `stream` and return without synchronising unless the comment says "synchronises".
+ *  - Return value: 0 OK, -1 invalid argument, -2 CUDA error, -3 bad state/handle, -4 out of memory, -5 unsupported
+ *    configuration.  ns_last_error() returns a static/handle-owned message.  No exceptions cross the ABI.
+ *    A handle is not thread-safe.  There is no CPU fallback: without a CUDA device every compute call returns -2.
+ *  - theta columns (Table 1 order): 0 Mc[Msun] 1 q 2 chi1 3 chi2 4 dL[Mpc] 5 theta_jn 6 psi 7 phase 8 tc[s]
+ *    9 ra 10 dec.  Unit-cube rows u use the same order.  Unphysical theta (q not in (0,1], |chi|>1, dL<=0, Mc<=0,
+ *    non-finite) gives logL = -inf for that row, never an error.
+ */
+#ifndef NSGW_H
+#define NSGW_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define NSGW_MAX_DIM 16
+#define NSGW_MAX_DET 4
+#define NSGW_STRUCT_VERSION 1
+
+enum { NSGW_LIKE_GAUSSIAN_TOY = 0, NSGW_LIKE_GW_TAYLORF2 = 1, NSGW_LIKE_GW_PHENOMD_FORM = 2, NSGW_LIKE_CUBE_SHELL = 3 };
+enum { NSGW_PRIOR_UNIFORM = 0, NSGW_PRIOR_POWERLAW2 = 1, NSGW_PRIOR_SINE = 2, NSGW_PRIOR_COSINE = 3, NSGW_PRIOR_FIXED = 4 };
+
+typedef struct ns_handle ns_handle;
+
+/* Problem + sampler description (plain data, copied by ns_init). */
+typedef struct {
+  int32_t struct_version;              /* NSGW_STRUCT_VERSION */
+  int32_t like_kind;                   /* NSGW_LIKE_* ; GW kinds need ndim = 11 */
+  int32_t ndim;                        /* 1..16 */
+  int32_t n_live, n_delete;            /* k = n_delete (num_delete); 1 <= k <= n_live - 2 */
+  int32_t naccept, maxmcmc;            /* 60, 5000 */
+  double walks0;                       /* initial walk length (R:L13), e.g. 100 */
+  double delay;                        /* walk-length smoothing; < 0 -> max(n_live/(10 k) - 1, 0) (R:L14) */
+  int32_t prior_kind[NSGW_MAX_DIM];    /* NSGW_PRIOR_* per dimension; FIXED dims take the value prior_lo */
+  double prior_lo[NSGW_MAX_DIM], prior_hi[NSGW_MAX_DIM];
+  int32_t periodic[NSGW_MAX_DIM];      /* 1 = wrap the unit-cube coordinate instead of rejecting */
+  int32_t n_det, n_freq;               /* GW: detectors (<= 4) and bins per detector */
+  double f_min, df;                    /* f_k = f_min + k df, k = 0..n_freq-1 (both ends inclusive, R:L1) */
+  double det_vertex[NSGW_MAX_DET][3];  /* Earth-fixed vertex position [m] */
+  double det_xarm[NSGW_MAX_DET][3], det_yarm[NSGW_MAX_DET][3]; /* arm unit vectors */
+  double gmst;                         /* Greenwich mean sidereal time at the reference epoch [rad] */
+  double toy_mean[NSGW_MAX_DIM];       /* GAUSSIAN_TOY: logL = toy_lognorm - (theta-mean)^T P (theta-mean) / 2 */
+  double toy_prec[NSGW_MAX_DIM * NSGW_MAX_DIM]; /* row-major [ndim][ndim] in the leading ndim*ndim entries */
+  double toy_lognorm;
+  const double* phenom_table_host;     /* [19][11] fit table (DESIGN.md A.2); NULL -> built-in surrogate default */
+} ns_config;
+
+/* Per-step report written by ns_step / ns_run. */
+typedef struct {
+  int64_t iteration;                   /* index of the step just done (0-based) */
+  double logl_star;                    /* threshold = largest logL of the deleted batch */
+  double logx, logz, h;                /* accumulators after the step (dead points only) */
+  double dlogz;                        /* logaddexp(logZ, max logL_live + logX) - logZ            (R:L18 kind 0) */
+  double live_frac_log;                /* logsumexp(logL_live) - ln n_live + logX - logZ          (R:L18 kind 1) */
+  int32_t walk_len;                    /* W used by this step (R:L12) */
+  int32_t pad0;
+  double walks_next;                   /* real-valued walk length after adaptation (R:L13) */
+  double accept_mean;                  /* mean accepted proposals per walker */
+  int32_t accept_min, accept_max;
+  int64_t n_eval, n_oob, n_stuck;      /* likelihood evaluations, out-of-bounds proposals, zero-accept walkers (R:L15) */
+  int64_t n_eval_total;                /* since ns_init, including the initial live points */
+} ns_stats;
+
+/* Creates a sampler/likelihood context.  live_u_dev: [n_live, ndim] unit-cube points (NULL -> drawn from `seed`,
+ * Philox tag 2).  strain_dev: [n_det, n_freq, 2] (re, im), time origin at the reference epoch (R:L4); psd_dev: [n_det, n_freq]
+ * one-sided PSD; both NULL for non-GW kinds.  Precomputes the noise-weighted tables and evaluates logL of every live point.
+ * n_live may be 0 (likelihood-only context: only gw_* and ns_prior_transform_batch / ns_walk_batch are then valid).
+ * Synchronises. */
+int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, const double* strain_dev, const double* psd_dev,
+            uint64_t seed, void* stream);
+void ns_free(ns_handle* h);
+const char* ns_last_error(const ns_handle* h); /* h may be NULL: message of the last failed ns_init */
+
+/* logL of B physical parameter rows (R:L1: sum_det <d,h> - <h,h>/2).  parts_dev (optional) [B, 2 n_det] receives
+ * <d,h>_det, <h,h>_det interleaved. */
+int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream);
+
+/* Detector-frame signal of ONE parameter row on the handle's grid: out_dev [n_det, n_freq, 2] (R:L3). Used to build injections. */
+int gw_waveform(ns_handle* h, const double* theta_dev, double* out_dev, void* stream);
+
+/* Unit cube -> physical parameters (Table 1 kinds). */
+int ns_prior_transform_batch(ns_handle* h, const double* u_dev, int64_t B, double* theta_dev, void* stream);
+
+/* logL of B unit-cube rows under the handle's likelihood (transform + likelihood). */
+int ns_loglike_u_batch(ns_handle* h, const double* u_dev, int64_t B, double* logl_dev, void* stream);
+
+/* Lock-step acceptance walk of B walkers, walk_len proposals each, all against the frozen donor set
+ * donors_u_dev [m, ndim] (m >= 2).  u_dev [B, ndim] / logl_dev [B]: start state in, end state out.  Walker row r uses Philox
+ * counter (block, step, slot0 + r, stream_id), key = seed.  Counters (optional, may be NULL): accepted,
+ * evaluated, out-of-bounds proposals per walker.  trace_flags_dev [B, walk_len] u8 (bit0 oob, bit1 accepted, bit2 evaluated)
+ * and trace_logl_dev [B, walk_len] (NaN when not evaluated) are optional. */
+int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u_dev, double* logl_dev, int64_t B,
+                  double logl_star, int32_t walk_len, uint64_t seed, uint32_t stream_id, int64_t slot0,
+                  int32_t* n_accept_dev, int32_t* n_eval_dev, int32_t* n_oob_dev, uint8_t* trace_flags_dev,
+                  double* trace_logl_dev, void* stream);
+
+/* One nested-sampling iteration: select the k lowest, evidence scan, start points, walks, write-back, adapt.
+ * stats_host (optional) is filled after a stream synchronise (synchronises iff non-NULL).  dead_dev (optional) [k, ndim+3]
+ * receives (u.., logL, log w, n_i) of the deleted points in ascending logL. */
+int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream);
+
+/* Steps until the termination rule fires (term_kind 0: dlogz < tol; 1: live evidence fraction < tol) or
+ * max_iter.  dead_dev (optional) [max_iter * k, ndim+3].  Returns the number of steps done (>= 0) or an error (< 0).
+ * Synchronises once per step (one 128-byte read-back). */
+int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host, double* dead_dev,
+               void* stream);
+
+/* Copies the live set out: u_dev [n_live, ndim], logl_dev [n_live] (either may be NULL). */
+int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream);
+
+/* Adds the remaining live points (n_i = n, n-1, .., 1; R:L17) to a copy of the accumulators.  Synchronises. */
+int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host, double* h_host, void* stream);
+
+/* Device FP64 FMA throughput probe used for the roofline denominator: runs `iters` dependent-chain DFMAs x 8 chains per
+ * thread on a full grid and returns achieved TFLOP/s in *tflops_host (synchronises; timed with CUDA events). */
+int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream);
+
+/* Optional timing of the dominant kernel (the bin sweep of gw_loglike_batch): while enabled, every launch is bracketed by a
+ * CUDA event pair on the launching stream (at most 4096 pairs are kept).  nsgw_profile_read synchronises on those events,
+ * returns their summed duration and count, and clears them. */
+int nsgw_profile_enable(ns_handle* h, int32_t on);
+int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_host);
+
+/* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */
+int64_t nsgw_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NSGW_H */

@@ -183,7 +183,7 @@ class OracleSampler:
         self.n_live, self.n_delete, self.ndim = n_live, n_delete, prob.ndim
 
     def __del__(self):
-        if getattr(self, "h", None):
+        if getattr(self, "h", None) and _lib is not None:
             _lib.orc_state_free(self.h)
             self.h = None
 

@@ -1,0 +1,1159 @@
+// nsgw.cu -- kernels and C-ABI of libnsgw.so (see include/nsgw.h for the contract, DESIGN.md for the design).
+//
+// Kernels
+//   k_tables          ns_init: per-bin tables and noise-weighted data (parameter independent)
+//   k_setup           theta[B,11] -> per-particle coefficient blocks (one thread per particle)
+//   k_bins            K1: CTA per P particles, bins strided over threads, shuffle + smem reduction
+//   k_walk_gw         K2: persistent lock-step acceptance walk, CTA per P walkers, W steps in-kernel
+//   k_walk_simple     K2 for bin-less likelihoods (Gaussian toy, cube shell): one thread per walker
+//   k_rank / k_evidence / k_gather_start / k_writeback / k_adapt   K3: select, evidence scan, replacement, adaptation
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <cmath>
+#include <string>
+#include <atomic>
+#include <vector>
+#include <algorithm>
+#include <climits>
+
+#include "../../include/nsgw.h"
+#include "nsgw_device.cuh"
+
+using namespace nsgw;
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+thread_local std::string g_init_error;
+
+// One CTA shape for every bin sweep (likelihood batch and walk): the same particle then gets bit-identical logL from
+// either entry point (same per-thread bin assignment, same reduction tree).
+constexpr int kBinsThreads = 256;
+constexpr int kWalkThreads = 256;
+
+// ======================================================================================================
+// Device state of the sampler
+// ======================================================================================================
+struct DevState {
+  double logx, logz, h, walks, delay, lstar;
+  long long iter, n_eval_total;
+  int W, naccept, maxmcmc, pad;
+  ns_stats stats;
+};
+
+// ======================================================================================================
+// ns_init kernels
+// ======================================================================================================
+__global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const double* __restrict__ psd, double* tf, double* ty,
+                         double* tL, double* tx, double* tf34, double2* wd, double* ws) {
+  const int nf = cfg->n_freq, nd = cfg->n_det;
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nf; k += gridDim.x * blockDim.x) {
+    double f = cfg->f_min + k * cfg->df;
+    double x = cbrt(f);
+    tf[k] = f; tx[k] = x; ty[k] = 1.0 / x; tL[k] = log(f); tf34[k] = sqrt(sqrt(f * f * f));
+    double a76 = 1.0 / (f * sqrt(x));      // f^-7/6
+    for (int d = 0; d < nd; ++d) {
+      double S = psd[(size_t)d * nf + k];
+      double w = 4.0 * cfg->df / S;
+      wd[(size_t)d * nf + k] = make_double2(w * a76 * strain[((size_t)d * nf + k) * 2], w * a76 * strain[((size_t)d * nf + k) * 2 + 1]);
+      ws[(size_t)d * nf + k] = w * a76 * a76;
+    }
+  }
+}
+
+// I_{7/3} per detector: deterministic single-CTA tree sum.
+__global__ void k_i73(DevCfg* cfg, const double* __restrict__ ws) {
+  __shared__ double sh[256];
+  const int nf = cfg->n_freq;
+  for (int d = 0; d < cfg->n_det; ++d) {
+    double acc = 0.0;
+    for (int k = threadIdx.x; k < nf; k += 256) acc += ws[(size_t)d * nf + k];
+    sh[threadIdx.x] = acc;
+    __syncthreads();
+    for (int s = 128; s > 0; s >>= 1) {
+      if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
+      __syncthreads();
+    }
+    if (threadIdx.x == 0) cfg->i73[d] = sh[0];
+    __syncthreads();
+  }
+}
+
+__global__ void k_draw_live(int ndim, long long n, uint32_t k0, uint32_t k1, double* u) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  for (int d = 0; d < ndim; d += 2) {
+    uint32_t w[4];
+    philox4x32_10((uint32_t)(d / 2), 0u, (uint32_t)i, 2u << 24, k0, k1, w);
+    u[i * ndim + d] = u01(w[0], w[1]);
+    if (d + 1 < ndim) u[i * ndim + d + 1] = u01(w[2], w[3]);
+  }
+}
+
+__global__ void k_prior_transform(const DevCfg* __restrict__ cfg, const double* __restrict__ u, long long B, double* theta) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  const int D = cfg->ndim;
+  if (i >= B * D) return;
+  int d = (int)(i % D);
+  theta[i] = prior_transform_dim(cfg->prior_kind[d], cfg->prior_lo[d], cfg->prior_hi[d], u[i]);
+}
+
+// ======================================================================================================
+// K1: set-up + bin loop
+// ======================================================================================================
+template <int MODEL>
+__global__ void k_setup(const DevCfg* __restrict__ cfg, const double* __restrict__ theta, long long B, double* cbs) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= B) return;
+  double th[11];
+#pragma unroll
+  for (int d = 0; d < 11; ++d) th[d] = theta[i * 11 + d];
+  setup_particle<MODEL>(*cfg, th, cbs + i * CB_SIZE);
+}
+
+// Start phasors: for particle p, detector d, thread t (bin t of the first sweep):
+//   R = (Cr + i Ci) * exp(i * dtq * f_t)  [quarter turns], built as lane-table x warp-table to keep it to one sincos per entry.
+// tabL[(p*NDET+d)*32 + lane] = exp(i dtq df lane); tabW[(p*NDET+d)*NW + w] = C * exp(i dtq (f_min + 32 w df)).
+template <int NDET, int P, int NT>
+__device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const double* cbs /*smem [P][CB_SIZE]*/, double2* tabL,
+                                                    double2* tabW, double2* step) {
+  constexpr int NW = NT / 32;
+  constexpr int NE = P * NDET * (32 + NW + 1);
+  for (int e = threadIdx.x; e < NE; e += NT) {
+    int pd = e / (32 + NW + 1), j = e % (32 + NW + 1);
+    int p = pd / NDET, d = pd % NDET;
+    const double* cb = cbs + p * CB_SIZE;
+    double dtq = cb[CB_DET + 4 * d + 2];
+    double s, c;
+    if (j < 32) {
+      sincos_qt(dtq * (cfg.df * j), s, c);
+      tabL[pd * 32 + j] = make_double2(c, s);
+    } else if (j < 32 + NW) {
+      int w = j - 32;
+      sincos_qt(dtq * (cfg.f_min + cfg.df * (32 * w)), s, c);
+      double cr = cb[CB_DET + 4 * d], ci = cb[CB_DET + 4 * d + 1];
+      tabW[pd * NW + w] = make_double2(cr * c - ci * s, cr * s + ci * c);
+    } else {
+      sincos_qt(dtq * (cfg.df * NT), s, c);
+      step[pd] = make_double2(c, s);
+    }
+  }
+}
+
+// Bin loop for P particles held by this CTA.  Outputs per particle/detector partial sums (per thread) of
+//   dh = sum_k Re(conj(wd_k) * amp_k * E_k * R_k),  hh = sum_k amp_k^2 ws_k   (PhenomD only; TaylorF2 uses I_{7/3}).
+template <int MODEL, int NDET, int P, int NT>
+__device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
+                                         const double2* tabW, const double2* step, const bool* active, double (&dh)[P][NDET],
+                                         double (&hh)[P][NDET]) {
+  constexpr int NW = NT / 32;
+  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
+  double2 R[P][NDET], St[P][NDET];
+#pragma unroll
+  for (int p = 0; p < P; ++p)
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      double2 a = tabL[(p * NDET + d) * 32 + lane], b = tabW[(p * NDET + d) * NW + wrp];
+      R[p][d] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+      St[p][d] = step[p * NDET + d];
+      dh[p][d] = 0.0; hh[p][d] = 0.0;
+    }
+  const int nf = cfg.n_freq;
+  for (int k = tid; k < nf; k += NT) {
+    BinBasis b = make_basis(tb, k, MODEL == 2);
+    double2 w[NDET];
+    double wsv[NDET];
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      w[d] = __ldg(tb.wd[d] + k);
+      if (MODEL == 2) wsv[d] = __ldg(tb.ws[d] + k);
+    }
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+      if (!active[p]) continue;
+      const double* cb = cbs + p * CB_SIZE;
+      double q, amp = 1.0;
+      if (MODEL == 1) q = phase_pn_qt(cb + CB_PH, b);
+      else phenom_bin(cb, b, q, amp);
+      double s, c;
+      sincos_qt(q, s, c);
+      double er = c, ei = -s;       // E = exp(-i Phi_c)
+      if (MODEL == 2) { er *= amp; ei *= amp; }
+      double a2 = amp * amp;
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) {
+        double gr = er * R[p][d].x - ei * R[p][d].y;
+        double gi = er * R[p][d].y + ei * R[p][d].x;
+        dh[p][d] = fma(w[d].x, gr, dh[p][d]);
+        dh[p][d] = fma(w[d].y, gi, dh[p][d]);
+        if (MODEL == 2) hh[p][d] = fma(a2, wsv[d], hh[p][d]);
+        // advance the detector phasor by one sweep
+        double nr = R[p][d].x * St[p][d].x - R[p][d].y * St[p][d].y;
+        double ni = R[p][d].x * St[p][d].y + R[p][d].y * St[p][d].x;
+        R[p][d].x = nr; R[p][d].y = ni;
+      }
+    }
+  }
+}
+
+// Deterministic block reduction of NV values per thread: warp shuffle tree, then fixed-order sum over warps by thread 0..NV-1.
+template <int NV, int NT>
+__device__ __forceinline__ void block_reduce(double (&v)[NV], double* red /*smem [NT/32][NV]*/, double* out /*smem [NV]*/) {
+  constexpr int NW = NT / 32;
+#pragma unroll
+  for (int i = 0; i < NV; ++i) {
+    double x = v[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+    v[i] = x;
+  }
+  if ((threadIdx.x & 31) == 0) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) red[(threadIdx.x >> 5) * NV + i] = v[i];
+  }
+  __syncthreads();
+  if (threadIdx.x < NV) {
+    double s = 0.0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) s += red[w * NV + threadIdx.x];
+    out[threadIdx.x] = s;
+  }
+  __syncthreads();
+}
+
+// Finishes logL of particle p from reduced sums (out: [P][NDET][2] = dh, hh).
+template <int MODEL, int NDET>
+__device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* cb, const double* sums, double* parts) {
+  if (cb[CB_VALID] == 0.0) {
+    if (parts) for (int d = 0; d < 2 * NDET; ++d) parts[d] = nan("");
+    return -INFINITY;
+  }
+  double logl = 0.0;
+#pragma unroll
+  for (int d = 0; d < NDET; ++d) {
+    double dh = sums[2 * d];
+    double hh = (MODEL == 1) ? cb[CB_DET + 4 * d + 3] * cfg.i73[d] : cb[CB_DET + 4 * d + 3] * sums[2 * d + 1];
+    if (parts) { parts[2 * d] = dh; parts[2 * d + 1] = hh; }
+    logl += dh - 0.5 * hh;
+  }
+  return logl;
+}
+
+template <int MODEL, int NDET, int P>
+__global__ void __launch_bounds__(kBinsThreads) k_bins(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
+                                                        long long B, double* logl, double* parts) {
+  constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * NDET * 2;
+  __shared__ double cbs[P * CB_SIZE];
+  __shared__ double2 tabL[P * NDET * 32], tabW[P * NDET * NW], step[P * NDET];
+  __shared__ double red[NW * NV], out[NV];
+  __shared__ bool active[P];
+  const DevCfg& cfg = *cfgp;
+  const long long p0 = (long long)blockIdx.x * P;
+  for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
+    long long p = p0 + e / CB_SIZE;
+    cbs[e] = (p < B) ? cbs_g[p * CB_SIZE + e % CB_SIZE] : 0.0;
+  }
+  __syncthreads();
+  if (threadIdx.x < P) active[threadIdx.x] = cbs[threadIdx.x * CB_SIZE + CB_VALID] != 0.0;
+  build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
+  __syncthreads();
+  double dh[P][NDET], hh[P][NDET];
+  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, dh, hh);
+  double v[NV];
+#pragma unroll
+  for (int p = 0; p < P; ++p)
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) { v[(p * NDET + d) * 2] = dh[p][d]; v[(p * NDET + d) * 2 + 1] = hh[p][d]; }
+  block_reduce<NV, NT>(v, red, out);
+  if (threadIdx.x < P && p0 + threadIdx.x < B) {
+    int p = threadIdx.x;
+    logl[p0 + p] = finish_logl<MODEL, NDET>(cfg, cbs + p * CB_SIZE, out + p * NDET * 2, parts ? parts + (p0 + p) * 2 * NDET : nullptr);
+  }
+}
+
+// Detector-frame waveform of one theta on the grid (for injections): out[n_det][n_freq][2].
+template <int MODEL>
+__global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ theta, double* out) {
+  __shared__ double cb[CB_SIZE];
+  const DevCfg& cfg = *cfgp;
+  if (threadIdx.x == 0) {
+    double th[11];
+    for (int d = 0; d < 11; ++d) th[d] = theta[d];
+    setup_particle<MODEL>(cfg, th, cb);
+  }
+  __syncthreads();
+  const int nf = cfg.n_freq;
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nf; k += gridDim.x * blockDim.x) {
+    BinBasis b = make_basis(tb, k, MODEL == 2);
+    double q, amp = 1.0;
+    if (MODEL == 1) q = phase_pn_qt(cb + CB_PH, b);
+    else phenom_bin(cb, b, q, amp);
+    double a76 = b.y3 * sqrt(b.y);   // f^-7/6
+    for (int d = 0; d < cfg.n_det; ++d) {
+      double s, c;
+      sincos_qt(q - cb[CB_DET + 4 * d + 2] * b.f, s, c);   // Phi_det = Phi_c + 2 pi f dt
+      double cr = cb[CB_DET + 4 * d] * amp * a76, ci = cb[CB_DET + 4 * d + 1] * amp * a76;
+      bool ok = cb[CB_VALID] != 0.0;
+      out[((size_t)d * nf + k) * 2] = ok ? cr * c + ci * s : nan("");
+      out[((size_t)d * nf + k) * 2 + 1] = ok ? ci * c - cr * s : nan("");
+    }
+  }
+}
+
+// ======================================================================================================
+// K2: acceptance walk
+// ======================================================================================================
+struct WalkArgs {
+  const double* donors;  // [m, D]
+  int m;
+  double* u;             // [B, D]
+  double* logl;          // [B]
+  long long B;
+  double lstar;
+  const double* lstar_dev;  // if non-null overrides lstar
+  int W;
+  const int* W_dev;         // if non-null overrides W
+  uint32_t k0, k1, stream_id;
+  const long long* iter_dev;  // if non-null: stream_id |= (*iter & 0xFFFFFF)
+  long long slot0;
+  int* n_accept; int* n_eval; int* n_oob;
+  uint8_t* tflags; double* tlogl;
+  int trace_stride;
+};
+
+// DE proposal for one walker (footnote P:120; R:L8-L10).  Returns false if out of bounds.
+__device__ __forceinline__ bool de_propose(const DevCfg& cfg, const WalkArgs& a, uint32_t sid, uint32_t t, uint32_t slot,
+                                           const double* cur, double* prop) {
+  uint32_t b0[4];
+  philox4x32_10(0u, t, slot, sid, a.k0, a.k1, b0);
+  uint32_t ia = __umulhi(b0[0], (uint32_t)a.m);
+  uint32_t ib = __umulhi(b0[1], (uint32_t)(a.m - 1));
+  ib += (ib >= ia) ? 1u : 0u;
+  double gamma = 1.0;
+  if (b0[2] >= 0x80000000u) {
+    uint32_t b1[4], b2[4];
+    philox4x32_10(1u, t, slot, sid, a.k0, a.k1, b1);
+    philox4x32_10(2u, t, slot, sid, a.k0, a.k1, b2);
+    double prod = ((u01(b1[0], b1[1]) * u01(b1[2], b1[3])) * u01(b2[0], b2[1])) * u01(b2[2], b2[3]);
+    gamma = (2.38 / sqrt(2.0 * cfg.n_free)) * (-0.25 * log(prod));
+  }
+  const int D = cfg.ndim;
+  bool inb = true;
+  for (int d = 0; d < D; ++d) {
+    if (cfg.prior_kind[d] == 4) { prop[d] = cur[d]; continue; }
+    double diff = a.donors[(size_t)ia * D + d] - a.donors[(size_t)ib * D + d];
+    double x = fma(gamma, diff, cur[d]);
+    if (cfg.periodic[d]) x = x - floor(x);
+    else if (!(x > 0.0 && x < 1.0)) inb = false;
+    prop[d] = x;
+  }
+  return inb;
+}
+
+__device__ __forceinline__ double simple_loglike(const DevCfg& cfg, const double* u) {
+  const int D = cfg.ndim;
+  if (cfg.like_kind == 3) {
+    double r = 0.0;
+    for (int d = 0; d < D; ++d) r = fmax(r, fabs(u[d] - 0.5));
+    return -r;
+  }
+  double th[kMaxDim];
+  for (int d = 0; d < D; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], u[d]) - cfg.toy_mean[d];
+  double qf = 0.0;
+  for (int i = 0; i < D; ++i)
+    for (int j = 0; j < D; ++j) qf += th[i] * cfg.toy_prec[i * D + j] * th[j];
+  return cfg.toy_lognorm - 0.5 * qf;
+}
+
+__global__ void k_loglike_simple(const DevCfg* __restrict__ cfgp, const double* __restrict__ u, long long B, double* logl) {
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (i >= B) return;
+  double uu[kMaxDim];
+  for (int d = 0; d < cfgp->ndim; ++d) uu[d] = u[i * cfgp->ndim + d];
+  logl[i] = simple_loglike(*cfgp, uu);
+}
+
+__global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
+  long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (row >= a.B) return;
+  const DevCfg& cfg = *cfgp;
+  const int D = cfg.ndim;
+  const int W = a.W_dev ? *a.W_dev : a.W;
+  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
+  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
+  const uint32_t slot = (uint32_t)(a.slot0 + row);
+  double cur[kMaxDim], prop[kMaxDim];
+  for (int d = 0; d < D; ++d) cur[d] = a.u[row * D + d];
+  double curl = a.logl[row];
+  int na = 0, ne = 0, no = 0;
+  for (int t = 0; t < W; ++t) {
+    bool inb = de_propose(cfg, a, sid, (uint32_t)t, slot, cur, prop);
+    uint8_t fl = 0;
+    double pl = nan("");
+    if (!inb) { ++no; fl = 1; }
+    else {
+      pl = simple_loglike(cfg, prop);
+      ++ne; fl = 4;
+      if (pl > lstar) {
+        for (int d = 0; d < D; ++d) cur[d] = prop[d];
+        curl = pl; ++na; fl |= 2;
+      }
+    }
+    if (a.tflags) a.tflags[row * a.trace_stride + t] = fl;
+    if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
+  }
+  for (int d = 0; d < D; ++d) a.u[row * D + d] = cur[d];
+  a.logl[row] = curl;
+  if (a.n_accept) a.n_accept[row] = na;
+  if (a.n_eval) a.n_eval[row] = ne;
+  if (a.n_oob) a.n_oob[row] = no;
+}
+
+// GW walk: CTA per P walkers.  Each step: lanes 0..P-1 propose + transform + set up (phase A), all threads sweep the bins
+// (phase B), lanes 0..P-1 accept (phase C, merged with the next phase A).  All walkers do exactly W steps.
+template <int MODEL, int NDET, int P>
+__global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+  constexpr int NT = kWalkThreads, NW = NT / 32, NV = P * NDET * 2;
+  __shared__ double cbs[P * CB_SIZE];
+  __shared__ double2 tabL[P * NDET * 32], tabW[P * NDET * NW], step[P * NDET];
+  __shared__ double red[NW * NV], out[NV];
+  __shared__ bool active[P];
+  __shared__ double s_cur[P][kMaxDim], s_prop[P][kMaxDim], s_curl[P];
+  const DevCfg& cfg = *cfgp;
+  const int D = cfg.ndim;
+  const int W = a.W_dev ? *a.W_dev : a.W;
+  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
+  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
+  const int tid = threadIdx.x;
+  const long long row = (long long)blockIdx.x * P + tid;
+  const bool owner = tid < P && row < a.B;
+  int na = 0, ne = 0, no = 0;
+  if (tid < P) {
+    active[tid] = false;
+    if (owner) {
+      for (int d = 0; d < D; ++d) s_cur[tid][d] = a.u[row * D + d];
+      s_curl[tid] = a.logl[row];
+    }
+  }
+  __syncthreads();
+  for (int t = 0; t < W; ++t) {
+    // ---- phase A: proposal, bounds, prior transform, waveform set-up
+    if (owner) {
+      bool inb = de_propose(cfg, a, sid, (uint32_t)t, (uint32_t)(a.slot0 + row), s_cur[tid], s_prop[tid]);
+      bool act = false;
+      if (inb) {
+        double th[11];
+#pragma unroll
+        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[tid][d]);
+        act = setup_particle<MODEL>(cfg, th, cbs + tid * CB_SIZE);
+        ++ne;
+      } else {
+        ++no;
+        cbs[tid * CB_SIZE + CB_VALID] = 0.0;
+      }
+      active[tid] = act;
+      if (!inb) {
+        if (a.tflags) a.tflags[row * a.trace_stride + t] = 1;
+        if (a.tlogl) a.tlogl[row * a.trace_stride + t] = nan("");
+      }
+      s_prop[tid][kMaxDim - 1] = inb ? 1.0 : 0.0;   // ndim <= 11 for GW: slot 15 is free
+    }
+    __syncthreads();
+    build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
+    __syncthreads();
+    // ---- phase B: bins
+    double dh[P][NDET], hh[P][NDET];
+    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, dh, hh);
+    double v[NV];
+#pragma unroll
+    for (int p = 0; p < P; ++p)
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) { v[(p * NDET + d) * 2] = dh[p][d]; v[(p * NDET + d) * 2 + 1] = hh[p][d]; }
+    block_reduce<NV, NT>(v, red, out);
+    // ---- phase C: accept iff in bounds and logL' > L*
+    if (owner && s_prop[tid][kMaxDim - 1] != 0.0) {
+      double pl = finish_logl<MODEL, NDET>(cfg, cbs + tid * CB_SIZE, out + tid * NDET * 2, nullptr);
+      uint8_t fl = 4;
+      if (pl > lstar) {
+        for (int d = 0; d < D; ++d) s_cur[tid][d] = s_prop[tid][d];
+        s_curl[tid] = pl; ++na; fl |= 2;
+      }
+      if (a.tflags) a.tflags[row * a.trace_stride + t] = fl;
+      if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
+    }
+    __syncthreads();
+  }
+  if (owner) {
+    for (int d = 0; d < D; ++d) a.u[row * D + d] = s_cur[tid][d];
+    a.logl[row] = s_curl[tid];
+    if (a.n_accept) a.n_accept[row] = na;
+    if (a.n_eval) a.n_eval[row] = ne;
+    if (a.n_oob) a.n_oob[row] = no;
+  }
+}
+
+// ======================================================================================================
+// K3: selection, evidence, replacement, adaptation
+// ======================================================================================================
+// Stable rank by counting: order[rank(i)] = i with rank(i) = #{j : l_j < l_i or (l_j == l_i and j < i)}  (R:L6).
+__global__ void k_rank(const double* __restrict__ logl, int n, int* order) {
+  __shared__ double tile[256];
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  double li = (i < n) ? logl[i] : 0.0;
+  int rank = 0;
+  for (int base = 0; base < n; base += 256) {
+    int j = base + threadIdx.x;
+    tile[threadIdx.x] = (j < n) ? logl[j] : INFINITY;
+    __syncthreads();
+    int lim = min(256, n - base);
+    for (int jj = 0; jj < lim; ++jj) {
+      double lj = tile[jj];
+      rank += (lj < li) || (lj == li && (base + jj) < i);
+    }
+    __syncthreads();
+  }
+  if (i < n) order[rank] = i;
+}
+
+__device__ __forceinline__ double logaddexp_d(double a, double b) {
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  double m = fmax(a, b);
+  return m + log1p(exp(-fabs(a - b)));
+}
+
+__device__ __forceinline__ void evidence_update(double li, double ni, double& logx, double& logz, double& h, double& logw) {
+  logw = logx + log(-expm1(-1.0 / ni));
+  double lw = li + logw;
+  double zn = logaddexp_d(logz, lw);
+  double hn = exp(lw - zn) * li;
+  if (logz != -INFINITY) hn += exp(logz - zn) * (h + logz);
+  hn -= zn;
+  h = hn; logz = zn; logx -= 1.0 / ni;
+}
+
+// Sequential evidence scan over the k dead points in ascending logL (eq. 3-5 with the saw-tooth live count; R:L16, L17).
+__global__ void k_evidence(DevState* st, const double* __restrict__ logl, const double* __restrict__ u, const int* __restrict__ order,
+                           int n, int k, int D, double* dead) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double logx = st->logx, logz = st->logz, h = st->h;
+  for (int i = 0; i < k; ++i) {
+    int id = order[i];
+    double logw;
+    evidence_update(logl[id], (double)(n - i), logx, logz, h, logw);
+    if (dead) {
+      double* row = dead + (size_t)i * (D + 3);
+      for (int d = 0; d < D; ++d) row[d] = u[(size_t)id * D + d];
+      row[D] = logl[id]; row[D + 1] = logw; row[D + 2] = (double)(n - i);
+    }
+  }
+  st->logx = logx; st->logz = logz; st->h = h;
+  st->lstar = logl[order[k - 1]];
+  int W = (int)floor(st->walks);
+  st->W = max(1, min(W, st->maxmcmc));
+}
+
+// Survivor array in ascending-logL order + start points (uniform survivor, Philox tag 1; R:L7).
+__global__ void k_gather_start(const DevState* __restrict__ st, const double* __restrict__ u, const double* __restrict__ logl,
+                               const int* __restrict__ order, int n, int k, int D, uint32_t k0, uint32_t k1, double* surv, double* cur_u,
+                               double* cur_l) {
+  const int m = n - k;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < m) {
+    int id = order[k + i];
+    for (int d = 0; d < D; ++d) surv[(size_t)i * D + d] = u[(size_t)id * D + d];
+  }
+  if (i < k) {
+    uint32_t w[4];
+    philox4x32_10(0u, 0u, (uint32_t)i, (1u << 24) | (uint32_t)(st->iter & 0xFFFFFF), k0, k1, w);
+    int id = order[k + __umulhi(w[0], (uint32_t)m)];
+    for (int d = 0; d < D; ++d) cur_u[(size_t)i * D + d] = u[(size_t)id * D + d];
+    cur_l[i] = logl[id];
+  }
+}
+
+__global__ void k_writeback(const int* __restrict__ order, int k, int D, const double* __restrict__ cur_u, const double* __restrict__ cur_l,
+                            double* u, double* logl) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= k) return;
+  int id = order[j];
+  for (int d = 0; d < D; ++d) u[(size_t)id * D + d] = cur_u[(size_t)j * D + d];
+  logl[id] = cur_l[j];
+}
+
+// Batch-level adaptation (R:L13-L15) and termination quantities (R:L18).  Single CTA, fixed-order reductions.
+__global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __restrict__ ne, const int* __restrict__ no, int k,
+                        const double* __restrict__ logl, int n) {
+  __shared__ long long s_a[256], s_e[256], s_o[256], s_s[256];
+  __shared__ int s_min[256], s_max[256];
+  __shared__ double s_d[256];
+  const int t = threadIdx.x;
+  long long a = 0, e = 0, o = 0, s = 0;
+  int mn = INT_MAX, mx = INT_MIN;
+  for (int j = t; j < k; j += 256) {
+    a += na[j]; e += ne[j]; o += no[j]; s += (na[j] == 0);
+    mn = min(mn, na[j]); mx = max(mx, na[j]);
+  }
+  s_a[t] = a; s_e[t] = e; s_o[t] = o; s_s[t] = s; s_min[t] = mn; s_max[t] = mx;
+  double lm = -INFINITY;
+  for (int i = t; i < n; i += 256) lm = fmax(lm, logl[i]);
+  s_d[t] = lm;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (t < w) {
+      s_a[t] += s_a[t + w]; s_e[t] += s_e[t + w]; s_o[t] += s_o[t + w]; s_s[t] += s_s[t + w];
+      s_min[t] = min(s_min[t], s_min[t + w]); s_max[t] = max(s_max[t], s_max[t + w]);
+      s_d[t] = fmax(s_d[t], s_d[t + w]);
+    }
+    __syncthreads();
+  }
+  const double lmax = s_d[0];
+  __syncthreads();
+  double acc = 0.0;
+  for (int i = t; i < n; i += 256) acc += exp(logl[i] - lmax);
+  s_d[t] = acc;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (t < w) s_d[t] += s_d[t + w];
+    __syncthreads();
+  }
+  if (t == 0) {
+    const int W = st->W;
+    double amean = (double)s_a[0] / k;
+    double r = fmax(0.5, amean) / W;
+    double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
+    st->walks = walks;
+    st->n_eval_total += s_e[0];
+    double lse = lmax + log(s_d[0]);
+    ns_stats& o_ = st->stats;
+    o_.iteration = st->iter;
+    o_.logl_star = st->lstar; o_.logx = st->logx; o_.logz = st->logz; o_.h = st->h;
+    o_.dlogz = logaddexp_d(st->logz, lmax + st->logx) - st->logz;
+    o_.live_frac_log = lse - log((double)n) + st->logx - st->logz;
+    o_.walk_len = W; o_.pad0 = 0; o_.walks_next = walks;
+    o_.accept_mean = amean; o_.accept_min = s_min[0]; o_.accept_max = s_max[0];
+    o_.n_eval = s_e[0]; o_.n_oob = s_o[0]; o_.n_stuck = s_s[0]; o_.n_eval_total = st->n_eval_total;
+    st->iter += 1;
+  }
+}
+
+// Final evidence: adds the live points with n_i = n..1 to a copy of the accumulators (R:L17).  out: logz, h.
+__global__ void k_finalize(const DevState* __restrict__ st, const double* __restrict__ logl, const int* __restrict__ order, int n,
+                           double* out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double logx = st->logx, logz = st->logz, h = st->h, lw;
+  for (int i = 0; i < n; ++i) evidence_update(logl[order[i]], (double)(n - i), logx, logz, h, lw);
+  out[0] = logz; out[1] = h;
+}
+
+// FP64 FMA throughput probe: 8 independent chains per thread.
+__global__ void k_dfma_probe(long long iters, double* sink) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, c = 1e-7;
+  for (long long i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) sink[0] = s;
+}
+
+}  // namespace
+
+// ======================================================================================================
+// Host side
+// ======================================================================================================
+struct ns_handle {
+  ns_config cfg;
+  DevCfg* d_cfg = nullptr;
+  DevState* d_state = nullptr;
+  Tables tb{};
+  double* d_tab = nullptr;      // f, y, L, x, f34 (5 * nf)
+  double2* d_wd = nullptr;      // [n_det][nf]
+  double* d_ws = nullptr;       // [n_det][nf]
+  double* d_live_u = nullptr;   // [n_live][D]
+  double* d_live_l = nullptr;
+  int* d_order = nullptr;
+  double* d_surv = nullptr;     // [n_live - k][D]
+  double* d_cur_u = nullptr;    // [k][D]
+  double* d_cur_l = nullptr;
+  int* d_cnt = nullptr;         // 3 * k
+  double* d_cb = nullptr;       // coefficient blocks scratch
+  long long cb_cap = 0;
+  double* d_theta = nullptr;    // scratch theta
+  long long theta_cap = 0;
+  double* d_fin = nullptr;      // 2 doubles
+  ns_stats* h_stats = nullptr;  // pinned
+  double* h_fin = nullptr;      // pinned
+  uint64_t seed = 0;
+  std::string err;
+  int n_free = 0;
+  bool prof = false;                                   // nsgw_profile_enable
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev;  // event pairs around the dominant kernel
+};
+
+namespace {
+
+int fail(ns_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_init_error = msg;
+  return code;
+}
+
+#define CU_CHECK(h, expr)                                                                         \
+  do {                                                                                            \
+    cudaError_t e_ = (expr);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return fail(h, e_ == cudaErrorMemoryAllocation ? -4 : -2, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+#define LAUNCH_CHECK(h)                                                                           \
+  do {                                                                                            \
+    g_launches.fetch_add(1);                                                                      \
+    cudaError_t e_ = cudaGetLastError();                                                          \
+    if (e_ != cudaSuccess) return fail(h, -2, std::string("kernel launch: ") + cudaGetErrorString(e_)); \
+  } while (0)
+
+const double kSurrogate[19][2] = {
+    {3931.9, -17395.8}, {-40105.5, 112253.0}, {83208.4, -191237.7}, {0.81498, 2.57476}, {0.0069274, 0.0302047},
+    {1.010344, 0.000899}, {1.308162, -0.005538}, {2096.55, 1463.75}, {-10114.06, -44631.0}, {22933.66, 230960.0},
+    {-14621.7, -377812.9}, {97.8975, -42.6597}, {-3.28270, -9.05138}, {-2.51564e-5, 1.97503e-5}, {43.3151, 638.633},
+    {-0.0702021, -0.162698}, {9.59881, -397.054}, {-0.0298949, 1.40221}, {0.997441, -0.00788445}};
+
+bool is_gw(int kind) { return kind == NSGW_LIKE_GW_TAYLORF2 || kind == NSGW_LIKE_GW_PHENOMD_FORM; }
+
+int ensure_cb(ns_handle* h, long long B) {
+  if (B > h->cb_cap) {
+    if (h->d_cb) cudaFree(h->d_cb);
+    h->d_cb = nullptr; h->cb_cap = 0;
+    CU_CHECK(h, cudaMalloc(&h->d_cb, sizeof(double) * CB_SIZE * (size_t)B));
+    h->cb_cap = B;
+  }
+  return 0;
+}
+int ensure_theta(ns_handle* h, long long B) {
+  if (B > h->theta_cap) {
+    if (h->d_theta) cudaFree(h->d_theta);
+    h->d_theta = nullptr; h->theta_cap = 0;
+    CU_CHECK(h, cudaMalloc(&h->d_theta, sizeof(double) * 16 * (size_t)B));
+    h->theta_cap = B;
+  }
+  return 0;
+}
+
+// particles per CTA of the bin loop as a function of the batch (fill 148 SMs first, then reuse table loads)
+int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
+
+template <int MODEL, int NDET>
+int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
+  int P = pick_p(B);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof && h->prof_ev.size() < 4096) {
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, s);
+  }
+  if (P == 2) {
+    k_bins<MODEL, NDET, 2><<<(unsigned)((B + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, logl, parts);
+  } else {
+    k_bins<MODEL, NDET, 1><<<(unsigned)B, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, logl, parts);
+  }
+  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
+  LAUNCH_CHECK(h);
+  return 0;
+}
+template <int MODEL>
+int launch_bins(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
+  switch (h->cfg.n_det) {
+    case 1: return launch_bins_nd<MODEL, 1>(h, B, logl, parts, s);
+    case 2: return launch_bins_nd<MODEL, 2>(h, B, logl, parts, s);
+    case 3: return launch_bins_nd<MODEL, 3>(h, B, logl, parts, s);
+    default: return fail(h, -5, "n_det must be 1..3 for the GW kernels");
+  }
+}
+
+int loglike_theta(ns_handle* h, const double* theta_dev, long long B, double* logl, double* parts, cudaStream_t s) {
+  if (B == 0) return 0;
+  int rc = ensure_cb(h, B);
+  if (rc) return rc;
+  unsigned g = (unsigned)((B + 127) / 128);
+  if (h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2) {
+    k_setup<1><<<g, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+    LAUNCH_CHECK(h);
+    return launch_bins<1>(h, B, logl, parts, s);
+  }
+  k_setup<2><<<g, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+  LAUNCH_CHECK(h);
+  return launch_bins<2>(h, B, logl, parts, s);
+}
+
+int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cudaStream_t s) {
+  if (B == 0) return 0;
+  if (!is_gw(h->cfg.like_kind)) {
+    k_loglike_simple<<<(unsigned)((B + 127) / 128), 128, 0, s>>>(h->d_cfg, u_dev, B, logl);
+    LAUNCH_CHECK(h);
+    return 0;
+  }
+  int rc = ensure_theta(h, B);
+  if (rc) return rc;
+  long long N = B * h->cfg.ndim;
+  k_prior_transform<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(h->d_cfg, u_dev, B, h->d_theta);
+  LAUNCH_CHECK(h);
+  return loglike_theta(h, h->d_theta, B, logl, nullptr, s);
+}
+
+template <int MODEL, int NDET>
+int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
+  // P walkers per CTA: 1 keeps all SMs busy for the k = 500..700 batches of a real run; 2 halves table traffic for big sweeps
+  if (a.B >= 2048) {
+    k_walk_gw<MODEL, NDET, 2><<<(unsigned)((a.B + 1) / 2), kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
+  } else {
+    k_walk_gw<MODEL, NDET, 1><<<(unsigned)a.B, kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
+  }
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+int launch_walk(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
+  if (a.B == 0) return 0;
+  if (!is_gw(h->cfg.like_kind)) {
+    k_walk_simple<<<(unsigned)((a.B + 63) / 64), 64, 0, s>>>(h->d_cfg, a);
+    LAUNCH_CHECK(h);
+    return 0;
+  }
+  const int nd = h->cfg.n_det;
+  if (h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2) {
+    if (nd == 1) return launch_walk_gw<1, 1>(h, a, s);
+    if (nd == 2) return launch_walk_gw<1, 2>(h, a, s);
+    if (nd == 3) return launch_walk_gw<1, 3>(h, a, s);
+  } else {
+    if (nd == 1) return launch_walk_gw<2, 1>(h, a, s);
+    if (nd == 2) return launch_walk_gw<2, 2>(h, a, s);
+    if (nd == 3) return launch_walk_gw<2, 3>(h, a, s);
+  }
+  return fail(h, -5, "n_det must be 1..3 for the GW kernels");
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ns_last_error(const ns_handle* h) { return h ? h->err.c_str() : g_init_error.c_str(); }
+
+int64_t nsgw_launch_count(void) { return g_launches.load(); }
+
+void ns_free(ns_handle* h) {
+  if (!h) return;
+  cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_wd); cudaFree(h->d_ws);
+  cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
+  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_theta); cudaFree(h->d_fin);
+  if (h->h_stats) cudaFreeHost(h->h_stats);
+  if (h->h_fin) cudaFreeHost(h->h_fin);
+  for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  delete h;
+}
+
+int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, const double* strain_dev, const double* psd_dev,
+            uint64_t seed, void* stream) {
+  if (!out || !cfg) return fail(nullptr, -1, "null argument");
+  *out = nullptr;
+  if (cfg->struct_version != NSGW_STRUCT_VERSION) return fail(nullptr, -1, "struct_version mismatch");
+  if (cfg->ndim < 1 || cfg->ndim > NSGW_MAX_DIM) return fail(nullptr, -1, "ndim out of range");
+  if (cfg->like_kind < 0 || cfg->like_kind > 3) return fail(nullptr, -5, "unknown like_kind");
+  const bool gw = is_gw(cfg->like_kind);
+  if (gw && cfg->ndim != 11) return fail(nullptr, -5, "GW likelihoods need ndim = 11");
+  if (gw && (cfg->n_det < 1 || cfg->n_det > 3)) return fail(nullptr, -5, "GW kernels are built for n_det = 1..3");
+  if (gw && (cfg->n_freq < 1 || !(cfg->df > 0.0) || !(cfg->f_min > 0.0))) return fail(nullptr, -1, "bad frequency grid");
+  if (gw && (!strain_dev || !psd_dev)) return fail(nullptr, -1, "GW likelihoods need strain and PSD");
+  if (cfg->n_live < 0) return fail(nullptr, -1, "n_live < 0");
+  if (cfg->n_live > 0) {
+    if (cfg->n_delete < 1 || cfg->n_delete > cfg->n_live - 2) return fail(nullptr, -1, "need 1 <= n_delete <= n_live - 2");
+    if (cfg->naccept < 1 || cfg->maxmcmc < 1 || !(cfg->walks0 >= 1.0)) return fail(nullptr, -1, "bad naccept/maxmcmc/walks0");
+  }
+  int n_free = 0;
+  for (int d = 0; d < cfg->ndim; ++d) {
+    if (cfg->prior_kind[d] < 0 || cfg->prior_kind[d] > 4) return fail(nullptr, -1, "bad prior kind");
+    if (cfg->prior_kind[d] != NSGW_PRIOR_FIXED) {
+      ++n_free;
+      if (!(cfg->prior_hi[d] > cfg->prior_lo[d])) return fail(nullptr, -1, "prior hi must exceed lo");
+    }
+  }
+  if (n_free == 0) return fail(nullptr, -1, "no free dimension");
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(nullptr, -2, "no CUDA device (there is no CPU fallback)");
+
+  cudaStream_t s = (cudaStream_t)stream;
+  ns_handle* h = new ns_handle();
+  h->cfg = *cfg;
+  h->cfg.phenom_table_host = nullptr;
+  h->seed = seed;
+  h->n_free = n_free;
+  auto bail = [&](int rc) { g_init_error = h->err; ns_free(h); return rc; };
+
+  // ---- device config
+  DevCfg hc;
+  memset(&hc, 0, sizeof(hc));
+  hc.like_kind = cfg->like_kind; hc.ndim = cfg->ndim; hc.n_free = n_free; hc.n_det = gw ? cfg->n_det : 0; hc.n_freq = gw ? cfg->n_freq : 0;
+  for (int d = 0; d < cfg->ndim; ++d) {
+    hc.prior_kind[d] = cfg->prior_kind[d]; hc.periodic[d] = cfg->periodic[d];
+    hc.prior_lo[d] = cfg->prior_lo[d]; hc.prior_hi[d] = cfg->prior_hi[d];
+    hc.toy_mean[d] = cfg->toy_mean[d];
+  }
+  for (int i = 0; i < cfg->ndim * cfg->ndim; ++i) hc.toy_prec[i] = cfg->toy_prec[i];
+  hc.toy_lognorm = cfg->toy_lognorm;
+  hc.f_min = cfg->f_min; hc.df = cfg->df; hc.gmst = cfg->gmst;
+  for (int d = 0; d < hc.n_det; ++d) {
+    const double* x = cfg->det_xarm[d];
+    const double* y = cfg->det_yarm[d];
+    for (int j = 0; j < 3; ++j) hc.det_vertex[d][j] = cfg->det_vertex[d][j];
+    int idx = 0;
+    for (int i = 0; i < 3; ++i)
+      for (int j = i; j < 3; ++j) hc.det_D[d][idx++] = 0.5 * (x[i] * x[j] - y[i] * y[j]);
+  }
+  for (int r = 0; r < 19; ++r)
+    for (int c = 0; c < 11; ++c)
+      hc.table[r][c] = cfg->phenom_table_host ? cfg->phenom_table_host[r * 11 + c] : (c < 2 ? kSurrogate[r][c] : 0.0);
+  if (cudaMalloc(&h->d_cfg, sizeof(DevCfg)) != cudaSuccess) { h->err = "cudaMalloc cfg"; return bail(-4); }
+  if (cudaMemcpyAsync(h->d_cfg, &hc, sizeof(DevCfg), cudaMemcpyHostToDevice, s) != cudaSuccess) { h->err = "H2D cfg"; return bail(-2); }
+
+#define INIT_CHECK(expr, code)                                                        \
+  do {                                                                                \
+    cudaError_t e_ = (expr);                                                          \
+    if (e_ != cudaSuccess) { h->err = std::string(#expr) + ": " + cudaGetErrorString(e_); return bail(e_ == cudaErrorMemoryAllocation ? -4 : code); } \
+  } while (0)
+
+  // ---- GW tables
+  if (gw) {
+    const size_t nf = cfg->n_freq, nd = cfg->n_det;
+    // validate PSD on the host side of the boundary is impossible without a copy; do it on a host copy (init-time only)
+    {
+      std::vector<double> hp(nf * nd);
+      INIT_CHECK(cudaMemcpyAsync(hp.data(), psd_dev, sizeof(double) * nf * nd, cudaMemcpyDeviceToHost, s), -2);
+      INIT_CHECK(cudaStreamSynchronize(s), -2);
+      for (double v : hp)
+        if (!(v > 0.0) || !std::isfinite(v)) { h->err = "PSD values must be positive and finite"; return bail(-1); }
+    }
+    INIT_CHECK(cudaMalloc(&h->d_tab, sizeof(double) * 5 * nf), -2);
+    INIT_CHECK(cudaMalloc(&h->d_wd, sizeof(double2) * nd * nf), -2);
+    INIT_CHECK(cudaMalloc(&h->d_ws, sizeof(double) * nd * nf), -2);
+    h->tb.f = h->d_tab; h->tb.y = h->d_tab + nf; h->tb.L = h->d_tab + 2 * nf; h->tb.x = h->d_tab + 3 * nf; h->tb.f34 = h->d_tab + 4 * nf;
+    for (size_t d = 0; d < nd; ++d) { h->tb.wd[d] = h->d_wd + d * nf; h->tb.ws[d] = h->d_ws + d * nf; }
+    k_tables<<<(unsigned)((nf + 255) / 256), 256, 0, s>>>(h->d_cfg, strain_dev, psd_dev, h->d_tab, h->d_tab + nf, h->d_tab + 2 * nf,
+                                                          h->d_tab + 3 * nf, h->d_tab + 4 * nf, h->d_wd, h->d_ws);
+    g_launches.fetch_add(1);
+    k_i73<<<1, 256, 0, s>>>(h->d_cfg, h->d_ws);
+    g_launches.fetch_add(1);
+    INIT_CHECK(cudaGetLastError(), -2);
+  }
+
+  // ---- sampler state
+  INIT_CHECK(cudaMalloc(&h->d_state, sizeof(DevState)), -2);
+  INIT_CHECK(cudaMalloc(&h->d_fin, sizeof(double) * 2), -2);
+  INIT_CHECK(cudaMallocHost(&h->h_stats, sizeof(ns_stats)), -2);
+  INIT_CHECK(cudaMallocHost(&h->h_fin, sizeof(double) * 2), -2);
+  const int n = cfg->n_live, k = cfg->n_delete, D = cfg->ndim;
+  DevState hs;
+  memset(&hs, 0, sizeof(hs));
+  hs.logx = 0.0; hs.logz = -INFINITY; hs.h = 0.0; hs.walks = cfg->walks0;
+  hs.delay = (n > 0) ? (cfg->delay >= 0.0 ? cfg->delay : std::max((double)n / (10.0 * k) - 1.0, 0.0)) : 0.0;
+  hs.iter = 0; hs.n_eval_total = n; hs.W = 1; hs.naccept = cfg->naccept; hs.maxmcmc = cfg->maxmcmc;
+  INIT_CHECK(cudaMemcpyAsync(h->d_state, &hs, sizeof(hs), cudaMemcpyHostToDevice, s), -2);
+  if (n > 0) {
+    INIT_CHECK(cudaMalloc(&h->d_live_u, sizeof(double) * (size_t)n * D), -2);
+    INIT_CHECK(cudaMalloc(&h->d_live_l, sizeof(double) * (size_t)n), -2);
+    INIT_CHECK(cudaMalloc(&h->d_order, sizeof(int) * (size_t)n), -2);
+    INIT_CHECK(cudaMalloc(&h->d_surv, sizeof(double) * (size_t)(n - k) * D), -2);
+    INIT_CHECK(cudaMalloc(&h->d_cur_u, sizeof(double) * (size_t)k * D), -2);
+    INIT_CHECK(cudaMalloc(&h->d_cur_l, sizeof(double) * (size_t)k), -2);
+    INIT_CHECK(cudaMalloc(&h->d_cnt, sizeof(int) * 3 * (size_t)k), -2);
+    if (live_u_dev) {
+      INIT_CHECK(cudaMemcpyAsync(h->d_live_u, live_u_dev, sizeof(double) * (size_t)n * D, cudaMemcpyDeviceToDevice, s), -2);
+    } else {
+      k_draw_live<<<(n + 127) / 128, 128, 0, s>>>(D, n, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32), h->d_live_u);
+      g_launches.fetch_add(1);
+    }
+    int rc = loglike_u(h, h->d_live_u, n, h->d_live_l, s);
+    if (rc) return bail(rc);
+  }
+  INIT_CHECK(cudaStreamSynchronize(s), -2);
+  INIT_CHECK(cudaGetLastError(), -2);
+#undef INIT_CHECK
+  *out = h;
+  return 0;
+}
+
+int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (B < 0 || (B > 0 && (!theta_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  return loglike_theta(h, theta_dev, B, logl_dev, parts_dev, (cudaStream_t)stream);
+}
+
+int gw_waveform(ns_handle* h, const double* theta_dev, double* out_dev, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (!theta_dev || !out_dev) return fail(h, -1, "null argument");
+  cudaStream_t s = (cudaStream_t)stream;
+  unsigned g = (unsigned)((h->cfg.n_freq + 255) / 256);
+  if (h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2) k_waveform<1><<<g, 256, 0, s>>>(h->d_cfg, h->tb, theta_dev, out_dev);
+  else k_waveform<2><<<g, 256, 0, s>>>(h->d_cfg, h->tb, theta_dev, out_dev);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+int ns_prior_transform_batch(ns_handle* h, const double* u_dev, int64_t B, double* theta_dev, void* stream) {
+  if (!h) return -3;
+  if (B < 0 || (B > 0 && (!u_dev || !theta_dev))) return fail(h, -1, "bad arguments");
+  if (B == 0) return 0;
+  long long N = B * h->cfg.ndim;
+  k_prior_transform<<<(unsigned)((N + 255) / 256), 256, 0, (cudaStream_t)stream>>>(h->d_cfg, u_dev, B, theta_dev);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+int ns_loglike_u_batch(ns_handle* h, const double* u_dev, int64_t B, double* logl_dev, void* stream) {
+  if (!h) return -3;
+  if (B < 0 || (B > 0 && (!u_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  return loglike_u(h, u_dev, B, logl_dev, (cudaStream_t)stream);
+}
+
+int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u_dev, double* logl_dev, int64_t B, double logl_star,
+                  int32_t walk_len, uint64_t seed, uint32_t stream_id, int64_t slot0, int32_t* n_accept_dev, int32_t* n_eval_dev,
+                  int32_t* n_oob_dev, uint8_t* trace_flags_dev, double* trace_logl_dev, void* stream) {
+  if (!h) return -3;
+  if (B < 0 || m < 2 || walk_len < 1 || !donors_u_dev || (B > 0 && (!u_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  WalkArgs a;
+  memset(&a, 0, sizeof(a));
+  a.donors = donors_u_dev; a.m = m; a.u = u_dev; a.logl = logl_dev; a.B = B; a.lstar = logl_star; a.W = walk_len;
+  a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32); a.stream_id = stream_id; a.slot0 = slot0;
+  a.n_accept = n_accept_dev; a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.tflags = trace_flags_dev; a.tlogl = trace_logl_dev;
+  a.trace_stride = walk_len;
+  return launch_walk(h, a, (cudaStream_t)stream);
+}
+
+int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) {
+  if (!h) return -3;
+  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int n = h->cfg.n_live, k = h->cfg.n_delete, D = h->cfg.ndim, m = n - k;
+  const uint32_t k0 = (uint32_t)(h->seed & 0xFFFFFFFFull), k1 = (uint32_t)(h->seed >> 32);
+  k_rank<<<(n + 255) / 256, 256, 0, s>>>(h->d_live_l, n, h->d_order);
+  LAUNCH_CHECK(h);
+  k_evidence<<<1, 32, 0, s>>>(h->d_state, h->d_live_l, h->d_live_u, h->d_order, n, k, D, dead_dev);
+  LAUNCH_CHECK(h);
+  k_gather_start<<<(std::max(m, k) + 127) / 128, 128, 0, s>>>(h->d_state, h->d_live_u, h->d_live_l, h->d_order, n, k, D, k0, k1, h->d_surv,
+                                                            h->d_cur_u, h->d_cur_l);
+  LAUNCH_CHECK(h);
+  WalkArgs a;
+  memset(&a, 0, sizeof(a));
+  a.donors = h->d_surv; a.m = m; a.u = h->d_cur_u; a.logl = h->d_cur_l; a.B = k;
+  a.lstar_dev = &h->d_state->lstar; a.W_dev = &h->d_state->W; a.iter_dev = &h->d_state->iter;
+  a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
+  a.n_accept = h->d_cnt; a.n_eval = h->d_cnt + k; a.n_oob = h->d_cnt + 2 * k;
+  int rc = launch_walk(h, a, s);
+  if (rc) return rc;
+  k_writeback<<<(k + 127) / 128, 128, 0, s>>>(h->d_order, k, D, h->d_cur_u, h->d_cur_l, h->d_live_u, h->d_live_l);
+  LAUNCH_CHECK(h);
+  k_adapt<<<1, 256, 0, s>>>(h->d_state, h->d_cnt, h->d_cnt + k, h->d_cnt + 2 * k, k, h->d_live_l, n);
+  LAUNCH_CHECK(h);
+  if (stats_host) {
+    CU_CHECK(h, cudaMemcpyAsync(h->h_stats, &h->d_state->stats, sizeof(ns_stats), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(h, cudaStreamSynchronize(s));
+    *stats_host = *h->h_stats;
+  }
+  return 0;
+}
+
+int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host, double* dead_dev, void* stream) {
+  if (!h) return -3;
+  if (term_kind < 0 || term_kind > 1 || max_iter < 0) return fail(h, -1, "bad arguments");
+  const size_t stride = (size_t)h->cfg.n_delete * (h->cfg.ndim + 3);
+  ns_stats st;
+  memset(&st, 0, sizeof(st));
+  int64_t it = 0;
+  while (it < max_iter) {
+    int rc = ns_step(h, &st, dead_dev ? dead_dev + it * stride : nullptr, stream);
+    if (rc) return rc;
+    ++it;
+    if (term_kind == 0 && st.dlogz < term_tol) break;
+    if (term_kind == 1 && st.live_frac_log < std::log(term_tol)) break;
+  }
+  if (last_host) *last_host = st;
+  return it;
+}
+
+int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream) {
+  if (!h) return -3;
+  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
+  cudaStream_t s = (cudaStream_t)stream;
+  const size_t n = h->cfg.n_live, D = h->cfg.ndim;
+  if (u_dev) CU_CHECK(h, cudaMemcpyAsync(u_dev, h->d_live_u, sizeof(double) * n * D, cudaMemcpyDeviceToDevice, s));
+  if (logl_dev) CU_CHECK(h, cudaMemcpyAsync(logl_dev, h->d_live_l, sizeof(double) * n, cudaMemcpyDeviceToDevice, s));
+  return 0;
+}
+
+int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host, double* h_host, void* stream) {
+  if (!h) return -3;
+  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int n = h->cfg.n_live, k = h->cfg.n_delete;
+  k_rank<<<(n + 255) / 256, 256, 0, s>>>(h->d_live_l, n, h->d_order);
+  LAUNCH_CHECK(h);
+  k_finalize<<<1, 32, 0, s>>>(h->d_state, h->d_live_l, h->d_order, n, h->d_fin);
+  LAUNCH_CHECK(h);
+  CU_CHECK(h, cudaMemcpyAsync(h->h_fin, h->d_fin, sizeof(double) * 2, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(h, cudaStreamSynchronize(s));
+  const double neff = k / std::log((double)n / (double)(n - k));
+  if (logz_host) *logz_host = h->h_fin[0];
+  if (h_host) *h_host = h->h_fin[1];
+  if (logz_err_host) *logz_err_host = std::sqrt(std::max(h->h_fin[1], 0.0) / neff);
+  return 0;
+}
+
+int nsgw_profile_enable(ns_handle* h, int32_t on) {
+  if (!h) return -3;
+  h->prof = on != 0;
+  return 0;
+}
+
+int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_host) {
+  if (!h || !total_ms_host || !launches_host) return -1;
+  double tot = 0.0;
+  for (auto& pr : h->prof_ev) {
+    if (cudaEventSynchronize(pr.second) != cudaSuccess) return fail(h, -2, "event sync");
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, pr.first, pr.second);
+    tot += ms;
+    cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+  }
+  *total_ms_host = tot;
+  *launches_host = (int64_t)h->prof_ev.size();
+  h->prof_ev.clear();
+  return 0;
+}
+
+int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream) {
+  if (iters < 1 || !tflops_host) return -1;
+  cudaStream_t s = (cudaStream_t)stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return -2;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  double* sink = nullptr;
+  if (cudaMalloc(&sink, 8) != cudaSuccess) return -4;
+  const int threads = 256, blocks = sms * 8;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  k_dfma_probe<<<blocks, threads, 0, s>>>(iters / 8 + 1, sink);   // warm-up
+  cudaEventRecord(e0, s);
+  k_dfma_probe<<<blocks, threads, 0, s>>>(iters, sink);
+  cudaEventRecord(e1, s);
+  g_launches.fetch_add(2);
+  cudaError_t e = cudaEventSynchronize(e1);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+  if (e != cudaSuccess) return -2;
+  *tflops_host = 2.0 * 8.0 * (double)iters * threads * blocks / (ms * 1e-3) / 1e12;
+  return 0;
+}
+
+}  // extern "C"

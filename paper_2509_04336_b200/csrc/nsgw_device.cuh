@@ -1,0 +1,475 @@
+// nsgw_device.cuh -- device-side building blocks of libnsgw (sm_100a, fp64 ALU path; no tensor cores: the
+// per-(particle, bin) work is a transcendental-heavy map + reduction, not a dense contraction).
+//
+// Contents: Philox4x32-10 and the uniform/index draws of the RNG contract, prior transforms
+// (Table 1), quarter-turn sincos, detector response (DESIGN.md A.3), per-particle waveform set-up
+// (DESIGN.md A.1/A.2) and the per-bin evaluation used by both the likelihood kernel and the walk kernel.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace nsgw {
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kGMsunS = 4.925490947641267e-6;                     // G Msun / c^3 [s]
+constexpr double kMpcS = 3.0856775814913673e22 / 299792458.0;        // 1 Mpc / c [s]
+constexpr double kC = 299792458.0;
+constexpr double kEulerGamma = 0.5772156649015329;
+constexpr double kQT = 2.0 / kPi;                                    // radians -> quarter turns
+
+constexpr int kMaxDim = 16;
+constexpr int kMaxDet = 4;
+
+// Device copy of the problem description (lives in global memory, one per handle).
+struct DevCfg {
+  int like_kind, ndim, n_free, n_det, n_freq;
+  int prior_kind[kMaxDim];
+  int periodic[kMaxDim];
+  double prior_lo[kMaxDim], prior_hi[kMaxDim];
+  double f_min, df, gmst;
+  double det_vertex[kMaxDet][3];
+  double det_D[kMaxDet][6];  // detector tensor (xx, xy, xz, yy, yz, zz) of D = (x x^T - y y^T)/2
+  double toy_mean[kMaxDim];
+  double toy_prec[kMaxDim * kMaxDim];
+  double toy_lognorm;
+  double table[19][11];
+  double i73[kMaxDet];       // 4 df sum_k f_k^-7/3 / S_k  (parameter-independent part of <h,h> for a power-law amplitude)
+};
+
+// Per-frequency tables built once by ns_init (SoA, length n_freq).
+struct Tables {
+  const double* f;      // f_k
+  const double* y;      // f^-1/3
+  const double* L;      // ln f
+  const double* x;      // f^1/3
+  const double* f34;    // f^3/4
+  const double2* wd[kMaxDet];  // 4 df d_k f_k^-7/6 / S_k   (complex)
+  const double* ws[kMaxDet];   // 4 df f_k^-7/3 / S_k
+};
+
+// ------------------------------------------------------------------------------------------------------
+// Philox4x32-10, counter (c0 block, c1 step, c2 slot, c3 stream id), key = seed.
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0, uint32_t k1,
+                                              uint32_t (&out)[4]) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// Uniform on the half-offset 2^-52 grid, strictly inside (0,1).
+__device__ __forceinline__ double u01(uint32_t hi, uint32_t lo) {
+  return ((double)(hi >> 6) * 67108864.0 + (double)(lo >> 6) + 0.5) * (1.0 / 4503599627370496.0);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// sin/cos of an angle given in quarter turns (q = angle * 2/pi).  Exact reduction: k = rint(q), r = q - k in
+// [-1/2, 1/2]; polynomials in r^2 fitted to sin(pi r/2)/r and cos(pi r/2) (max error 5e-18 / 3e-20).
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void sincos_qt(double q, double& s, double& c) {
+  const double magic = 6755399441055744.0;  // 1.5 * 2^52
+  double kk = q + magic;
+  int ki = __double2loint(kk);
+  kk -= magic;
+  double r = q - kk;
+  double z = r * r;
+  double ps = 5.633936132273839028e-8;
+  ps = fma(ps, z, -3.5986433706134925899e-6);
+  ps = fma(ps, z, 0.00016044115074714990863);
+  ps = fma(ps, z, -0.0046817541323416188617);
+  ps = fma(ps, z, 0.079692626246043040805);
+  ps = fma(ps, z, -0.64596409750624431654);
+  ps = fma(ps, z, 1.5707963267948966143);
+  ps *= r;
+  double pc = -6.3212589210323875261e-9;
+  pc = fma(pc, z, 4.710609744708126973e-7);
+  pc = fma(pc, z, -0.000025202036771077321298);
+  pc = fma(pc, z, 0.00091926027418326090632);
+  pc = fma(pc, z, -0.020863480763311218307);
+  pc = fma(pc, z, 0.25366950790104670948);
+  pc = fma(pc, z, -1.2337005501361698118);
+  pc = fma(pc, z, 1.0);
+  if (ki & 1) { double t = ps; ps = pc; pc = -t; }
+  if (ki & 2) { ps = -ps; pc = -pc; }
+  s = ps; c = pc;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Prior transform of one coordinate (Table 1; d_L^2 power law P:182).
+// ------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double prior_transform_dim(int kind, double lo, double hi, double u) {
+  if (kind == 0) return lo + (hi - lo) * u;
+  if (kind == 1) { double a3 = lo * lo * lo, b3 = hi * hi * hi; return cbrt(a3 + u * (b3 - a3)); }
+  if (kind == 2) { double cl = cos(lo), ch = cos(hi); return acos(cl - u * (cl - ch)); }
+  if (kind == 3) { double sl = sin(lo), sh = sin(hi); return asin(sl + u * (sh - sl)); }
+  return lo;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Coefficient block of one particle (doubles).  Written by setup_particle, read by the bin loop.
+// ------------------------------------------------------------------------------------------------------
+enum {
+  CB_VALID = 0,
+  CB_DET = 1,        // per detector, stride 4: Cr, Ci (A0 * C_det), dtq (-4 dt_det: quarter turns per Hz), c2 (|A0 C_det|^2)
+  CB_PH = 17,        // TaylorF2 / inspiral phase: y5 y3 y2 y 1 L x xL x2 f | fx fx2 ff   (13)
+  CB_PB = 30,        // intermediate phase: 1 L f f^-3                                   (4)
+  CB_PM = 34,        // merger-ringdown phase: 1 f 1/f f^3/4 | atan coefficient, f0, 1/fd  (7)
+  CB_FP1 = 41, CB_FP2 = 42, CB_FA1 = 43, CB_FA2 = 44,   // region boundaries [Hz]
+  CB_AI = 45,        // inspiral amplitude: degree-9 polynomial in x = f^1/3              (10)
+  CB_AH = 55,        // intermediate amplitude: f1, 1/(f3-f1), quartic h0..h4             (7)
+  CB_AM = 62,        // merger-ringdown amplitude: f_rd, g1, wh^2, -gamma2/wh             (4)
+  CB_SIZE = 68
+};
+
+struct DetResp { double fp, fx, dt; };
+
+__device__ __forceinline__ DetResp detector_response(const DevCfg& cfg, int det, double sg, double cg, double sd, double cd,
+                                                     double sp, double cp) {
+  // polarisation basis X, Y and propagation direction n (DESIGN.md A.3), g = gmst - ra
+  double X0 = -cp * sg - sp * cg * sd, X1 = -cp * cg + sp * sg * sd, X2 = sp * cd;
+  double Y0 = sp * sg - cp * cg * sd, Y1 = sp * cg + cp * sg * sd, Y2 = cp * cd;
+  const double* D = cfg.det_D[det];
+  // D X and D Y with the symmetric tensor (xx xy xz yy yz zz)
+  double DX0 = D[0] * X0 + D[1] * X1 + D[2] * X2, DX1 = D[1] * X0 + D[3] * X1 + D[4] * X2, DX2 = D[2] * X0 + D[4] * X1 + D[5] * X2;
+  double DY0 = D[0] * Y0 + D[1] * Y1 + D[2] * Y2, DY1 = D[1] * Y0 + D[3] * Y1 + D[4] * Y2, DY2 = D[2] * Y0 + D[4] * Y1 + D[5] * Y2;
+  DetResp r;
+  r.fp = (X0 * DX0 + X1 * DX1 + X2 * DX2) - (Y0 * DY0 + Y1 * DY1 + Y2 * DY2);
+  r.fx = 2.0 * (X0 * DY0 + X1 * DY1 + X2 * DY2);
+  const double* v = cfg.det_vertex[det];
+  r.dt = -(v[0] * cd * cg - v[1] * cd * sg + v[2] * sd) / kC;
+  return r;
+}
+
+// 3.5PN aligned-spin TaylorF2 phase coefficients phi_k, phi_k^(l) (DESIGN.md A.1).
+__device__ __forceinline__ void pn_phase_coeffs(double eta, double delta, double chis, double chia, double (&ph)[8], double& c5,
+                                                double& p6l) {
+  const double pi = kPi, e2 = eta * eta, e3 = e2 * eta;
+  ph[0] = 1.0; ph[1] = 0.0;
+  ph[2] = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
+  ph[3] = -16.0 * pi + 113.0 / 3.0 * delta * chia + (113.0 / 3.0 - 76.0 / 3.0 * eta) * chis;
+  ph[4] = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * e2 + (-405.0 / 8.0 + 200.0 * eta) * chia * chia -
+          405.0 / 4.0 * delta * chia * chis + (-405.0 / 8.0 + 2.5 * eta) * chis * chis;
+  c5 = 38645.0 / 756.0 * pi - 65.0 / 9.0 * pi * eta + delta * (-732985.0 / 2268.0 - 140.0 / 9.0 * eta) * chia +
+       (-732985.0 / 2268.0 + 24260.0 / 81.0 * eta + 340.0 / 9.0 * e2) * chis;
+  ph[5] = c5;
+  ph[6] = 11583231236531.0 / 4694215680.0 - 6848.0 / 21.0 * kEulerGamma - 640.0 / 3.0 * pi * pi +
+          (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi * pi) * eta + 76055.0 / 1728.0 * e2 - 127825.0 / 1296.0 * e3 -
+          6848.0 / 63.0 * 4.1588830833596715 /* ln 64 */ + 2270.0 / 3.0 * pi * delta * chia + (2270.0 / 3.0 * pi - 520.0 * pi * eta) * chis;
+  p6l = -6848.0 / 21.0;
+  ph[7] = 77096675.0 / 254016.0 * pi + 378515.0 / 1512.0 * pi * eta - 74045.0 / 756.0 * pi * e2 +
+          delta * (-25150083775.0 / 3048192.0 + 26804935.0 / 6048.0 * eta - 1985.0 / 48.0 * e2) * chia +
+          (-25150083775.0 / 3048192.0 + 10566655595.0 / 762048.0 * eta - 1042165.0 / 3024.0 * e2 + 5345.0 / 36.0 * e3) * chis;
+}
+
+// Per-particle set-up: theta[11] -> coefficient block cb[CB_SIZE] (generic pointer: shared or global).
+// Returns false (and sets cb[CB_VALID] = 0) for unphysical theta (logL = -inf).
+template <int MODEL>
+__device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) {
+  const double Mc = th[0], q = th[1], chi1 = th[2], chi2 = th[3], dL = th[4], iota = th[5], psi = th[6], phic = th[7], tc = th[8],
+               ra = th[9], dec = th[10];
+  bool ok = true;
+#pragma unroll
+  for (int i = 0; i < 11; ++i) ok = ok && isfinite(th[i]);
+  ok = ok && (Mc > 0.0) && (q > 0.0) && (q <= 1.0) && (fabs(chi1) <= 1.0) && (fabs(chi2) <= 1.0) && (dL > 0.0);
+  if (!ok) { cb[CB_VALID] = 0.0; return false; }
+  cb[CB_VALID] = 1.0;
+
+  const double eta = q / ((1.0 + q) * (1.0 + q));
+  const double M = Mc * kGMsunS * pow(eta, -0.6);
+  const double m1 = M / (1.0 + q), m2 = M * q / (1.0 + q);
+  const double delta = (m1 - m2) / M;
+  const double chis = 0.5 * (chi1 + chi2), chia = 0.5 * (chi1 - chi2);
+
+  // ---- extrinsic: detector projections -------------------------------------------------------------
+  double sg, cg, sd, cd, sp, cp;
+  sincos(cfg.gmst - ra, &sg, &cg);
+  sincos(dec, &sd, &cd);
+  sincos(psi, &sp, &cp);
+  const double ci = cos(iota);
+  const double A0 = sqrt(5.0 / 24.0) * pow(kPi, -2.0 / 3.0) * pow(Mc * kGMsunS, 5.0 / 6.0) / (dL * kMpcS);
+  for (int d = 0; d < cfg.n_det; ++d) {
+    DetResp r = detector_response(cfg, d, sg, cg, sd, cd, sp, cp);
+    double cr = A0 * r.fp * 0.5 * (1.0 + ci * ci), cim = -A0 * r.fx * ci;
+    cb[CB_DET + 4 * d + 0] = cr;
+    cb[CB_DET + 4 * d + 1] = cim;
+    cb[CB_DET + 4 * d + 2] = -4.0 * r.dt;
+    cb[CB_DET + 4 * d + 3] = cr * cr + cim * cim;
+  }
+
+  // ---- intrinsic phase: PN part in the basis y5 y3 y2 y 1 L x xL x2 f ---------------------------------
+  double ph[8], c5, p6l;
+  pn_phase_coeffs(eta, delta, chis, chia, ph, c5, p6l);
+  const double cv = cbrt(kPi * M), lncv = log(cv);
+  const double K = 3.0 / (128.0 * eta);
+  const double cv2 = cv * cv;
+  const double e5 = K, e4 = K / cv, e3 = K / cv2, e2 = e3 / cv, e0 = e2 / cv2, e6 = K * cv, e7 = K * cv2;
+  double a[13];
+  a[0] = e0 * ph[0];
+  a[1] = e2 * ph[2];
+  a[2] = e3 * ph[3];
+  a[3] = e4 * ph[4];
+  a[4] = -0.25 * kPi - 2.0 * phic + e5 * (c5 + 3.0 * c5 * lncv);
+  a[5] = e5 * c5;                       // phi5^(l)/3 = c5
+  a[6] = e6 * (ph[6] + p6l * lncv);
+  a[7] = e6 * p6l / 3.0;
+  a[8] = e7 * ph[7];
+  a[9] = 2.0 * kPi * tc;
+  a[10] = a[11] = a[12] = 0.0;
+
+  if (MODEL == 1) {
+#pragma unroll
+    for (int i = 0; i < 13; ++i) cb[CB_PH + i] = a[i] * kQT;
+    return true;
+  }
+
+  // ---- PhenomD-form (DESIGN.md A.2) ------------------------------------------------------------------
+  double Lm[19];
+  {
+    const double chieff = (m1 * chi1 + m2 * chi2) / M;
+    const double xi = chieff - 38.0 / 113.0 * eta * (chi1 + chi2) - 1.0;
+    const double e2_ = eta * eta, xi2 = xi * xi, xi3 = xi2 * xi;
+    for (int r = 0; r < 19; ++r) {
+      const double* t = cfg.table[r];
+      Lm[r] = t[0] + t[1] * eta + xi * (t[2] + t[3] * eta + t[4] * e2_) + xi2 * (t[5] + t[6] * eta + t[7] * e2_) +
+              xi3 * (t[8] + t[9] * eta + t[10] * e2_);
+    }
+  }
+  const double rho1 = Lm[0], rho2 = Lm[1], rho3 = Lm[2], v2 = Lm[3], gam1 = Lm[4], gam2 = Lm[5], gam3 = Lm[6];
+  const double sig1 = Lm[7], sig2 = Lm[8], sig3 = Lm[9], sig4 = Lm[10], bet1 = Lm[11], bet2 = Lm[12], bet3 = Lm[13];
+  const double alp1 = Lm[14], alp2 = Lm[15], alp3 = Lm[16], alp4 = Lm[17], alp5 = Lm[18];
+  // final state and ringdown frequencies (surrogate fits)
+  const double eta2 = eta * eta, eta3 = eta2 * eta;
+  const double S = (m1 * m1 * chi1 + m2 * m2 * chi2) / (M * M);
+  double af = 2.0 * sqrt(3.0) * eta - 3.871 * eta2 + 4.028 * eta3 + S;
+  af = fmin(0.99, fmax(-0.99, af));
+  const double Erad = 0.05597 * eta + 0.5810 * eta2 - 0.9607 * eta3 + 3.352 * eta2 * eta2;
+  const double Frd = (1.5251 - 1.1568 * pow(1.0 - af, 0.1292)) / (2.0 * kPi * (1.0 - Erad));
+  const double Qf = 0.7 + 1.4187 * pow(1.0 - af, -0.4990);
+  const double Fdamp = Frd / (2.0 * Qf);
+  const double wF = gam3 * Fdamp;
+  double Fpeak;
+  if (gam2 < 1.0) Fpeak = fabs(Frd + wF * (sqrt(1.0 - gam2 * gam2) - 1.0) / gam2);
+  else Fpeak = fabs(Frd - wF / gam2);
+
+  // -- phase pieces in F = M f and their connection (C0/C1 at 0.018 and Frd/2, analytic derivatives) --
+  const double ieta = 1.0 / eta;
+  auto pn_phase = [&](double F, double& val, double& der) {
+    double v = cbrt(kPi * F), lv = log(v);
+    double vk[8];
+    vk[0] = 1.0;
+#pragma unroll
+    for (int k = 1; k < 8; ++k) vk[k] = vk[k - 1] * v;
+    double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      double pl = (k == 5) ? 3.0 * c5 : ((k == 6) ? p6l : 0.0);
+      double t = ph[k] + pl * lv;
+      s0 += t * vk[k];
+      s1 += ((k - 5.0) * t + pl) * vk[k];
+    }
+    double v5 = vk[5];
+    val = -0.25 * kPi + K * s0 / v5;
+    der = K * s1 / (v5 * v) * v / (3.0 * F);
+  };
+  auto ins_phase = [&](double F, double& val, double& der) {
+    pn_phase(F, val, der);
+    double F13 = cbrt(F), F23 = F13 * F13;
+    val += ieta * (sig1 * F + 0.75 * sig2 * F * F13 + 0.6 * sig3 * F * F23 + 0.5 * sig4 * F * F);
+    der += ieta * (sig1 + sig2 * F13 + sig3 * F23 + sig4 * F);
+  };
+  auto int_phase = [&](double F, double& val, double& der) {
+    double iF = 1.0 / F, iF3 = iF * iF * iF;
+    val = ieta * (bet1 * F + bet2 * log(F) - bet3 * iF3 / 3.0);
+    der = ieta * (bet1 + bet2 * iF + bet3 * iF3 * iF);
+  };
+  auto mr_phase = [&](double F, double& val, double& der) {
+    double yy = (F - alp5 * Frd) / Fdamp;
+    double F14 = sqrt(sqrt(F));
+    val = ieta * (alp1 * F - alp2 / F + 4.0 / 3.0 * alp3 * F14 * F14 * F14 + alp4 * atan(yy));
+    der = ieta * (alp1 + alp2 / (F * F) + alp3 / F14 + alp4 / (Fdamp * (1.0 + yy * yy)));
+  };
+  double vi, di, vb, db, vm, dm;
+  const double Fa = 0.018, Fb = 0.5 * Frd;
+  ins_phase(Fa, vi, di);
+  int_phase(Fa, vb, db);
+  const double C2i = di - db, C1i = vi - vb - C2i * Fa;
+  int_phase(Fb, vb, db);
+  mr_phase(Fb, vm, dm);
+  const double C2m = (db + C2i) - dm, C1m = (vb + C1i + C2i * Fb) - vm - C2m * Fb;
+  mr_phase(Fpeak, vm, dm);
+  const double t0 = dm + C2m;
+
+  const double M13 = cbrt(M), M23 = M13 * M13;
+  a[4] = -0.25 * kPi - 2.0 * phic + e5 * (c5 + 3.0 * c5 * lncv);
+  a[9] = 2.0 * kPi * tc + (sig1 * ieta - t0) * M;
+  a[10] = 0.75 * sig2 * ieta * M * M13;
+  a[11] = 0.6 * sig3 * ieta * M * M23;
+  a[12] = 0.5 * sig4 * ieta * M * M;
+#pragma unroll
+  for (int i = 0; i < 13; ++i) cb[CB_PH + i] = a[i] * kQT;
+  cb[CB_PB + 0] = (bet2 * ieta * log(M) + C1i - 2.0 * phic) * kQT;
+  cb[CB_PB + 1] = bet2 * ieta * kQT;
+  cb[CB_PB + 2] = ((bet1 * ieta + C2i - t0) * M + 2.0 * kPi * tc) * kQT;
+  cb[CB_PB + 3] = -bet3 * ieta / (3.0 * M * M * M) * kQT;
+  const double M34 = sqrt(sqrt(M * M * M));
+  cb[CB_PM + 0] = (C1m - 2.0 * phic) * kQT;
+  cb[CB_PM + 1] = ((alp1 * ieta + C2m - t0) * M + 2.0 * kPi * tc) * kQT;
+  cb[CB_PM + 2] = -alp2 * ieta / M * kQT;
+  cb[CB_PM + 3] = 4.0 / 3.0 * alp3 * ieta * M34 * kQT;
+  cb[CB_PM + 4] = alp4 * ieta * kQT;
+  cb[CB_PM + 5] = alp5 * Frd / M;
+  cb[CB_PM + 6] = M / Fdamp;
+  cb[CB_FP1] = Fa / M;
+  cb[CB_FP2] = Fb / M;
+  cb[CB_FA1] = 0.014 / M;
+  cb[CB_FA2] = Fpeak / M;
+
+  // -- amplitude --------------------------------------------------------------------------------------
+  double A[7];
+  A[0] = 1.0; A[1] = 0.0;
+  A[2] = -323.0 / 224.0 + 451.0 / 168.0 * eta;
+  A[3] = (27.0 / 8.0 - 11.0 / 6.0 * eta) * chis + 27.0 / 8.0 * delta * chia;
+  A[4] = -27312085.0 / 8128512.0 - 1975055.0 / 338688.0 * eta + 105271.0 / 24192.0 * eta2 + (-81.0 / 32.0 + 8.0 * eta) * chia * chia -
+         81.0 / 16.0 * delta * chia * chis + (-81.0 / 32.0 + 17.0 / 8.0 * eta) * chis * chis;
+  A[5] = -85.0 / 64.0 * kPi + 85.0 / 16.0 * kPi * eta + (285197.0 / 16128.0 - 1579.0 / 4032.0 * eta) * delta * chia +
+         (285197.0 / 16128.0 - 15317.0 / 672.0 * eta - 2227.0 / 1008.0 * eta2) * chis;
+  A[6] = -177520268561.0 / 8583708672.0 + (545384828789.0 / 5007163392.0 - 205.0 / 48.0 * kPi * kPi) * eta -
+         3248849057.0 / 178827264.0 * eta2 + 34473079.0 / 6386688.0 * eta3 +
+         (1614569.0 / 64512.0 - 1873643.0 / 16128.0 * eta + 2167.0 / 42.0 * eta2) * chia * chia +
+         (31.0 / 12.0 * kPi - 7.0 / 3.0 * kPi * eta) * chis + (1614569.0 / 64512.0 - 61391.0 / 1344.0 * eta + 57451.0 / 4032.0 * eta2) * chis * chis +
+         delta * chia * (31.0 / 12.0 * kPi + (1614569.0 / 32256.0 - 165961.0 / 2688.0 * eta) * chis);
+  // inspiral amplitude as a degree-9 polynomial in x = f^1/3: (pi F)^(i/3) = (cv x)^i, F^(7/3) = M^(7/3) x^7, ...
+  double ai[10];
+  {
+    double cvp = 1.0;
+#pragma unroll
+    for (int i = 0; i < 7; ++i) { ai[i] = A[i] * cvp; cvp *= cv; }
+    const double M2 = M * M;
+    ai[7] = rho1 * M2 * M13;
+    ai[8] = rho2 * M2 * M23;
+    ai[9] = rho3 * M2 * M;
+#pragma unroll
+    for (int i = 0; i < 10; ++i) cb[CB_AI + i] = ai[i];
+  }
+  // value and slope (per unit F) of the inspiral amplitude at F1 = 0.014
+  const double F1 = 0.014;
+  double v1, d1;
+  {
+    double x1 = cbrt(F1 / M);  // x at the junction: f^1/3
+    double p = 0.0, dp = 0.0;
+#pragma unroll
+    for (int i = 9; i >= 0; --i) { dp = dp * x1 + p; p = p * x1 + ai[i]; }
+    v1 = p;
+    d1 = dp * x1 / (3.0 * F1);   // dA/dF = dA/dx * x/(3 f) / M, with f = F1/M
+  }
+  // merger-ringdown amplitude at its peak
+  double v3, d3;
+  {
+    double xx = Fpeak - Frd;
+    double lor = gam1 * wF / (xx * xx + wF * wF);
+    v3 = lor * exp(-gam2 * xx / wF);
+    d3 = v3 * (-2.0 * xx / (xx * xx + wF * wF) - gam2 / wF);
+  }
+  {
+    const double Lw = Fpeak - F1;
+    const double t1 = Lw * d1, t3 = Lw * d3;
+    const double Bb = v2 - (0.5 * v1 + 0.125 * t1 + 0.5 * v3 - 0.125 * t3);
+    cb[CB_AH + 0] = F1 / M;
+    cb[CB_AH + 1] = M / Lw;
+    cb[CB_AH + 2] = v1;
+    cb[CB_AH + 3] = t1;
+    cb[CB_AH + 4] = -3.0 * v1 - 2.0 * t1 + 3.0 * v3 - t3 + 16.0 * Bb;
+    cb[CB_AH + 5] = 2.0 * v1 + t1 - 2.0 * v3 + t3 - 32.0 * Bb;
+    cb[CB_AH + 6] = 16.0 * Bb;
+  }
+  {
+    const double wh = wF / M;
+    cb[CB_AM + 0] = Frd / M;
+    cb[CB_AM + 1] = gam1 * wh / M;
+    cb[CB_AM + 2] = wh * wh;
+    cb[CB_AM + 3] = -gam2 / wh;
+  }
+  return true;
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Per-bin evaluation: common phase (quarter turns) and amplitude factor relative to A0 f^-7/6.
+// ------------------------------------------------------------------------------------------------------
+struct BinBasis {
+  double f, y, L, x, f34;
+  double y2, y3, y5, xL, x2;
+};
+
+__device__ __forceinline__ BinBasis make_basis(const Tables& tb, int k, bool phenom) {
+  BinBasis b;
+  b.f = __ldg(tb.f + k); b.y = __ldg(tb.y + k); b.L = __ldg(tb.L + k); b.x = __ldg(tb.x + k);
+  b.f34 = phenom ? __ldg(tb.f34 + k) : 0.0;
+  b.y2 = b.y * b.y; b.y3 = b.y2 * b.y; b.y5 = b.y3 * b.y2; b.xL = b.x * b.L; b.x2 = b.x * b.x;
+  return b;
+}
+
+__device__ __forceinline__ double phase_pn_qt(const double* a, const BinBasis& b) {
+  double q = fma(a[0], b.y5, a[4]);
+  q = fma(a[1], b.y3, q);
+  q = fma(a[2], b.y2, q);
+  q = fma(a[3], b.y, q);
+  q = fma(a[5], b.L, q);
+  q = fma(a[6], b.x, q);
+  q = fma(a[7], b.xL, q);
+  q = fma(a[8], b.x2, q);
+  q = fma(a[9], b.f, q);
+  return q;
+}
+
+// PhenomD-form: phase [quarter turns] and amplitude factor for one bin.
+__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, double& q, double& amp) {
+  const double f = b.f;
+  if (f < cb[CB_FP1]) {
+    const double* a = cb + CB_PH;
+    q = phase_pn_qt(a, b);
+    double fx = f * b.x;
+    q = fma(a[10], fx, q);
+    q = fma(a[11], fx * b.x, q);
+    q = fma(a[12], f * f, q);
+  } else if (f < cb[CB_FP2]) {
+    const double* p = cb + CB_PB;
+    double if3 = b.y3 * b.y3 * b.y3;
+    q = fma(p[1], b.L, p[0]);
+    q = fma(p[2], f, q);
+    q = fma(p[3], if3, q);
+  } else {
+    const double* p = cb + CB_PM;
+    q = fma(p[1], f, p[0]);
+    q = fma(p[2], b.y3, q);
+    q = fma(p[3], b.f34, q);
+    q = fma(p[4], atan((f - p[5]) * p[6]), q);
+  }
+  if (f < cb[CB_FA1]) {
+    const double* c = cb + CB_AI;
+    double p = c[9];
+#pragma unroll
+    for (int i = 8; i >= 0; --i) p = fma(p, b.x, c[i]);
+    amp = p;
+  } else if (f < cb[CB_FA2]) {
+    const double* c = cb + CB_AH;
+    double xh = (f - c[0]) * c[1];
+    double p = c[6];
+    p = fma(p, xh, c[5]);
+    p = fma(p, xh, c[4]);
+    p = fma(p, xh, c[3]);
+    p = fma(p, xh, c[2]);
+    amp = p;
+  } else {
+    const double* c = cb + CB_AM;
+    double fx = f - c[0];
+    amp = c[1] / fma(fx, fx, c[2]) * exp(c[3] * fx);
+  }
+}
+
+}  // namespace nsgw

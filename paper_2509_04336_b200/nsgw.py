@@ -1,0 +1,246 @@
+"""Thin Python binding of libnsgw.so (include/nsgw.h): argument marshalling only.
+
+torch is used for device memory and streams; every step of the hot path runs in the library's CUDA kernels.
+There is no CPU fallback: if the shared library is missing or no CUDA device is present, calls raise.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libnsgw.so")
+
+MAX_DIM, MAX_DET = 16, 4
+
+
+class NsConfig(C.Structure):
+    _fields_ = [
+        ("struct_version", C.c_int32), ("like_kind", C.c_int32), ("ndim", C.c_int32),
+        ("n_live", C.c_int32), ("n_delete", C.c_int32), ("naccept", C.c_int32), ("maxmcmc", C.c_int32),
+        ("walks0", C.c_double), ("delay", C.c_double),
+        ("prior_kind", C.c_int32 * MAX_DIM), ("prior_lo", C.c_double * MAX_DIM), ("prior_hi", C.c_double * MAX_DIM),
+        ("periodic", C.c_int32 * MAX_DIM),
+        ("n_det", C.c_int32), ("n_freq", C.c_int32), ("f_min", C.c_double), ("df", C.c_double),
+        ("det_vertex", (C.c_double * 3) * MAX_DET), ("det_xarm", (C.c_double * 3) * MAX_DET), ("det_yarm", (C.c_double * 3) * MAX_DET),
+        ("gmst", C.c_double),
+        ("toy_mean", C.c_double * MAX_DIM), ("toy_prec", C.c_double * (MAX_DIM * MAX_DIM)), ("toy_lognorm", C.c_double),
+        ("phenom_table_host", C.POINTER(C.c_double)),
+    ]
+
+
+class NsStats(C.Structure):
+    _fields_ = [
+        ("iteration", C.c_int64), ("logl_star", C.c_double), ("logx", C.c_double), ("logz", C.c_double), ("h", C.c_double),
+        ("dlogz", C.c_double), ("live_frac_log", C.c_double), ("walk_len", C.c_int32), ("pad0", C.c_int32),
+        ("walks_next", C.c_double), ("accept_mean", C.c_double), ("accept_min", C.c_int32), ("accept_max", C.c_int32),
+        ("n_eval", C.c_int64), ("n_oob", C.c_int64), ("n_stuck", C.c_int64), ("n_eval_total", C.c_int64),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad0"}
+
+
+EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_waveform", "ns_prior_transform_batch",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_get_live", "ns_finalize_evidence",
+           "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read"]
+
+_lib = None
+
+
+def lib():
+    """Loads libnsgw.so (fails loudly if it has not been built: run `python -m paper_2509_04336_b200.build`)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} is missing: build it with `python -m paper_2509_04336_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(_LIB_PATH)
+        L.ns_last_error.restype = C.c_char_p
+        L.ns_last_error.argtypes = [C.c_void_p]
+        L.ns_run.restype = C.c_int64
+        L.nsgw_launch_count.restype = C.c_int64
+        L.ns_free.restype = None
+        L.ns_free.argtypes = [C.c_void_p]
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    if t is None:
+        return C.c_void_p(0)
+    assert t.is_cuda and t.is_contiguous(), "device pointers must be contiguous CUDA tensors"
+    return C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _f64(x, device="cuda"):
+    return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64)).to(device)
+
+
+def make_config(spec, sampler=None):
+    """spec / sampler: plain dicts as produced by paper_2509_04336_b200.workloads."""
+    c = NsConfig()
+    c.struct_version = 1
+    c.like_kind = int(spec["like_kind"])
+    D = c.ndim = int(spec["ndim"])
+    s = sampler or {}
+    c.n_live = int(s.get("n_live", 0))
+    c.n_delete = int(s.get("n_delete", 0))
+    c.naccept = int(s.get("naccept", 60))
+    c.maxmcmc = int(s.get("maxmcmc", 5000))
+    c.walks0 = float(s.get("walks0", 100.0))
+    c.delay = float(s.get("delay", -1.0))
+    for d in range(D):
+        c.prior_kind[d] = int(spec["prior_kind"][d])
+        c.prior_lo[d] = float(spec["prior_lo"][d])
+        c.prior_hi[d] = float(spec["prior_hi"][d])
+        c.periodic[d] = int(spec["periodic"][d])
+    c.n_det = int(spec.get("n_det", 0))
+    c.n_freq = int(spec.get("n_freq", 0))
+    c.f_min = float(spec.get("f_min", 0.0))
+    c.df = float(spec.get("df", 0.0))
+    c.gmst = float(spec.get("gmst", 0.0))
+    for i in range(c.n_det):
+        for j in range(3):
+            c.det_vertex[i][j] = float(spec["det_vertex"][i][j])
+            c.det_xarm[i][j] = float(spec["det_xarm"][i][j])
+            c.det_yarm[i][j] = float(spec["det_yarm"][i][j])
+    if "toy_mean" in spec:
+        prec = np.asarray(spec["toy_prec"], dtype=np.float64).reshape(D, D)
+        for i in range(D):
+            c.toy_mean[i] = float(spec["toy_mean"][i])
+            for j in range(D):
+                c.toy_prec[i * D + j] = prec[i, j]
+        c.toy_lognorm = float(spec["toy_lognorm"])
+    keep = None
+    if spec.get("phenom_table") is not None:
+        keep = np.ascontiguousarray(spec["phenom_table"], dtype=np.float64).reshape(19 * 11)
+        c.phenom_table_host = keep.ctypes.data_as(C.POINTER(C.c_double))
+    return c, keep
+
+
+class NsgwError(RuntimeError):
+    pass
+
+
+class Handle:
+    """RAII wrapper of ns_handle.  All array arguments are CUDA float64 tensors unless stated."""
+
+    def __init__(self, spec, sampler=None, live_u=None, strain=None, psd=None, seed=1):
+        L = lib()
+        if not torch.cuda.is_available():
+            raise NsgwError("no CUDA device: libnsgw has no CPU fallback")
+        cfg, keep = make_config(spec, sampler)
+        self.cfg = cfg
+        self.ndim, self.n_det, self.n_freq = cfg.ndim, cfg.n_det, cfg.n_freq
+        self.n_live, self.n_delete = cfg.n_live, cfg.n_delete
+        self._h = C.c_void_p(0)
+        if strain is None and spec.get("strain") is not None:
+            strain = _f64(spec["strain"])
+        if psd is None and spec.get("psd") is not None:
+            psd = _f64(spec["psd"])
+        if live_u is not None and not torch.is_tensor(live_u):
+            live_u = _f64(live_u)
+        rc = L.ns_init(C.byref(self._h), C.byref(cfg), _ptr(live_u), _ptr(strain), _ptr(psd), C.c_uint64(seed), _stream())
+        if rc != 0:
+            raise NsgwError(f"ns_init failed ({rc}): {L.ns_last_error(None).decode()}")
+
+    def _check(self, rc, what):
+        if rc < 0:
+            raise NsgwError(f"{what} failed ({rc}): {lib().ns_last_error(self._h).decode()}")
+        return rc
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value and _lib is not None:
+            _lib.ns_free(self._h)
+            self._h = C.c_void_p(0)
+
+    __del__ = close
+
+    # ---- likelihood ------------------------------------------------------------------------------
+    def gw_loglike_batch(self, theta, parts=False, out=None, parts_out=None):
+        B = theta.shape[0]
+        logl = out if out is not None else torch.empty(B, dtype=torch.float64, device="cuda")
+        pr = parts_out if parts_out is not None else (torch.empty(B, 2 * self.n_det, dtype=torch.float64, device="cuda") if parts else None)
+        self._check(lib().gw_loglike_batch(self._h, _ptr(theta), C.c_int64(B), _ptr(logl), _ptr(pr), _stream()), "gw_loglike_batch")
+        return (logl, pr) if parts else logl
+
+    def gw_waveform(self, theta):
+        out = torch.empty(self.n_det, self.n_freq, 2, dtype=torch.float64, device="cuda")
+        self._check(lib().gw_waveform(self._h, _ptr(theta), _ptr(out), _stream()), "gw_waveform")
+        return out
+
+    def prior_transform_batch(self, u):
+        th = torch.empty_like(u)
+        self._check(lib().ns_prior_transform_batch(self._h, _ptr(u), C.c_int64(u.shape[0]), _ptr(th), _stream()), "ns_prior_transform_batch")
+        return th
+
+    def loglike_u_batch(self, u):
+        logl = torch.empty(u.shape[0], dtype=torch.float64, device="cuda")
+        self._check(lib().ns_loglike_u_batch(self._h, _ptr(u), C.c_int64(u.shape[0]), _ptr(logl), _stream()), "ns_loglike_u_batch")
+        return logl
+
+    # ---- walk --------------------------------------------------------------------------------------
+    def walk_batch(self, donors_u, u, logl, logl_star, walk_len, seed, stream_id, slot0=0, trace=False, counters=True):
+        """In place on u / logl.  Returns dict of counters (+ trace)."""
+        B = u.shape[0]
+        na = torch.zeros(B, dtype=torch.int32, device="cuda") if counters else None
+        ne = torch.zeros(B, dtype=torch.int32, device="cuda") if counters else None
+        no = torch.zeros(B, dtype=torch.int32, device="cuda") if counters else None
+        fl = torch.zeros(B, walk_len, dtype=torch.uint8, device="cuda") if trace else None
+        tl = torch.zeros(B, walk_len, dtype=torch.float64, device="cuda") if trace else None
+        self._check(lib().ns_walk_batch(self._h, _ptr(donors_u), C.c_int32(donors_u.shape[0]), _ptr(u), _ptr(logl), C.c_int64(B),
+                                        C.c_double(logl_star), C.c_int32(walk_len), C.c_uint64(seed), C.c_uint32(stream_id),
+                                        C.c_int64(slot0), _ptr(na), _ptr(ne), _ptr(no), _ptr(fl), _ptr(tl), _stream()), "ns_walk_batch")
+        out = dict(n_accept=na, n_eval=ne, n_oob=no)
+        if trace:
+            out["flags"], out["trace_logl"] = fl, tl
+        return out
+
+    # ---- sampler -----------------------------------------------------------------------------------
+    def step(self, want_stats=True, dead=None):
+        st = NsStats()
+        self._check(lib().ns_step(self._h, C.byref(st) if want_stats else None, _ptr(dead), _stream()), "ns_step")
+        return st.as_dict() if want_stats else None
+
+    def run(self, term_kind, term_tol, max_iter, dead=None):
+        st = NsStats()
+        n = self._check(lib().ns_run(self._h, C.c_int32(term_kind), C.c_double(term_tol), C.c_int64(max_iter), C.byref(st), _ptr(dead),
+                                     _stream()), "ns_run")
+        return int(n), st.as_dict()
+
+    def get_live(self):
+        u = torch.empty(self.n_live, self.ndim, dtype=torch.float64, device="cuda")
+        l = torch.empty(self.n_live, dtype=torch.float64, device="cuda")
+        self._check(lib().ns_get_live(self._h, _ptr(u), _ptr(l), _stream()), "ns_get_live")
+        return u, l
+
+    def profile_enable(self, on=True):
+        self._check(lib().nsgw_profile_enable(self._h, C.c_int32(1 if on else 0)), "nsgw_profile_enable")
+
+    def profile_read(self):
+        ms, n = C.c_double(), C.c_int64()
+        self._check(lib().nsgw_profile_read(self._h, C.byref(ms), C.byref(n)), "nsgw_profile_read")
+        return ms.value, n.value
+
+    def finalize_evidence(self):
+        a, b, c = C.c_double(), C.c_double(), C.c_double()
+        self._check(lib().ns_finalize_evidence(self._h, C.byref(a), C.byref(b), C.byref(c), _stream()), "ns_finalize_evidence")
+        return a.value, b.value, c.value
+
+
+def measure_fp64_peak(iters=1 << 18):
+    t = C.c_double()
+    rc = lib().nsgw_measure_fp64_peak(C.c_int64(iters), C.byref(t), _stream())
+    if rc != 0:
+        raise NsgwError(f"nsgw_measure_fp64_peak failed ({rc})")
+    return t.value
+
+
+def launch_count():
+    return int(lib().nsgw_launch_count())
