@@ -36,18 +36,35 @@ def alg_flops_per_bin(n_det, model="taylorf2"):
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    """Samples SM clock and throttle reasons while the timed region runs (NVML every 20 ms; nvidia-smi as a fallback)."""
 
     def __init__(self, index=0):
-        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.samples, self.reasons, self.max_mhz, self.how = [], set(), None, None
         self._stop = threading.Event()
         self.index = index
         self._t = threading.Thread(target=self._run, daemon=True)
 
-    def _run(self):
+    def _run_nvml(self):
+        import pynvml as N
+        N.nvmlInit()
+        h = N.nvmlDeviceGetHandleByIndex(self.index)
+        self.max_mhz = float(N.nvmlDeviceGetMaxClockInfo(h, N.NVML_CLOCK_SM))
+        bits = {"hw_slowdown": N.nvmlClocksThrottleReasonHwSlowdown, "hw_thermal_slowdown": N.nvmlClocksThrottleReasonHwThermalSlowdown,
+                "sw_thermal_slowdown": N.nvmlClocksThrottleReasonSwThermalSlowdown, "sw_power_cap": N.nvmlClocksThrottleReasonSwPowerCap}
+        self.how = "nvml"
+        while not self._stop.is_set():
+            self.samples.append(float(N.nvmlDeviceGetClockInfo(h, N.NVML_CLOCK_SM)))
+            r = N.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+            for n, b in bits.items():
+                if r & b:
+                    self.reasons.add(n)
+            self._stop.wait(0.02)
+
+    def _run_smi(self):
         q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        self.how = "nvidia-smi"
         while not self._stop.is_set():
             try:
                 out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
@@ -62,6 +79,12 @@ class ClockSampler:
                 pass
             self._stop.wait(0.1)
 
+    def _run(self):
+        try:
+            self._run_nvml()
+        except Exception:
+            self._run_smi()
+
     def __enter__(self):
         self._t.start()
         return self
@@ -72,7 +95,7 @@ class ClockSampler:
 
     def summary(self):
         return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+                "reasons": sorted(self.reasons), "samples": len(self.samples), "how": self.how}
 
 
 def measured_peaks():
@@ -93,7 +116,7 @@ def run_reference(args):
     P = O.OracleProblem(spec)
     cores = os.cpu_count()
     B = args.ref_batch
-    theta = P.prior_transform(W.uniforms(B, 11, 2))
+    theta = P.prior_transform(W.uniform_rows(0, B, 11, seed=2))
     for _ in range(args.warmup):
         P.gw_loglike(theta[: max(64, B // 8)])
     t0 = time.perf_counter()
@@ -117,22 +140,16 @@ def run_reference(args):
 # --------------------------------------------------------------------------------------------------------------
 def run_ours(args):
     import torch
-    import torch.distributed as dist
-    from paper_2509_04336_b200 import nsgw, workloads as W
+    from paper_2509_04336_b200 import dist as D, nsgw, workloads as W
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
+    rank, world, local = D.env()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    D.init("nccl", torch.device("cuda", local))
 
     def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
+        D.barrier("cuda")
 
     # ---- workload: config 2.  The injected signal comes from the CUDA library itself (gw_waveform).
     def wf_cuda(spec, th):
@@ -147,7 +164,8 @@ def run_ours(args):
     h = nsgw.Handle(spec)
     B = args.batch
     n_det, n_freq = spec["n_det"], spec["n_freq"]
-    u = torch.as_tensor(W.uniforms(B, 11, 2 + rank)).cuda()       # each rank: its own B rows (weak scaling, no collective)
+    # weak scaling, no data-path collective: rank r owns rows [r B, (r+1) B) of one index-keyed stream of unit-cube rows
+    u = torch.as_tensor(W.uniform_rows(rank * B, (rank + 1) * B, 11, seed=2)).cuda()
     theta = h.prior_transform_batch(u)
     logl = torch.empty(B, dtype=torch.float64, device="cuda")
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
@@ -173,23 +191,16 @@ def run_ours(args):
     h.profile_enable(False)
     launches = nsgw.launch_count() - n0
     ms = sum(a.elapsed_time(b) for a, b in ev)
-    t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms = float(t.item())
+    ms = D.max_over_ranks(ms, "cuda")
     value = world * B * args.steps / (ms * 1e-3)
     kern_ms, kern_n = h.profile_read()
 
-    # ---- end to end through the binding with HOST buffers: pinned theta -> H2D -> gw_loglike_batch -> D2H logL
+    # ---- end to end through the host-buffer C-ABI call: pinned theta -> H2D -> set-up + bin sweep -> D2H logL, all timed
     th_host = theta.cpu().pin_memory()
     out_host = torch.empty(B, dtype=torch.float64).pin_memory()
-    th_dev = torch.empty_like(theta)
 
     def e2e_step():
-        th_dev.copy_(th_host, non_blocking=True)
-        h.gw_loglike_batch(th_dev, out=logl)
-        out_host.copy_(logl, non_blocking=True)
-        torch.cuda.synchronize()
+        h.gw_loglike_batch_host(th_host, out_host)       # synchronises
 
     for _ in range(3):
         e2e_step()
@@ -198,11 +209,8 @@ def run_ours(args):
     for _ in range(args.steps):
         e2e_step()
     barrier()
-    e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_val = world * B * args.steps / float(t.item())
+    e2e_s = D.max_over_ranks(time.perf_counter() - t0, "cuda")
+    e2e_val = world * B * args.steps / e2e_s
     assert torch.equal(out_host, logl.cpu())
 
     line = None
@@ -280,8 +288,7 @@ def run_ours(args):
     if rank == 0:
         print(json.dumps(line), flush=True)
     h.close()
-    if world > 1:
-        dist.destroy_process_group()
+    D.finalize()
 
 
 def wf_cuda_for(nsgw, torch):

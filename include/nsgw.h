@@ -91,6 +91,11 @@ const char* ns_last_error(const ns_handle* h); /* h may be NULL: message of the 
  * <d,h>_det, <h,h>_det interleaved. */
 int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream);
 
+/* Same with HOST buffers (the end-to-end entry point bench.py's `e2e` leg times): theta_host [B, 11] -> H2D into handle-owned
+ * scratch -> the same kernels -> D2H into logl_host [B].  Pinned host memory makes the copies asynchronous; pageable works too.
+ * Synchronises before returning. */
+int gw_loglike_batch_host(ns_handle* h, const double* theta_host, int64_t B, double* logl_host, void* stream);
+
 /* Detector-frame signal of ONE parameter row on the handle's grid: out_dev [n_det, n_freq, 2] (R:L3). Used to build injections. */
 int gw_waveform(ns_handle* h, const double* theta_dev, double* out_dev, void* stream);
 

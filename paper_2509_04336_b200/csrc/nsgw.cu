@@ -683,6 +683,8 @@ struct ns_handle {
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
   long long theta_cap = 0;
+  double* d_hio = nullptr;      // host-entry scratch: theta [B,11] + logl [B]
+  long long hio_cap = 0;
   double* d_fin = nullptr;      // 2 doubles
   ns_stats* h_stats = nullptr;  // pinned
   double* h_fin = nullptr;      // pinned
@@ -845,7 +847,7 @@ void ns_free(ns_handle* h) {
   if (!h) return;
   cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
-  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_theta); cudaFree(h->d_fin);
+  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -986,6 +988,28 @@ int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* l
   if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
   if (B < 0 || (B > 0 && (!theta_dev || !logl_dev))) return fail(h, -1, "bad arguments");
   return loglike_theta(h, theta_dev, B, logl_dev, parts_dev, (cudaStream_t)stream);
+}
+
+int gw_loglike_batch_host(ns_handle* h, const double* theta_host, int64_t B, double* logl_host, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (B < 0 || (B > 0 && (!theta_host || !logl_host))) return fail(h, -1, "bad arguments");
+  if (B == 0) return 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (B > h->hio_cap) {
+    if (h->d_hio) cudaFree(h->d_hio);
+    h->d_hio = nullptr; h->hio_cap = 0;
+    CU_CHECK(h, cudaMalloc(&h->d_hio, sizeof(double) * 12 * (size_t)B));
+    h->hio_cap = B;
+  }
+  double* th = h->d_hio;
+  double* lg = h->d_hio + 11 * (size_t)B;
+  CU_CHECK(h, cudaMemcpyAsync(th, theta_host, sizeof(double) * 11 * (size_t)B, cudaMemcpyHostToDevice, s));
+  int rc = loglike_theta(h, th, B, lg, nullptr, s);
+  if (rc) return rc;
+  CU_CHECK(h, cudaMemcpyAsync(logl_host, lg, sizeof(double) * (size_t)B, cudaMemcpyDeviceToHost, s));
+  CU_CHECK(h, cudaStreamSynchronize(s));
+  return 0;
 }
 
 int gw_waveform(ns_handle* h, const double* theta_dev, double* out_dev, void* stream) {

@@ -42,7 +42,7 @@ class NsStats(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad0"}
 
 
-EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_waveform", "ns_prior_transform_batch",
+EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
            "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_get_live", "ns_finalize_evidence",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read"]
 
@@ -169,6 +169,15 @@ class Handle:
         pr = parts_out if parts_out is not None else (torch.empty(B, 2 * self.n_det, dtype=torch.float64, device="cuda") if parts else None)
         self._check(lib().gw_loglike_batch(self._h, _ptr(theta), C.c_int64(B), _ptr(logl), _ptr(pr), _stream()), "gw_loglike_batch")
         return (logl, pr) if parts else logl
+
+    def gw_loglike_batch_host(self, theta_host, out_host):
+        """theta_host [B, 11], out_host [B]: CPU float64 tensors (pinned for asynchronous copies).  Synchronises."""
+        assert (not theta_host.is_cuda) and (not out_host.is_cuda) and theta_host.is_contiguous() and out_host.is_contiguous()
+        assert theta_host.dtype == torch.float64 and out_host.dtype == torch.float64
+        B = theta_host.shape[0]
+        self._check(lib().gw_loglike_batch_host(self._h, C.c_void_p(theta_host.data_ptr()), C.c_int64(B),
+                                                C.c_void_p(out_host.data_ptr()), _stream()), "gw_loglike_batch_host")
+        return out_host
 
     def gw_waveform(self, theta):
         out = torch.empty(self.n_det, self.n_freq, 2, dtype=torch.float64, device="cuda")

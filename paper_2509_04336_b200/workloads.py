@@ -118,6 +118,20 @@ def uniforms(n, ndim, seed):
     return rng.random((n, ndim)) * (1.0 - 2e-12) + 1e-12
 
 
+def uniform_rows(lo, hi, ndim, seed):
+    """Rows lo..hi-1 of an index-keyed stream of unit-cube rows: row i is the same whatever range it is drawn in, so a
+    multi-GPU run that shards rows by global index sees exactly the rows of a single-GPU run (numpy Philox, counter
+    advanced to the row)."""
+    # numpy's Philox yields 4 doubles per counter step: start at the enclosing block boundary and slice
+    bg = np.random.Philox(key=seed)
+    first = (lo * ndim) // 4
+    bg.advance(first)
+    rng = np.random.Generator(bg)
+    skip = lo * ndim - 4 * first
+    flat = rng.random(skip + (hi - lo) * ndim)[skip:]
+    return flat.reshape(hi - lo, ndim) * (1.0 - 2e-12) + 1e-12
+
+
 # ------------------------------------------------------------------------------------------------------
 # BASELINE.json configs
 # ------------------------------------------------------------------------------------------------------
