@@ -45,13 +45,18 @@ struct DevState {
 // ======================================================================================================
 // ns_init kernels
 // ======================================================================================================
-__global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const double* __restrict__ psd, double* tf, double* ty,
-                         double* tL, double* tx, double* tf34, double2* wd, double* ws) {
+__global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const double* __restrict__ psd, double2* t01, double2* t23,
+                         double2* t45, double2* t67, double* tf, double* tf34, double2* wd, double* ws) {
   const int nf = cfg->n_freq, nd = cfg->n_det;
   for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nf; k += gridDim.x * blockDim.x) {
     double f = cfg->f_min + k * cfg->df;
-    double x = cbrt(f);
-    tf[k] = f; tx[k] = x; ty[k] = 1.0 / x; tL[k] = log(f); tf34[k] = sqrt(sqrt(f * f * f));
+    double x = cbrt(f), y = 1.0 / x, L = log(f);
+    double y2 = y * y, y3 = y2 * y;
+    t01[k] = make_double2(y3 * y2, y3);
+    t23[k] = make_double2(y2, y);
+    t45[k] = make_double2(L, x);
+    t67[k] = make_double2(x * L, x * x);
+    tf[k] = f; tf34[k] = sqrt(sqrt(f * f * f));
     double a76 = 1.0 / (f * sqrt(x));      // f^-7/6
     for (int d = 0; d < nd; ++d) {
       double S = psd[(size_t)d * nf + k];
@@ -112,17 +117,28 @@ __global__ void k_setup(const DevCfg* __restrict__ cfg, const double* __restrict
   setup_particle<MODEL>(*cfg, th, cbs + i * CB_SIZE);
 }
 
-// Start phasors: for particle p, detector d, thread t (bin t of the first sweep):
-//   R = (Cr + i Ci) * exp(i * dtq * f_t)  [quarter turns], built as lane-table x warp-table to keep it to one sincos per entry.
-// tabL[(p*NDET+d)*32 + lane] = exp(i dtq df lane); tabW[(p*NDET+d)*NW + w] = C * exp(i dtq (f_min + 32 w df)).
+// Number of per-thread partial sums of one particle: X0 = sum conj(wd_0) amp E (complex; detector 0 carries no phasor, its
+// C_0 is applied once after the reduction), dh_d for d >= 1, and for PhenomD-form hh_d = sum amp^2 ws_d for every detector.
+template <int MODEL, int NDET>
+struct AccLayout {
+  static constexpr int ND1 = NDET - 1;
+  static constexpr int kDh = 2;                          // dh_d at kDh + d - 1 (d >= 1)
+  static constexpr int kHh = 2 + ND1;                    // hh_d at kHh + d (PhenomD-form only)
+  static constexpr int N = 2 + ND1 + (MODEL == 2 ? NDET : 0);
+};
+
+// Start phasors of the detectors d >= 1: for particle p, thread t (bin t of the first sweep)
+//   R = (Cr + i Ci) * exp(i * dtq * f_t)  [dtq: quarter turns per Hz relative to detector 0],
+// built as lane-table x warp-table to keep it to one sincos per entry.
+// tabL[(p*ND1+d-1)*32 + lane] = exp(i dtq df lane); tabW[(p*ND1+d-1)*NW + w] = C * exp(i dtq (f_min + 32 w df)).
 template <int NDET, int P, int NT>
 __device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const double* cbs /*smem [P][CB_SIZE]*/, double2* tabL,
                                                     double2* tabW, double2* step) {
-  constexpr int NW = NT / 32;
-  constexpr int NE = P * NDET * (32 + NW + 1);
+  constexpr int NW = NT / 32, ND1 = NDET - 1;
+  constexpr int NE = P * ND1 * (32 + NW + 1);
   for (int e = threadIdx.x; e < NE; e += NT) {
     int pd = e / (32 + NW + 1), j = e % (32 + NW + 1);
-    int p = pd / NDET, d = pd % NDET;
+    int p = pd / ND1, d = pd % ND1 + 1;
     const double* cb = cbs + p * CB_SIZE;
     double dtq = cb[CB_DET + 4 * d + 2];
     double s, c;
@@ -141,27 +157,39 @@ __device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const dou
   }
 }
 
-// Bin loop for P particles held by this CTA.  Outputs per particle/detector partial sums (per thread) of
-//   dh = sum_k Re(conj(wd_k) * amp_k * E_k * R_k),  hh = sum_k amp_k^2 ws_k   (PhenomD only; TaylorF2 uses I_{7/3}).
+// Bin loop for P particles held by this CTA: thread t handles bins t, t + NT, ...; the table values of a bin are loaded once
+// and used for the P particles.  Per (particle, bin): common phase (9 FMA), one sincos, 4 FMA for detector 0, and for each
+// further detector a complex product with its phasor, 2 FMA and the phasor advance.
 template <int MODEL, int NDET, int P, int NT>
 __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                         const double2* tabW, const double2* step, const bool* active, double (&dh)[P][NDET],
-                                         double (&hh)[P][NDET]) {
-  constexpr int NW = NT / 32;
+                                         const double2* tabW, const double2* step, const bool* active,
+                                         double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
+  using AL = AccLayout<MODEL, NDET>;
+  constexpr int NW = NT / 32, ND1 = NDET - 1;
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-  double2 R[P][NDET], St[P][NDET];
+  double2 R[P][ND1 > 0 ? ND1 : 1], St[P][ND1 > 0 ? ND1 : 1];
+  double a[P][MODEL == 1 ? 10 : 1];
+  bool any = false;
 #pragma unroll
-  for (int p = 0; p < P; ++p)
+  for (int p = 0; p < P; ++p) {
+    any = any || active[p];
 #pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      double2 a = tabL[(p * NDET + d) * 32 + lane], b = tabW[(p * NDET + d) * NW + wrp];
-      R[p][d] = make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-      St[p][d] = step[p * NDET + d];
-      dh[p][d] = 0.0; hh[p][d] = 0.0;
+    for (int i = 0; i < AL::N; ++i) acc[p][i] = 0.0;
+#pragma unroll
+    for (int d = 0; d < ND1; ++d) {
+      double2 u = tabL[(p * ND1 + d) * 32 + lane], v = tabW[(p * ND1 + d) * NW + wrp];
+      R[p][d] = make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x);
+      St[p][d] = step[p * ND1 + d];
     }
+    if (MODEL == 1) {
+#pragma unroll
+      for (int i = 0; i < 10; ++i) a[p][i] = cbs[p * CB_SIZE + CB_PH + i];
+    }
+  }
+  if (!any) return;   // block-uniform: nothing to evaluate (all proposals of this CTA were out of bounds)
   const int nf = cfg.n_freq;
   for (int k = tid; k < nf; k += NT) {
-    BinBasis b = make_basis(tb, k, MODEL == 2);
+    const BinBasis b = make_basis(tb, k, MODEL == 2);
     double2 w[NDET];
     double wsv[NDET];
 #pragma unroll
@@ -171,27 +199,33 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
     }
 #pragma unroll
     for (int p = 0; p < P; ++p) {
-      if (!active[p]) continue;
-      const double* cb = cbs + p * CB_SIZE;
       double q, amp = 1.0;
-      if (MODEL == 1) q = phase_pn_qt(cb + CB_PH, b);
-      else phenom_bin(cb, b, q, amp);
-      double s, c;
-      sincos_qt(q, s, c);
-      double er = c, ei = -s;       // E = exp(-i Phi_c)
-      if (MODEL == 2) { er *= amp; ei *= amp; }
-      double a2 = amp * amp;
+      if (MODEL == 1) q = phase_pn_qt(a[p], b);
+      else phenom_bin(cbs + p * CB_SIZE, b, q, amp);
+      double sn, cs;
+      sincos_qt(q, sn, cs);
+      if (MODEL == 2) { sn *= amp; cs *= amp; }
+      // E = amp exp(-i Phi) = cs - i sn;  X0 += conj(wd_0) E
+      acc[p][0] = fma(w[0].x, cs, acc[p][0]);
+      acc[p][1] = fma(-w[0].x, sn, acc[p][1]);
+      acc[p][0] = fma(-w[0].y, sn, acc[p][0]);
+      acc[p][1] = fma(-w[0].y, cs, acc[p][1]);
+      if (MODEL == 2) {
+        const double a2 = amp * amp;
 #pragma unroll
-      for (int d = 0; d < NDET; ++d) {
-        double gr = er * R[p][d].x - ei * R[p][d].y;
-        double gi = er * R[p][d].y + ei * R[p][d].x;
-        dh[p][d] = fma(w[d].x, gr, dh[p][d]);
-        dh[p][d] = fma(w[d].y, gi, dh[p][d]);
-        if (MODEL == 2) hh[p][d] = fma(a2, wsv[d], hh[p][d]);
+        for (int d = 0; d < NDET; ++d) acc[p][AL::kHh + d] = fma(a2, wsv[d], acc[p][AL::kHh + d]);
+      }
+#pragma unroll
+      for (int d = 0; d < ND1; ++d) {
+        const double rx = R[p][d].x, ry = R[p][d].y;
+        // G = E R_d;  dh_d += Re(conj(wd_d) G)
+        const double gr = fma(cs, rx, sn * ry);
+        const double gi = fma(cs, ry, -(sn * rx));
+        acc[p][AL::kDh + d] = fma(w[d + 1].x, gr, acc[p][AL::kDh + d]);
+        acc[p][AL::kDh + d] = fma(w[d + 1].y, gi, acc[p][AL::kDh + d]);
         // advance the detector phasor by one sweep
-        double nr = R[p][d].x * St[p][d].x - R[p][d].y * St[p][d].y;
-        double ni = R[p][d].x * St[p][d].y + R[p][d].y * St[p][d].x;
-        R[p][d].x = nr; R[p][d].y = ni;
+        R[p][d].x = fma(rx, St[p][d].x, -(ry * St[p][d].y));
+        R[p][d].y = fma(rx, St[p][d].y, ry * St[p][d].x);
       }
     }
   }
@@ -222,9 +256,10 @@ __device__ __forceinline__ void block_reduce(double (&v)[NV], double* red /*smem
   __syncthreads();
 }
 
-// Finishes logL of particle p from reduced sums (out: [P][NDET][2] = dh, hh).
+// Finishes logL of one particle from its reduced sums (AccLayout order).
 template <int MODEL, int NDET>
 __device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* cb, const double* sums, double* parts) {
+  using AL = AccLayout<MODEL, NDET>;
   if (cb[CB_VALID] == 0.0) {
     if (parts) for (int d = 0; d < 2 * NDET; ++d) parts[d] = nan("");
     return -INFINITY;
@@ -232,8 +267,8 @@ __device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* c
   double logl = 0.0;
 #pragma unroll
   for (int d = 0; d < NDET; ++d) {
-    double dh = sums[2 * d];
-    double hh = (MODEL == 1) ? cb[CB_DET + 4 * d + 3] * cfg.i73[d] : cb[CB_DET + 4 * d + 3] * sums[2 * d + 1];
+    double dh = (d == 0) ? fma(cb[CB_DET], sums[0], -(cb[CB_DET + 1] * sums[1])) : sums[AL::kDh + d - 1];
+    double hh = (MODEL == 1) ? cb[CB_DET + 4 * d + 3] * cfg.i73[d] : cb[CB_DET + 4 * d + 3] * sums[AL::kHh + d];
     if (parts) { parts[2 * d] = dh; parts[2 * d + 1] = hh; }
     logl += dh - 0.5 * hh;
   }
@@ -241,11 +276,12 @@ __device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* c
 }
 
 template <int MODEL, int NDET, int P>
-__global__ void __launch_bounds__(kBinsThreads) k_bins(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
-                                                        long long B, double* logl, double* parts) {
-  constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * NDET * 2;
-  __shared__ double cbs[P * CB_SIZE];
-  __shared__ double2 tabL[P * NDET * 32], tabW[P * NDET * NW], step[P * NDET];
+__global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
+                                                           long long B, double* logl, double* parts) {
+  using AL = AccLayout<MODEL, NDET>;
+  constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
+  __shared__ __align__(16) double cbs[P * CB_SIZE];
+  __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
   __shared__ double red[NW * NV], out[NV];
   __shared__ bool active[P];
   const DevCfg& cfg = *cfgp;
@@ -258,17 +294,17 @@ __global__ void __launch_bounds__(kBinsThreads) k_bins(const DevCfg* __restrict_
   if (threadIdx.x < P) active[threadIdx.x] = cbs[threadIdx.x * CB_SIZE + CB_VALID] != 0.0;
   build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
   __syncthreads();
-  double dh[P][NDET], hh[P][NDET];
-  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, dh, hh);
+  double acc[P][AL::N];
+  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, acc);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < P; ++p)
 #pragma unroll
-    for (int d = 0; d < NDET; ++d) { v[(p * NDET + d) * 2] = dh[p][d]; v[(p * NDET + d) * 2 + 1] = hh[p][d]; }
+    for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
   block_reduce<NV, NT>(v, red, out);
   if (threadIdx.x < P && p0 + threadIdx.x < B) {
     int p = threadIdx.x;
-    logl[p0 + p] = finish_logl<MODEL, NDET>(cfg, cbs + p * CB_SIZE, out + p * NDET * 2, parts ? parts + (p0 + p) * 2 * NDET : nullptr);
+    logl[p0 + p] = finish_logl<MODEL, NDET>(cfg, cbs + p * CB_SIZE, out + p * AL::N, parts ? parts + (p0 + p) * 2 * NDET : nullptr);
   }
 }
 
@@ -414,9 +450,10 @@ __global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
 // (phase B), lanes 0..P-1 accept (phase C, merged with the next phase A).  All walkers do exactly W steps.
 template <int MODEL, int NDET, int P>
 __global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
-  constexpr int NT = kWalkThreads, NW = NT / 32, NV = P * NDET * 2;
-  __shared__ double cbs[P * CB_SIZE];
-  __shared__ double2 tabL[P * NDET * 32], tabW[P * NDET * NW], step[P * NDET];
+  using AL = AccLayout<MODEL, NDET>;
+  constexpr int NT = kWalkThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
+  __shared__ __align__(16) double cbs[P * CB_SIZE];
+  __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
   __shared__ double red[NW * NV], out[NV];
   __shared__ bool active[P];
   __shared__ double s_cur[P][kMaxDim], s_prop[P][kMaxDim], s_curl[P];
@@ -463,17 +500,17 @@ __global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restri
     build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
     __syncthreads();
     // ---- phase B: bins
-    double dh[P][NDET], hh[P][NDET];
-    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, dh, hh);
+    double acc[P][AL::N];
+    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, acc);
     double v[NV];
 #pragma unroll
     for (int p = 0; p < P; ++p)
 #pragma unroll
-      for (int d = 0; d < NDET; ++d) { v[(p * NDET + d) * 2] = dh[p][d]; v[(p * NDET + d) * 2 + 1] = hh[p][d]; }
+      for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
     block_reduce<NV, NT>(v, red, out);
     // ---- phase C: accept iff in bounds and logL' > L*
     if (owner && s_prop[tid][kMaxDim - 1] != 0.0) {
-      double pl = finish_logl<MODEL, NDET>(cfg, cbs + tid * CB_SIZE, out + tid * NDET * 2, nullptr);
+      double pl = finish_logl<MODEL, NDET>(cfg, cbs + tid * CB_SIZE, out + tid * AL::N, nullptr);
       uint8_t fl = 4;
       if (pl > lstar) {
         for (int d = 0; d < D; ++d) s_cur[tid][d] = s_prop[tid][d];
@@ -669,7 +706,7 @@ struct ns_handle {
   DevCfg* d_cfg = nullptr;
   DevState* d_state = nullptr;
   Tables tb{};
-  double* d_tab = nullptr;      // f, y, L, x, f34 (5 * nf)
+  double* d_tab = nullptr;      // four double2 pair tables, f, f34 (10 * nf doubles)
   double2* d_wd = nullptr;      // [n_det][nf]
   double* d_ws = nullptr;       // [n_det][nf]
   double* d_live_u = nullptr;   // [n_live][D]
@@ -934,13 +971,15 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
       for (double v : hp)
         if (!(v > 0.0) || !std::isfinite(v)) { h->err = "PSD values must be positive and finite"; return bail(-1); }
     }
-    INIT_CHECK(cudaMalloc(&h->d_tab, sizeof(double) * 5 * nf), -2);
+    INIT_CHECK(cudaMalloc(&h->d_tab, sizeof(double) * 10 * nf), -2);
     INIT_CHECK(cudaMalloc(&h->d_wd, sizeof(double2) * nd * nf), -2);
     INIT_CHECK(cudaMalloc(&h->d_ws, sizeof(double) * nd * nf), -2);
-    h->tb.f = h->d_tab; h->tb.y = h->d_tab + nf; h->tb.L = h->d_tab + 2 * nf; h->tb.x = h->d_tab + 3 * nf; h->tb.f34 = h->d_tab + 4 * nf;
+    double2* t2 = reinterpret_cast<double2*>(h->d_tab);
+    h->tb.t01 = t2; h->tb.t23 = t2 + nf; h->tb.t45 = t2 + 2 * nf; h->tb.t67 = t2 + 3 * nf;
+    h->tb.f = h->d_tab + 8 * nf; h->tb.f34 = h->d_tab + 9 * nf;
     for (size_t d = 0; d < nd; ++d) { h->tb.wd[d] = h->d_wd + d * nf; h->tb.ws[d] = h->d_ws + d * nf; }
-    k_tables<<<(unsigned)((nf + 255) / 256), 256, 0, s>>>(h->d_cfg, strain_dev, psd_dev, h->d_tab, h->d_tab + nf, h->d_tab + 2 * nf,
-                                                          h->d_tab + 3 * nf, h->d_tab + 4 * nf, h->d_wd, h->d_ws);
+    k_tables<<<(unsigned)((nf + 255) / 256), 256, 0, s>>>(h->d_cfg, strain_dev, psd_dev, t2, t2 + nf, t2 + 2 * nf, t2 + 3 * nf,
+                                                          h->d_tab + 8 * nf, h->d_tab + 9 * nf, h->d_wd, h->d_ws);
     g_launches.fetch_add(1);
     k_i73<<<1, 256, 0, s>>>(h->d_cfg, h->d_ws);
     g_launches.fetch_add(1);

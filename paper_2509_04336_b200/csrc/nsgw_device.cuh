@@ -36,12 +36,15 @@ struct DevCfg {
   double i73[kMaxDet];       // 4 df sum_k f_k^-7/3 / S_k  (parameter-independent part of <h,h> for a power-law amplitude)
 };
 
-// Per-frequency tables built once by ns_init (SoA, length n_freq).
+// Per-frequency tables built once by ns_init (length n_freq).  The ten basis functions of the PN phase are stored as
+// double2 pairs so that a thread fetches them with coalesced 128-bit loads and the bin loop has no pow/log/cbrt and no
+// per-bin products.
 struct Tables {
+  const double2* t01;   // (f^-5/3, f^-1)
+  const double2* t23;   // (f^-2/3, f^-1/3)
+  const double2* t45;   // (ln f, f^1/3)
+  const double2* t67;   // (f^1/3 ln f, f^2/3)
   const double* f;      // f_k
-  const double* y;      // f^-1/3
-  const double* L;      // ln f
-  const double* x;      // f^1/3
   const double* f34;    // f^3/4
   const double2* wd[kMaxDet];  // 4 df d_k f_k^-7/6 / S_k   (complex)
   const double* ws[kMaxDet];   // 4 df f_k^-7/3 / S_k
@@ -70,34 +73,48 @@ __device__ __forceinline__ double u01(uint32_t hi, uint32_t lo) {
 
 // ------------------------------------------------------------------------------------------------------
 // sin/cos of an angle given in quarter turns (q = angle * 2/pi).  Exact reduction: k = rint(q), r = q - k in
-// [-1/2, 1/2]; polynomials in r^2 fitted to sin(pi r/2)/r and cos(pi r/2) (max error 5e-18 / 3e-20).
+// [-1/2, 1/2]; polynomials in r^2 fitted to sin(pi r/2)/r and cos(pi r/2) (max error 5e-18 / 3e-20).  The coefficients
+// live in constant memory so that every DFMA takes its constant as a c[bank][offset] operand (a literal would cost two
+// UMOVs per use), and the quadrant fix-up is integer work on the sign/high words (no FP64 pipe slots).
 // ------------------------------------------------------------------------------------------------------
+__constant__ double kSinQ[7] = {1.5707963267948966143, -0.64596409750624431654, 0.079692626246043040805, -0.0046817541323416188617,
+                                0.00016044115074714990863, -3.5986433706134925899e-6, 5.633936132273839028e-8};
+__constant__ double kCosQ[8] = {1.0, -1.2337005501361698118, 0.25366950790104670948, -0.020863480763311218307,
+                                0.00091926027418326090632, -0.000025202036771077321298, 4.710609744708126973e-7,
+                                -6.3212589210323875261e-9};
+
 __device__ __forceinline__ void sincos_qt(double q, double& s, double& c) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52
   double kk = q + magic;
-  int ki = __double2loint(kk);
+  const int ki = __double2loint(kk);
   kk -= magic;
-  double r = q - kk;
-  double z = r * r;
-  double ps = 5.633936132273839028e-8;
-  ps = fma(ps, z, -3.5986433706134925899e-6);
-  ps = fma(ps, z, 0.00016044115074714990863);
-  ps = fma(ps, z, -0.0046817541323416188617);
-  ps = fma(ps, z, 0.079692626246043040805);
-  ps = fma(ps, z, -0.64596409750624431654);
-  ps = fma(ps, z, 1.5707963267948966143);
+  const double r = q - kk;
+  const double z = r * r;
+  double ps = kSinQ[6];
+  double pc = kCosQ[7];
+  pc = fma(pc, z, kCosQ[6]);
+  ps = fma(ps, z, kSinQ[5]);
+  pc = fma(pc, z, kCosQ[5]);
+  ps = fma(ps, z, kSinQ[4]);
+  pc = fma(pc, z, kCosQ[4]);
+  ps = fma(ps, z, kSinQ[3]);
+  pc = fma(pc, z, kCosQ[3]);
+  ps = fma(ps, z, kSinQ[2]);
+  pc = fma(pc, z, kCosQ[2]);
+  ps = fma(ps, z, kSinQ[1]);
+  pc = fma(pc, z, kCosQ[1]);
+  ps = fma(ps, z, kSinQ[0]);
+  pc = fma(pc, z, kCosQ[0]);
   ps *= r;
-  double pc = -6.3212589210323875261e-9;
-  pc = fma(pc, z, 4.710609744708126973e-7);
-  pc = fma(pc, z, -0.000025202036771077321298);
-  pc = fma(pc, z, 0.00091926027418326090632);
-  pc = fma(pc, z, -0.020863480763311218307);
-  pc = fma(pc, z, 0.25366950790104670948);
-  pc = fma(pc, z, -1.2337005501361698118);
-  pc = fma(pc, z, 1.0);
-  if (ki & 1) { double t = ps; ps = pc; pc = -t; }
-  if (ki & 2) { ps = -ps; pc = -pc; }
-  s = ps; c = pc;
+  // quadrant: k odd swaps; sin is negated for k = 2, 3 (mod 4), cos for k = 1, 2
+  const int slo = __double2loint(ps), shi = __double2hiint(ps), clo = __double2loint(pc), chi = __double2hiint(pc);
+  const bool sw = (ki & 1) != 0;
+  const int s_lo = sw ? clo : slo, c_lo = sw ? slo : clo;
+  int s_hi = sw ? chi : shi, c_hi = sw ? shi : chi;
+  s_hi ^= (ki & 2) << 30;
+  c_hi ^= ((ki + 1) & 2) << 30;
+  s = __hiloint2double(s_hi, s_lo);
+  c = __hiloint2double(c_hi, c_lo);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -116,7 +133,8 @@ __device__ __forceinline__ double prior_transform_dim(int kind, double lo, doubl
 // ------------------------------------------------------------------------------------------------------
 enum {
   CB_VALID = 0,
-  CB_DET = 1,        // per detector, stride 4: Cr, Ci (A0 * C_det), dtq (-4 dt_det: quarter turns per Hz), c2 (|A0 C_det|^2)
+  CB_DET = 1,        // per detector, stride 4: Cr, Ci (A0 * C_det), dtq (-4 (dt_det - dt_0): quarter turns per Hz relative to
+                     // detector 0, whose delay is folded into the f coefficient of the common phase), c2 (|A0 C_det|^2)
   CB_PH = 17,        // TaylorF2 / inspiral phase: y5 y3 y2 y 1 L x xL x2 f | fx fx2 ff   (13)
   CB_PB = 30,        // intermediate phase: 1 L f f^-3                                   (4)
   CB_PM = 34,        // merger-ringdown phase: 1 f 1/f f^3/4 | atan coefficient, f0, 1/fd  (7)
@@ -193,12 +211,14 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   sincos(psi, &sp, &cp);
   const double ci = cos(iota);
   const double A0 = sqrt(5.0 / 24.0) * pow(kPi, -2.0 / 3.0) * pow(Mc * kGMsunS, 5.0 / 6.0) / (dL * kMpcS);
+  double tc0 = tc, dt0 = 0.0;   // tc0 = tc + dt of detector 0: the common phase carries detector 0's arrival time
   for (int d = 0; d < cfg.n_det; ++d) {
     DetResp r = detector_response(cfg, d, sg, cg, sd, cd, sp, cp);
     double cr = A0 * r.fp * 0.5 * (1.0 + ci * ci), cim = -A0 * r.fx * ci;
+    if (d == 0) { dt0 = r.dt; tc0 = tc + dt0; }
     cb[CB_DET + 4 * d + 0] = cr;
     cb[CB_DET + 4 * d + 1] = cim;
-    cb[CB_DET + 4 * d + 2] = -4.0 * r.dt;
+    cb[CB_DET + 4 * d + 2] = -4.0 * (r.dt - dt0);
     cb[CB_DET + 4 * d + 3] = cr * cr + cim * cim;
   }
 
@@ -219,7 +239,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   a[6] = e6 * (ph[6] + p6l * lncv);
   a[7] = e6 * p6l / 3.0;
   a[8] = e7 * ph[7];
-  a[9] = 2.0 * kPi * tc;
+  a[9] = 2.0 * kPi * tc0;
   a[10] = a[11] = a[12] = 0.0;
 
   if (MODEL == 1) {
@@ -307,7 +327,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
 
   const double M13 = cbrt(M), M23 = M13 * M13;
   a[4] = -0.25 * kPi - 2.0 * phic + e5 * (c5 + 3.0 * c5 * lncv);
-  a[9] = 2.0 * kPi * tc + (sig1 * ieta - t0) * M;
+  a[9] = 2.0 * kPi * tc0 + (sig1 * ieta - t0) * M;
   a[10] = 0.75 * sig2 * ieta * M * M13;
   a[11] = 0.6 * sig3 * ieta * M * M23;
   a[12] = 0.5 * sig4 * ieta * M * M;
@@ -315,11 +335,11 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   for (int i = 0; i < 13; ++i) cb[CB_PH + i] = a[i] * kQT;
   cb[CB_PB + 0] = (bet2 * ieta * log(M) + C1i - 2.0 * phic) * kQT;
   cb[CB_PB + 1] = bet2 * ieta * kQT;
-  cb[CB_PB + 2] = ((bet1 * ieta + C2i - t0) * M + 2.0 * kPi * tc) * kQT;
+  cb[CB_PB + 2] = ((bet1 * ieta + C2i - t0) * M + 2.0 * kPi * tc0) * kQT;
   cb[CB_PB + 3] = -bet3 * ieta / (3.0 * M * M * M) * kQT;
   const double M34 = sqrt(sqrt(M * M * M));
   cb[CB_PM + 0] = (C1m - 2.0 * phic) * kQT;
-  cb[CB_PM + 1] = ((alp1 * ieta + C2m - t0) * M + 2.0 * kPi * tc) * kQT;
+  cb[CB_PM + 1] = ((alp1 * ieta + C2m - t0) * M + 2.0 * kPi * tc0) * kQT;
   cb[CB_PM + 2] = -alp2 * ieta / M * kQT;
   cb[CB_PM + 3] = 4.0 / 3.0 * alp3 * ieta * M34 * kQT;
   cb[CB_PM + 4] = alp4 * ieta * kQT;
@@ -408,12 +428,14 @@ struct BinBasis {
 
 __device__ __forceinline__ BinBasis make_basis(const Tables& tb, int k, bool phenom) {
   BinBasis b;
-  b.f = __ldg(tb.f + k); b.y = __ldg(tb.y + k); b.L = __ldg(tb.L + k); b.x = __ldg(tb.x + k);
+  const double2 a = __ldg(tb.t01 + k), c = __ldg(tb.t23 + k), e = __ldg(tb.t45 + k), g = __ldg(tb.t67 + k);
+  b.y5 = a.x; b.y3 = a.y; b.y2 = c.x; b.y = c.y; b.L = e.x; b.x = e.y; b.xL = g.x; b.x2 = g.y;
+  b.f = __ldg(tb.f + k);
   b.f34 = phenom ? __ldg(tb.f34 + k) : 0.0;
-  b.y2 = b.y * b.y; b.y3 = b.y2 * b.y; b.y5 = b.y3 * b.y2; b.xL = b.x * b.L; b.x2 = b.x * b.x;
   return b;
 }
 
+// PN phase in the tabulated basis: nine FMAs (independent particles held by the same thread supply the ILP).
 __device__ __forceinline__ double phase_pn_qt(const double* a, const BinBasis& b) {
   double q = fma(a[0], b.y5, a[4]);
   q = fma(a[1], b.y3, q);
