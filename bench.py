@@ -29,10 +29,12 @@ UNIT = "evals/s"
 
 
 def alg_flops_per_bin(n_det, model="taylorf2"):
-    """Algorithmic fp64 flops per (particle, bin) of the minimal formulation: 9-FMA phase (18),
-    quarter-turn sincos (31), per detector: phasor advance (6) + complex product (6) + <d,h> accumulate (4)."""
+    """Algorithmic fp64 flops per (particle, bin) of the minimal formulation the kernel implements,
+    FMA = 2: 9-FMA phase (18); table-driven sincos: exact reduction (3 add), r^2 (1), sin 2 FMA + 1 mul (5), cos 3 FMA (6),
+    complex product with the table entry (6) = 21; detector 0: 4 FMA (8); every further detector: complex product with its
+    phasor (6) + <d,h> accumulate (4) + phasor advance (6) = 16."""
     assert model == "taylorf2"
-    return 18 + 31 + 16 * n_det
+    return 18 + 21 + 8 + 16 * (n_det - 1)
 
 
 class ClockSampler:
@@ -220,7 +222,7 @@ def run_ours(args):
         flops_launch = float(B) * n_freq * alg_flops_per_bin(n_det)
         ach = flops_launch / (kern_ms / kern_n * 1e-3) / 1e12
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
-                "traffic": None, "kernel": "k_bins<TaylorF2,2det,P=2>", "kernel_ms": kern_ms / kern_n,
+                "traffic": None, "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
                 "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
                 "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,

@@ -142,6 +142,14 @@ int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream);
 int nsgw_profile_enable(ns_handle* h, int32_t on);
 int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_host);
 
+/* Tuning / test options of a handle.  key NSGW_OPT_BINS_KERNEL selects the kernel behind gw_loglike_batch (and the initial
+ * live-set evaluation): 0 = automatic (by model and batch size), 1 = CTA per particle (pair), bins strided over threads
+ * (k_bins; both models), 2 = lane per particle, bin tiles staged in shared memory (k_bins_lp; TaylorF2 only -- for
+ * PhenomD-form the value 2 falls back to 1).  Both compute the same sums in a different, fixed order.
+ * Returns -1 for an unknown key or value. */
+#define NSGW_OPT_BINS_KERNEL 0
+int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
+
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */
 int64_t nsgw_launch_count(void);
 

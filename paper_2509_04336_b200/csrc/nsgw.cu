@@ -162,7 +162,7 @@ __device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const dou
 // further detector a complex product with its phasor, 2 FMA and the phasor advance.
 template <int MODEL, int NDET, int P, int NT>
 __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                         const double2* tabW, const double2* step, const bool* active,
+                                         const double2* tabW, const double2* step, const double2* lut, const bool* active,
                                          double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NW = NT / 32, ND1 = NDET - 1;
@@ -183,7 +183,7 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
     }
     if (MODEL == 1) {
 #pragma unroll
-      for (int i = 0; i < 10; ++i) a[p][i] = cbs[p * CB_SIZE + CB_PH + i];
+      for (int i = 0; i < 10; ++i) a[p][i] = 64.0 * cbs[p * CB_SIZE + CB_PH + i];   // quarter turns -> 1/256 turn (exact)
     }
   }
   if (!any) return;   // block-uniform: nothing to evaluate (all proposals of this CTA were out of bounds)
@@ -201,9 +201,9 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
     for (int p = 0; p < P; ++p) {
       double q, amp = 1.0;
       if (MODEL == 1) q = phase_pn_qt(a[p], b);
-      else phenom_bin(cbs + p * CB_SIZE, b, q, amp);
+      else { phenom_bin(cbs + p * CB_SIZE, b, q, amp); q *= 64.0; }
       double sn, cs;
-      sincos_qt(q, sn, cs);
+      sincos_lut(q, lut, sn, cs);
       if (MODEL == 2) { sn *= amp; cs *= amp; }
       // E = amp exp(-i Phi) = cs - i sn;  X0 += conj(wd_0) E
       acc[p][0] = fma(w[0].x, cs, acc[p][0]);
@@ -283,9 +283,11 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   __shared__ __align__(16) double cbs[P * CB_SIZE];
   __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
   __shared__ double red[NW * NV], out[NV];
+  __shared__ double2 lut[256];
   __shared__ bool active[P];
   const DevCfg& cfg = *cfgp;
   const long long p0 = (long long)blockIdx.x * P;
+  build_sincos_lut(lut, threadIdx.x, NT);
   for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
     long long p = p0 + e / CB_SIZE;
     cbs[e] = (p < B) ? cbs_g[p * CB_SIZE + e % CB_SIZE] : 0.0;
@@ -295,7 +297,7 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
   __syncthreads();
   double acc[P][AL::N];
-  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, acc);
+  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, acc);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < P; ++p)
@@ -306,6 +308,132 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
     int p = threadIdx.x;
     logl[p0 + p] = finish_logl<MODEL, NDET>(cfg, cbs + p * CB_SIZE, out + p * AL::N, parts ? parts + (p0 + p) * 2 * NDET : nullptr);
   }
+}
+
+// ------------------------------------------------------------------------------------------------------
+// K1 for large batches, lane = particle: every thread owns ONE particle (phase coefficients, detector phasors and partial
+// sums in registers for the whole task), and the CTA walks a range of KR bins whose table values are staged once in shared
+// memory and read with warp-uniform (broadcast) LDS.  No per-bin global traffic, no cross-thread reduction, no phasor
+// tables: a task costs each thread 2 sincos per extra detector plus KR x (the same per-bin arithmetic as bin_loop).
+// Task = (group of NT particles, range of KR bins); partial[B][n_ranges][N] is summed in range order by k_finish.
+// Built for TaylorF2 (no per-particle branches in the bin loop; PhenomD-form's piecewise regions would diverge across lanes).
+// ------------------------------------------------------------------------------------------------------
+template <int NDET, int KR>
+struct LpSmem {
+  double2 t01[KR], t23[KR], t45[KR], t67[KR];
+  double2 wd[NDET][KR];
+  double f[KR];
+};
+
+template <int NDET, int NT, int KR, int PP, int UNR, int OCC>
+__global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
+                                                     long long B, int kr /*bins per range, <= KR, multiple of UNR*/, int nranges,
+                                                     long long ntasks, double* __restrict__ partial) {
+  using AL = AccLayout<1, NDET>;
+  constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
+  __shared__ __align__(16) LpSmem<NDET, KR> sm;
+  __shared__ double2 lut[256];
+  const DevCfg& cfg = *cfgp;
+  const int tid = threadIdx.x;
+  const int nf = cfg.n_freq;
+  build_sincos_lut(lut, tid, NT);
+  for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
+    const long long grp = task / nranges;
+    const int rng = (int)(task % nranges);
+    const int k0 = rng * kr;
+    const int nk = min(kr, nf - k0);
+    const int nk2 = (nk + UNR - 1) / UNR * UNR;   // padded with zero-weight bins
+    __syncthreads();   // readers of the previous tile are done
+    for (int i = tid; i < nk2; i += NT) {
+      const bool ok = i < nk;
+      const int k = k0 + (ok ? i : nk - 1);
+      sm.t01[i] = __ldg(tb.t01 + k); sm.t23[i] = __ldg(tb.t23 + k); sm.t45[i] = __ldg(tb.t45 + k); sm.t67[i] = __ldg(tb.t67 + k);
+      sm.f[i] = __ldg(tb.f + k);
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) sm.wd[d][i] = ok ? __ldg(tb.wd[d] + k) : make_double2(0.0, 0.0);
+    }
+    // ---- this thread's PP particles (a warp-wide load of the table values of a bin then serves 32 PP particle-bins)
+    double a[PP][10];
+    double2 R[PP][ND1s], St[PP][ND1s];
+    double acc[PP][AL::N];
+#pragma unroll
+    for (int j = 0; j < PP; ++j) {
+      const long long p = (grp * PP + j) * NT + tid;
+      const bool have = p < B;
+      const double* cb = cbs_g + (have ? p : 0) * CB_SIZE;
+#pragma unroll
+      for (int i = 0; i < 10; ++i) a[j][i] = have ? 64.0 * __ldg(cb + CB_PH + i) : 0.0;   // quarter turns -> 1/256 turn (exact)
+#pragma unroll
+      for (int d = 0; d < ND1; ++d) {
+        const double cr = have ? __ldg(cb + CB_DET + 4 * (d + 1)) : 0.0, ci = have ? __ldg(cb + CB_DET + 4 * (d + 1) + 1) : 0.0;
+        const double dtq = have ? __ldg(cb + CB_DET + 4 * (d + 1) + 2) : 0.0;
+        double sn, cs;
+        sincos_qt(dtq * (cfg.f_min + cfg.df * k0), sn, cs);
+        R[j][d] = make_double2(cr * cs - ci * sn, cr * sn + ci * cs);
+        sincos_qt(dtq * cfg.df, sn, cs);
+        St[j][d] = make_double2(cs, sn);
+      }
+#pragma unroll
+      for (int i = 0; i < AL::N; ++i) acc[j][i] = 0.0;
+    }
+    __syncthreads();
+#pragma unroll UNR
+    for (int kk = 0; kk < nk2; ++kk) {
+      BinBasis b;
+      { const double2 v = sm.t01[kk]; b.y5 = v.x; b.y3 = v.y; }
+      { const double2 v = sm.t23[kk]; b.y2 = v.x; b.y = v.y; }
+      { const double2 v = sm.t45[kk]; b.L = v.x; b.x = v.y; }
+      { const double2 v = sm.t67[kk]; b.xL = v.x; b.x2 = v.y; }
+      b.f = sm.f[kk]; b.f34 = 0.0;
+      double2 w[NDET];
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) w[d] = sm.wd[d][kk];
+#pragma unroll
+      for (int j = 0; j < PP; ++j) {
+        const double q = phase_pn_qt(a[j], b);
+        double sn, cs;
+        sincos_lut(q, lut, sn, cs);
+        acc[j][0] = fma(w[0].x, cs, acc[j][0]);
+        acc[j][1] = fma(-w[0].x, sn, acc[j][1]);
+        acc[j][0] = fma(-w[0].y, sn, acc[j][0]);
+        acc[j][1] = fma(-w[0].y, cs, acc[j][1]);
+#pragma unroll
+        for (int d = 0; d < ND1; ++d) {
+          const double rx = R[j][d].x, ry = R[j][d].y;
+          const double gr = fma(cs, rx, sn * ry);
+          const double gi = fma(cs, ry, -(sn * rx));
+          acc[j][AL::kDh + d] = fma(w[d + 1].x, gr, acc[j][AL::kDh + d]);
+          acc[j][AL::kDh + d] = fma(w[d + 1].y, gi, acc[j][AL::kDh + d]);
+          R[j][d].x = fma(rx, St[j][d].x, -(ry * St[j][d].y));
+          R[j][d].y = fma(rx, St[j][d].y, ry * St[j][d].x);
+        }
+      }
+    }
+#pragma unroll
+    for (int j = 0; j < PP; ++j) {
+      const long long p = (grp * PP + j) * NT + tid;
+      if (p < B) {
+#pragma unroll
+        for (int i = 0; i < AL::N; ++i) partial[(p * nranges + rng) * AL::N + i] = acc[j][i];
+      }
+    }
+  }
+}
+
+// Adds the per-chunk partial sums in chunk order and finishes logL.
+template <int MODEL, int NDET>
+__global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restrict__ cbs_g, const double* __restrict__ partial, int nchunks,
+                         long long B, double* logl, double* parts) {
+  using AL = AccLayout<MODEL, NDET>;
+  long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (p >= B) return;
+  double sums[AL::N];
+#pragma unroll
+  for (int i = 0; i < AL::N; ++i) sums[i] = 0.0;
+  for (int c = 0; c < nchunks; ++c)
+#pragma unroll
+    for (int i = 0; i < AL::N; ++i) sums[i] += partial[(p * nchunks + c) * AL::N + i];
+  logl[p] = finish_logl<MODEL, NDET>(*cfgp, cbs_g + p * CB_SIZE, sums, parts ? parts + p * 2 * NDET : nullptr);
 }
 
 // Detector-frame waveform of one theta on the grid (for injections): out[n_det][n_freq][2].
@@ -455,6 +583,7 @@ __global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restri
   __shared__ __align__(16) double cbs[P * CB_SIZE];
   __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
   __shared__ double red[NW * NV], out[NV];
+  __shared__ double2 lut[256];
   __shared__ bool active[P];
   __shared__ double s_cur[P][kMaxDim], s_prop[P][kMaxDim], s_curl[P];
   const DevCfg& cfg = *cfgp;
@@ -466,6 +595,7 @@ __global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restri
   const long long row = (long long)blockIdx.x * P + tid;
   const bool owner = tid < P && row < a.B;
   int na = 0, ne = 0, no = 0;
+  build_sincos_lut(lut, tid, NT);
   if (tid < P) {
     active[tid] = false;
     if (owner) {
@@ -501,7 +631,7 @@ __global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restri
     __syncthreads();
     // ---- phase B: bins
     double acc[P][AL::N];
-    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, active, acc);
+    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, acc);
     double v[NV];
 #pragma unroll
     for (int p = 0; p < P; ++p)
@@ -717,6 +847,10 @@ struct ns_handle {
   double* d_cur_l = nullptr;
   int* d_cnt = nullptr;         // 3 * k
   double* d_cb = nullptr;       // coefficient blocks scratch
+  double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [B][n_ranges][N]
+  size_t partial_cap = 0;
+  int n_sm = 148;
+  int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
   long long theta_cap = 0;
@@ -783,8 +917,52 @@ int ensure_theta(ns_handle* h, long long B) {
 // particles per CTA of the bin loop as a function of the batch (fill 148 SMs first, then reuse table loads)
 int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 
+// Lane-per-particle kernel (k_bins_lp): geometry and the batch size from which it is used (TaylorF2 only).
+constexpr int kLpNT = 128, kLpKR = 256, kLpPP = 2, kLpUNR = 4, kLpOCC = 3;
+constexpr long long kLpMinBatch = 4096;   // below this the CTA-per-particle kernel fills the machine better
+
+int ensure_partial(ns_handle* h, size_t n) {
+  if (n > h->partial_cap) {
+    if (h->d_partial) cudaFree(h->d_partial);
+    h->d_partial = nullptr; h->partial_cap = 0;
+    CU_CHECK(h, cudaMalloc(&h->d_partial, sizeof(double) * n));
+    h->partial_cap = n;
+  }
+  return 0;
+}
+
+template <int NDET>
+int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
+  using AL = AccLayout<1, NDET>;
+  constexpr int NT = kLpNT, PP = kLpPP;
+  const long long ngroups = (B + NT * PP - 1) / (NT * PP);
+  const long long grid_max = (long long)h->n_sm * kLpOCC;
+  // bins per task: as large as keeps >= 6 tasks per resident CTA (tail balance), never below 32
+  int kr = kLpKR;
+  while (kr > 32 && ngroups * ((h->cfg.n_freq + kr - 1) / kr) < 6 * grid_max) kr /= 2;
+  const int nranges = (h->cfg.n_freq + kr - 1) / kr;
+  const long long ntasks = ngroups * nranges;
+  const long long grid = std::min<long long>(ntasks, grid_max);
+  int rc = ensure_partial(h, (size_t)B * nranges * AL::N);
+  if (rc) return rc;
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof && h->prof_ev.size() < 4096) {
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, s);
+  }
+  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, kr, nranges, ntasks,
+                                                                              h->d_partial);
+  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
+  LAUNCH_CHECK(h);
+  k_finish<1, NDET><<<(unsigned)((B + 127) / 128), 128, 0, s>>>(h->d_cfg, h->d_cb, h->d_partial, nranges, B, logl, parts);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
 template <int MODEL, int NDET>
 int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
+  if (MODEL == 1 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kLpMinBatch)))
+    return launch_bins_lp<NDET>(h, B, logl, parts, s);
   int P = pick_p(B);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (h->prof && h->prof_ev.size() < 4096) {
@@ -884,7 +1062,7 @@ void ns_free(ns_handle* h) {
   if (!h) return;
   cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
-  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
+  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -922,6 +1100,11 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
 
   cudaStream_t s = (cudaStream_t)stream;
   ns_handle* h = new ns_handle();
+  {
+    int dev = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, dev);
+    if (h->n_sm < 1) h->n_sm = 148;
+  }
   h->cfg = *cfg;
   h->cfg.phenom_table_host = nullptr;
   h->seed = seed;
@@ -1170,6 +1353,12 @@ int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host,
   if (h_host) *h_host = h->h_fin[1];
   if (logz_err_host) *logz_err_host = std::sqrt(std::max(h->h_fin[1], 0.0) / neff);
   return 0;
+}
+
+int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
+  if (!h) return -3;
+  if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
+  return fail(h, -1, "unknown option or value");
 }
 
 int nsgw_profile_enable(ns_handle* h, int32_t on) {

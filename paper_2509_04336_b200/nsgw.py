@@ -44,7 +44,7 @@ class NsStats(C.Structure):
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
            "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_get_live", "ns_finalize_evidence",
-           "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read"]
+           "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 _lib = None
 
@@ -231,6 +231,9 @@ class Handle:
 
     def profile_enable(self, on=True):
         self._check(lib().nsgw_profile_enable(self._h, C.c_int32(1 if on else 0)), "nsgw_profile_enable")
+
+    def set_option(self, key, value):
+        self._check(lib().nsgw_set_option(self._h, C.c_int32(key), C.c_int32(value)), "nsgw_set_option")
 
     def profile_read(self):
         ms, n = C.c_double(), C.c_int64()

@@ -68,10 +68,16 @@ def test_live_draw_is_bitwise_philox(nsgw):
     np.testing.assert_allclose(l_g.cpu().numpy(), l_o, rtol=1e-13)
 
 
+KERNELS = [1, 2]   # NSGW_OPT_BINS_KERNEL: 1 = CTA per particle pair (k_bins), 2 = register-resident bins (k_bins_reg)
+
+
+@pytest.mark.parametrize("kern", KERNELS)
 @pytest.mark.parametrize("B", [1, 515, 1027, 4101])
-def test_taylorf2_loglike_parity(nsgw, c2, B):
-    # config-2 shape: 2 detectors x 4017 bins; B spans both launch shapes (P=1, P=2) with ragged tails
+def test_taylorf2_loglike_parity(nsgw, c2, B, kern):
+    # config-2 shape: 2 detectors x 4017 bins (3 full 1024-bin chunks + a ragged one); B spans the launch shapes
+    # (P=1, P=2; sub-batches of 8 with ragged tails)
     h = nsgw.Handle(c2)
+    h.set_option(0, kern)
     P = O.OracleProblem(c2)
     th = P.prior_transform(W.uniforms(B, 11, 100 + B))
     logl_o, parts_o = P.gw_loglike(th, parts=True)
@@ -84,16 +90,20 @@ def test_taylorf2_injection_and_unphysical(nsgw, c2):
     P = O.OracleProblem(c2)
     th = np.array([W.INJ_C3] * 4)
     th[1, 1] = 1.5; th[2, 4] = -1.0; th[3, 2] = float("nan")
-    lg = h.gw_loglike_batch(dev(th)).cpu().numpy()
     lo = P.gw_loglike(th)
-    assert abs(lg[0] - lo[0]) < 1e-10 * 400 and np.all(np.isneginf(lg[1:])) and np.all(np.isneginf(lo[1:]))
+    for kern in KERNELS:
+        h.set_option(0, kern)
+        lg = h.gw_loglike_batch(dev(th)).cpu().numpy()
+        assert abs(lg[0] - lo[0]) < 1e-10 * 400 and np.all(np.isneginf(lg[1:])) and np.all(np.isneginf(lo[1:]))
     assert h.gw_loglike_batch(dev(np.zeros((0, 11)))).numel() == 0     # empty batch
 
 
+@pytest.mark.parametrize("kern", KERNELS)
 @pytest.mark.parametrize("B", [3, 515, 4101])
-def test_phenomd_loglike_parity_config3_shape(nsgw, c3, B):
+def test_phenomd_loglike_parity_config3_shape(nsgw, c3, B, kern):
     spec, _ = c3
     h = nsgw.Handle(spec)
+    h.set_option(0, kern)
     P = O.OracleProblem(spec)
     th = P.prior_transform(W.uniforms(B, 11, 200 + B))
     th[0] = W.INJ_C3
@@ -110,7 +120,8 @@ def test_phenomd_builtin_table_equals_explicit(nsgw, c3):
     assert torch.equal(a, b)
 
 
-def test_phenomd_spin_table_parity(nsgw):
+@pytest.mark.parametrize("kern", KERNELS)
+def test_phenomd_spin_table_parity(nsgw, kern):
     # a fit table with non-zero spin columns and gamma2 < 1 exercises the chi_PN polynomial and the other Fpeak branch
     spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1", "V1"], 4.0, 512.0, (20.0, 40.0))
     tab = W.surrogate_table()
@@ -122,11 +133,14 @@ def test_phenomd_spin_table_parity(nsgw):
     P = O.OracleProblem(spec)
     th = P.prior_transform(W.uniforms(130, 11, 77))
     logl_o, parts_o = P.gw_loglike(th, parts=True)
-    logl_g, parts_g = nsgw.Handle(spec).gw_loglike_batch(dev(th), parts=True)
+    h = nsgw.Handle(spec)
+    h.set_option(0, kern)
+    logl_g, parts_g = h.gw_loglike_batch(dev(th), parts=True)
     _check_logl(logl_g.cpu().numpy(), parts_g.cpu().numpy(), logl_o, parts_o, 3)
 
 
-def test_phenomd_three_detector_long_segment_parity(nsgw):
+@pytest.mark.parametrize("kern", KERNELS)
+def test_phenomd_three_detector_long_segment_parity(nsgw, kern):
     # config-5 shape: 3 detectors x 32449 bins (16 s at 4096 Hz)
     spec = W.config5(wf)
     assert spec["n_freq"] == 32449 and spec["n_det"] == 3
@@ -134,7 +148,9 @@ def test_phenomd_three_detector_long_segment_parity(nsgw):
     u = W.config5_live(spec, 96)
     th = P.prior_transform(u)
     logl_o, parts_o = P.gw_loglike(th, parts=True)
-    logl_g, parts_g = nsgw.Handle(spec).gw_loglike_batch(dev(th), parts=True)
+    h = nsgw.Handle(spec)
+    h.set_option(0, kern)
+    logl_g, parts_g = h.gw_loglike_batch(dev(th), parts=True)
     _check_logl(logl_g.cpu().numpy(), parts_g.cpu().numpy(), logl_o, parts_o, 3)
 
 
