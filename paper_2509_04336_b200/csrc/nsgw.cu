@@ -38,7 +38,7 @@ constexpr int kWalkThreads = 256;
 struct DevState {
   double logx, logz, h, walks, delay, lstar;
   long long iter, n_eval_total;
-  int W, naccept, maxmcmc, pad;
+  int W, naccept, maxmcmc, spec;   // spec: speculative steps per chunk of the next walk
   ns_stats stats;
 };
 
@@ -131,14 +131,14 @@ struct AccLayout {
 //   R = (Cr + i Ci) * exp(i * dtq * f_t)  [dtq: quarter turns per Hz relative to detector 0],
 // built as lane-table x warp-table to keep it to one sincos per entry.
 // tabL[(p*ND1+d-1)*32 + lane] = exp(i dtq df lane); tabW[(p*ND1+d-1)*NW + w] = C * exp(i dtq (f_min + 32 w df)).
-template <int NDET, int P, int NT>
-__device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const double* cbs /*smem [P][CB_SIZE]*/, double2* tabL,
+template <int NDET, int NT>
+__device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const double* cbs /*smem [np][CB_SIZE]*/, int np, double2* tabL,
                                                     double2* tabW, double2* step) {
-  constexpr int NW = NT / 32, ND1 = NDET - 1;
-  constexpr int NE = P * ND1 * (32 + NW + 1);
+  constexpr int NW = NT / 32, ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
+  const int NE = np * ND1 * (32 + NW + 1);
   for (int e = threadIdx.x; e < NE; e += NT) {
     int pd = e / (32 + NW + 1), j = e % (32 + NW + 1);
-    int p = pd / ND1, d = pd % ND1 + 1;
+    int p = pd / ND1s, d = pd % ND1s + 1;
     const double* cb = cbs + p * CB_SIZE;
     double dtq = cb[CB_DET + 4 * d + 2];
     double s, c;
@@ -163,27 +163,31 @@ __device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const dou
 template <int MODEL, int NDET, int P, int NT>
 __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
                                          const double2* tabW, const double2* step, const double2* lut, const bool* active,
+                                         const int* slot /*smem [P]: coefficient-block / phasor-table slot of particle p*/,
                                          double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NW = NT / 32, ND1 = NDET - 1;
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   double2 R[P][ND1 > 0 ? ND1 : 1], St[P][ND1 > 0 ? ND1 : 1];
   double a[P][MODEL == 1 ? 10 : 1];
+  const double* cbp[P];
   bool any = false;
 #pragma unroll
   for (int p = 0; p < P; ++p) {
+    const int sl = slot[p];
+    cbp[p] = cbs + sl * CB_SIZE;
     any = any || active[p];
 #pragma unroll
     for (int i = 0; i < AL::N; ++i) acc[p][i] = 0.0;
 #pragma unroll
     for (int d = 0; d < ND1; ++d) {
-      double2 u = tabL[(p * ND1 + d) * 32 + lane], v = tabW[(p * ND1 + d) * NW + wrp];
+      double2 u = tabL[(sl * ND1 + d) * 32 + lane], v = tabW[(sl * ND1 + d) * NW + wrp];
       R[p][d] = make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x);
-      St[p][d] = step[p * ND1 + d];
+      St[p][d] = step[sl * ND1 + d];
     }
     if (MODEL == 1) {
 #pragma unroll
-      for (int i = 0; i < 10; ++i) a[p][i] = 64.0 * cbs[p * CB_SIZE + CB_PH + i];   // quarter turns -> 1/256 turn (exact)
+      for (int i = 0; i < 10; ++i) a[p][i] = 64.0 * cbp[p][CB_PH + i];   // quarter turns -> 1/256 turn (exact)
     }
   }
   if (!any) return;   // block-uniform: nothing to evaluate (all proposals of this CTA were out of bounds)
@@ -201,7 +205,7 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
     for (int p = 0; p < P; ++p) {
       double q, amp = 1.0;
       if (MODEL == 1) q = phase_pn_qt(a[p], b);
-      else { phenom_bin(cbs + p * CB_SIZE, b, q, amp); q *= 64.0; }
+      else { phenom_bin(cbp[p], b, q, amp); q *= 64.0; }
       double sn, cs;
       sincos_lut(q, lut, sn, cs);
       if (MODEL == 2) { sn *= amp; cs *= amp; }
@@ -285,19 +289,21 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   __shared__ double red[NW * NV], out[NV];
   __shared__ double2 lut[256];
   __shared__ bool active[P];
+  __shared__ int slot[P];
   const DevCfg& cfg = *cfgp;
   const long long p0 = (long long)blockIdx.x * P;
   build_sincos_lut(lut, threadIdx.x, NT);
+  if (threadIdx.x < P) slot[threadIdx.x] = threadIdx.x;
   for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
     long long p = p0 + e / CB_SIZE;
     cbs[e] = (p < B) ? cbs_g[p * CB_SIZE + e % CB_SIZE] : 0.0;
   }
   __syncthreads();
   if (threadIdx.x < P) active[threadIdx.x] = cbs[threadIdx.x * CB_SIZE + CB_VALID] != 0.0;
-  build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
+  build_phasor_tables<NDET, NT>(cfg, cbs, P, tabL, tabW, step);
   __syncthreads();
   double acc[P][AL::N];
-  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, acc);
+  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, acc);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < P; ++p)
@@ -484,6 +490,8 @@ struct WalkArgs {
   int* n_accept; int* n_eval; int* n_oob;
   uint8_t* tflags; double* tlogl;
   int trace_stride;
+  int spec;                 // speculative steps per chunk (1..kWalkDMax)
+  const int* spec_dev;      // if non-null overrides spec
 };
 
 // DE proposal for one walker (footnote P:120; R:L8-L10).  Returns false if out of bounds.
@@ -574,86 +582,144 @@ __global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
   if (a.n_oob) a.n_oob[row] = no;
 }
 
-// GW walk: CTA per P walkers.  Each step: lanes 0..P-1 propose + transform + set up (phase A), all threads sweep the bins
-// (phase B), lanes 0..P-1 accept (phase C, merged with the next phase A).  All walkers do exactly W steps.
-template <int MODEL, int NDET, int P>
-__global__ void __launch_bounds__(kWalkThreads) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+// GW walk: one CTA per walker, all W steps in one launch, speculative chunks of up to DMAX steps.
+//
+// A walker's chain is serial (proposal t+1 starts from the point accepted at t), and one step is: propose + transform + ~3 kflop
+// of serial waveform set-up by ONE thread, then a bin sweep.  With acceptance rates of 0.1-10 % per step the outcome "rejected" is
+// almost certain, so the kernel evaluates the next D steps AT ONCE, all from the current point: lanes 0..D-1 of warp 0 build the
+// D proposals (Philox counters t0..t0+D-1) and their coefficient blocks side by side (SIMT: D set-ups for the latency of one),
+// the in-bounds ones are swept together (PG particles per pass share every table load and supply ILP), and thread 0 then walks
+// through the D outcomes in order: out-of-bounds -> counted; logL' > L* -> accepted, and the steps after it are DISCARDED (they
+// started from a stale point) and redone in the next chunk from t0 + j + 1.  The decisions, counters and trace are exactly those
+// of the sequential algorithm (oracle_walk); only work is wasted, never semantics changed.  D is a launch argument (1 = no
+// speculation) chosen from the previous batch's acceptance rate.
+constexpr int kWalkDMax = 8;   // speculative steps per chunk
+constexpr int kWalkPG = 2;     // particles per bin sweep
+
+template <int MODEL, int NDET, int PG, int NT>
+__device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
+                                            const double2* tabW, const double2* step, const double2* lut, const bool* active,
+                                            const int* slot, double* red, double* out /*smem [PG][N]*/) {
   using AL = AccLayout<MODEL, NDET>;
-  constexpr int NT = kWalkThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
-  __shared__ __align__(16) double cbs[P * CB_SIZE];
-  __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
-  __shared__ double red[NW * NV], out[NV];
+  constexpr int NV = PG * AL::N;
+  double acc[PG][AL::N];
+  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, acc);
+  double v[NV];
+#pragma unroll
+  for (int p = 0; p < PG; ++p)
+#pragma unroll
+    for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
+  block_reduce<NV, NT>(v, red, out);
+}
+
+template <int MODEL, int NDET>
+__global__ void __launch_bounds__(kWalkThreads, 2) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+  using AL = AccLayout<MODEL, NDET>;
+  constexpr int NT = kWalkThreads, NW = NT / 32, DM = kWalkDMax, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
+  __shared__ __align__(16) double cbs[DM * CB_SIZE];
+  __shared__ double2 tabL[DM * ND1 * 32], tabW[DM * ND1 * NW], step[DM * ND1];
+  __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DM];
   __shared__ double2 lut[256];
-  __shared__ bool active[P];
-  __shared__ double s_cur[P][kMaxDim], s_prop[P][kMaxDim], s_curl[P];
+  __shared__ bool active[PG];
+  __shared__ int slot[PG];
+  __shared__ double s_cur[kMaxDim], s_prop[DM][kMaxDim], s_curl;
+  __shared__ int s_flag[DM];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
+  __shared__ int s_t0;
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const int W = a.W_dev ? *a.W_dev : a.W;
+  const int spec = max(1, min(DM, a.spec_dev ? *a.spec_dev : a.spec));
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
   const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
   const int tid = threadIdx.x;
-  const long long row = (long long)blockIdx.x * P + tid;
-  const bool owner = tid < P && row < a.B;
-  int na = 0, ne = 0, no = 0;
+  const long long row = blockIdx.x;
+  int na = 0, ne = 0, no = 0;   // thread 0's counters
   build_sincos_lut(lut, tid, NT);
-  if (tid < P) {
-    active[tid] = false;
-    if (owner) {
-      for (int d = 0; d < D; ++d) s_cur[tid][d] = a.u[row * D + d];
-      s_curl[tid] = a.logl[row];
-    }
+  if (tid == 0) {
+    for (int d = 0; d < D; ++d) s_cur[d] = a.u[row * D + d];
+    s_curl = a.logl[row];
+    s_t0 = 0;
   }
   __syncthreads();
-  for (int t = 0; t < W; ++t) {
-    // ---- phase A: proposal, bounds, prior transform, waveform set-up
-    if (owner) {
-      bool inb = de_propose(cfg, a, sid, (uint32_t)t, (uint32_t)(a.slot0 + row), s_cur[tid], s_prop[tid]);
-      bool act = false;
+  while (true) {
+    const int t0 = s_t0;
+    if (t0 >= W) break;
+    const int nd = min(spec, W - t0);
+    // ---- phase A: nd proposals from the current point, side by side
+    if (tid < nd) {
+      const int j = tid;
+      bool inb = de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur, s_prop[j]);
+      int fl = 0;
       if (inb) {
         double th[11];
 #pragma unroll
-        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[tid][d]);
-        act = setup_particle<MODEL>(cfg, th, cbs + tid * CB_SIZE);
-        ++ne;
-      } else {
-        ++no;
-        cbs[tid * CB_SIZE + CB_VALID] = 0.0;
+        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[j][d]);
+        fl = setup_particle<MODEL>(cfg, th, cbs + j * CB_SIZE) ? 2 : 1;
       }
-      active[tid] = act;
-      if (!inb) {
-        if (a.tflags) a.tflags[row * a.trace_stride + t] = 1;
-        if (a.tlogl) a.tlogl[row * a.trace_stride + t] = nan("");
-      }
-      s_prop[tid][kMaxDim - 1] = inb ? 1.0 : 0.0;   // ndim <= 11 for GW: slot 15 is free
+      s_flag[j] = fl;
     }
     __syncthreads();
-    build_phasor_tables<NDET, P, NT>(cfg, cbs, tabL, tabW, step);
-    __syncthreads();
-    // ---- phase B: bins
-    double acc[P][AL::N];
-    bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, acc);
-    double v[NV];
+    // the proposals that need a sweep, in order (every thread counts them the same way)
+    int n_in = 0;
 #pragma unroll
-    for (int p = 0; p < P; ++p)
+    for (int j = 0; j < DM; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
+    if (n_in > 0) {
+      build_phasor_tables<NDET, NT>(cfg, cbs, nd, tabL, tabW, step);
+      __syncthreads();
+      // ---- phase B: sweeps, PG particles at a time (a single left-over goes through the one-particle loop)
+      for (int g = 0; g < n_in; g += PG) {
+        const int ng = min(PG, n_in - g);
+        if (tid < PG) {
+          int cnt = 0, mine = -1, first = 0;
 #pragma unroll
-      for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
-    block_reduce<NV, NT>(v, red, out);
-    // ---- phase C: accept iff in bounds and logL' > L*
-    if (owner && s_prop[tid][kMaxDim - 1] != 0.0) {
-      double pl = finish_logl<MODEL, NDET>(cfg, cbs + tid * CB_SIZE, out + tid * AL::N, nullptr);
-      uint8_t fl = 4;
-      if (pl > lstar) {
-        for (int d = 0; d < D; ++d) s_cur[tid][d] = s_prop[tid][d];
-        s_curl[tid] = pl; ++na; fl |= 2;
+          for (int j = 0; j < DM; ++j) {
+            if (j < nd && s_flag[j] == 2) {
+              if (cnt == g) first = j;
+              if (cnt == g + tid) mine = j;
+              ++cnt;
+            }
+          }
+          slot[tid] = (mine >= 0) ? mine : first;
+          active[tid] = mine >= 0;
+        }
+        __syncthreads();
+        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, red, out);
+        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, red, out);
+        if (tid < ng) s_logl[slot[tid]] = finish_logl<MODEL, NDET>(cfg, cbs + slot[tid] * CB_SIZE, out + tid * AL::N, nullptr);
+        __syncthreads();
       }
-      if (a.tflags) a.tflags[row * a.trace_stride + t] = fl;
-      if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
+    }
+    // ---- phase C: the nd outcomes in order; the first acceptance invalidates the rest of the chunk
+    if (tid == 0) {
+      int used = nd;
+      for (int j = 0; j < nd; ++j) {
+        const int t = t0 + j;
+        const int fl = s_flag[j];
+        if (fl == 0) {
+          ++no;
+          if (a.tflags) a.tflags[row * a.trace_stride + t] = 1;
+          if (a.tlogl) a.tlogl[row * a.trace_stride + t] = nan("");
+          continue;
+        }
+        ++ne;
+        const double pl = (fl == 2) ? s_logl[j] : -INFINITY;
+        uint8_t tf = 4;
+        const bool acc_ = pl > lstar;
+        if (acc_) {
+          for (int d = 0; d < D; ++d) s_cur[d] = s_prop[j][d];
+          s_curl = pl; ++na; tf |= 2;
+        }
+        if (a.tflags) a.tflags[row * a.trace_stride + t] = tf;
+        if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
+        if (acc_) { used = j + 1; break; }
+      }
+      s_t0 = t0 + used;
     }
     __syncthreads();
   }
-  if (owner) {
-    for (int d = 0; d < D; ++d) a.u[row * D + d] = s_cur[tid][d];
-    a.logl[row] = s_curl[tid];
+  if (tid == 0) {
+    for (int d = 0; d < D; ++d) a.u[row * D + d] = s_cur[d];
+    a.logl[row] = s_curl;
     if (a.n_accept) a.n_accept[row] = na;
     if (a.n_eval) a.n_eval[row] = ne;
     if (a.n_oob) a.n_oob[row] = no;
@@ -791,6 +857,11 @@ __global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __r
     double r = fmax(0.5, amean) / W;
     double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
     st->walks = walks;
+    // speculative chunk length of the next walk: keep the expected waste (steps after an acceptance) near 1/8 of the work
+    {
+      const double per_step = fmax(amean, 0.05) / W;
+      st->spec = max(1, min(kWalkDMax, (int)floor(0.25 / per_step)));
+    }
     st->n_eval_total += s_e[0];
     double lse = lmax + log(s_d[0]);
     ns_stats& o_ = st->stats;
@@ -850,6 +921,7 @@ struct ns_handle {
   double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [B][n_ranges][N]
   size_t partial_cap = 0;
   int n_sm = 148;
+  int opt_walk_spec = 0;        // 0 auto (from the acceptance rate), 1..8 fixed speculative chunk length
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
@@ -1020,12 +1092,7 @@ int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cuda
 
 template <int MODEL, int NDET>
 int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
-  // P walkers per CTA: 1 keeps all SMs busy for the k = 500..700 batches of a real run; 2 halves table traffic for big sweeps
-  if (a.B >= 2048) {
-    k_walk_gw<MODEL, NDET, 2><<<(unsigned)((a.B + 1) / 2), kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
-  } else {
-    k_walk_gw<MODEL, NDET, 1><<<(unsigned)a.B, kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
-  }
+  k_walk_gw<MODEL, NDET><<<(unsigned)a.B, kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
   LAUNCH_CHECK(h);
   return 0;
 }
@@ -1179,7 +1246,7 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
   memset(&hs, 0, sizeof(hs));
   hs.logx = 0.0; hs.logz = -INFINITY; hs.h = 0.0; hs.walks = cfg->walks0;
   hs.delay = (n > 0) ? (cfg->delay >= 0.0 ? cfg->delay : std::max((double)n / (10.0 * k) - 1.0, 0.0)) : 0.0;
-  hs.iter = 0; hs.n_eval_total = n; hs.W = 1; hs.naccept = cfg->naccept; hs.maxmcmc = cfg->maxmcmc;
+  hs.iter = 0; hs.n_eval_total = n; hs.W = 1; hs.spec = 2; hs.naccept = cfg->naccept; hs.maxmcmc = cfg->maxmcmc;
   INIT_CHECK(cudaMemcpyAsync(h->d_state, &hs, sizeof(hs), cudaMemcpyHostToDevice, s), -2);
   if (n > 0) {
     INIT_CHECK(cudaMalloc(&h->d_live_u, sizeof(double) * (size_t)n * D), -2);
@@ -1273,6 +1340,7 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
   a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32); a.stream_id = stream_id; a.slot0 = slot0;
   a.n_accept = n_accept_dev; a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.tflags = trace_flags_dev; a.tlogl = trace_logl_dev;
   a.trace_stride = walk_len;
+  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
   return launch_walk(h, a, (cudaStream_t)stream);
 }
 
@@ -1293,6 +1361,7 @@ int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) 
   memset(&a, 0, sizeof(a));
   a.donors = h->d_surv; a.m = m; a.u = h->d_cur_u; a.logl = h->d_cur_l; a.B = k;
   a.lstar_dev = &h->d_state->lstar; a.W_dev = &h->d_state->W; a.iter_dev = &h->d_state->iter;
+  if (h->opt_walk_spec > 0) a.spec = h->opt_walk_spec; else a.spec_dev = &h->d_state->spec;
   a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
   a.n_accept = h->d_cnt; a.n_eval = h->d_cnt + k; a.n_oob = h->d_cnt + 2 * k;
   int rc = launch_walk(h, a, s);
@@ -1358,6 +1427,7 @@ int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host,
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (!h) return -3;
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
+  if (key == NSGW_OPT_WALK_SPEC && value >= 0 && value <= kWalkDMax) { h->opt_walk_spec = value; return 0; }
   return fail(h, -1, "unknown option or value");
 }
 

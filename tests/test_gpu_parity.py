@@ -187,12 +187,17 @@ def _compare_traces(res_g, res_o, lstar, W_):
     return clean, n_excused, n_steps
 
 
-@pytest.mark.parametrize("kind,B,Wlen", [(W.LIKE_TAYLORF2, 37, 12), (W.LIKE_PHENOMD, 2051, 3), (W.LIKE_PHENOMD, 70, 10)])
-def test_walk_decision_parity(nsgw, kind, B, Wlen):
+# spec = speculative chunk length of k_walk_gw (NSGW_OPT_WALK_SPEC): 1 = one step at a time, 8 = eight steps evaluated at once
+# and the ones after an acceptance discarded, 3 = chunks that do not divide the walk length.  Results must not depend on it.
+@pytest.mark.parametrize("kind,B,Wlen,spec_len", [(W.LIKE_TAYLORF2, 37, 12, 8), (W.LIKE_TAYLORF2, 37, 12, 1),
+                                                  (W.LIKE_PHENOMD, 2051, 3, 8), (W.LIKE_PHENOMD, 70, 10, 3),
+                                                  (W.LIKE_PHENOMD, 70, 10, 0)])
+def test_walk_decision_parity(nsgw, kind, B, Wlen, spec_len):
     spec = W.gw_spec(kind, ["H1", "L1"], 4.0, 256.0, (20.0, 40.0))
     spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
     P = O.OracleProblem(spec)
     h = nsgw.Handle(spec)
+    h.set_option(1, spec_len)
     rng = np.random.default_rng(4)
     m = 300
     u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
@@ -217,6 +222,38 @@ def test_walk_decision_parity(nsgw, kind, B, Wlen):
     np.testing.assert_allclose(lg_.cpu().numpy()[clean], res_o["logl"][clean], rtol=0, atol=1e-9 * max(1.0, abs(lstar)))
     fl = res_o["flags"]
     assert (fl & 1).any() and (fl & 2).any() and ((fl & 4) > (fl & 2) * 2).any()      # the case exercises oob, accept and reject
+
+
+def test_walk_speculation_is_invisible(nsgw):
+    """The speculative chunk length is a scheduling choice: end points, logL, counters and the whole trace are bit-identical
+    for every value (the discarded steps are redone from the accepted point with the same Philox counters)."""
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1", "V1"], 4.0, 256.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    h = nsgw.Handle(spec)
+    rng = np.random.default_rng(11)
+    m, B, Wlen = 200, 130, 37
+    u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+    donors = u_inj[None, :] + rng.normal(0, 1, (m, 11)) * np.array(W.C5_SIGMA) * 0.5
+    per = np.array(spec["periodic"], bool)
+    donors[:, per] -= np.floor(donors[:, per])
+    donors[:, ~per] = np.clip(donors[:, ~per], 1e-6, 1 - 1e-6)
+    ld = h.loglike_u_batch(dev(donors)).cpu().numpy()
+    lstar = float(np.quantile(ld, 0.2))
+    start = rng.integers(0, m, B)
+    ref = None
+    for spec_len in (1, 2, 5, 8):
+        h.set_option(1, spec_len)
+        ug, lg_ = dev(donors[start]), dev(ld[start])
+        res = h.walk_batch(dev(donors), ug, lg_, lstar, Wlen, 77, (5 << 24) | 3, slot0=0, trace=True)
+        cur = [ug.cpu().numpy(), lg_.cpu().numpy()] + [res[k].cpu().numpy() for k in ("n_accept", "n_eval", "n_oob", "flags")]
+        tl = res["trace_logl"].cpu().numpy()
+        cur.append(np.where(np.isnan(tl), -1.0, tl))
+        if ref is None:
+            ref = cur
+            assert ref[2].sum() > B and (ref[5] & 1).any()      # accepts and out-of-bounds steps both occur
+        else:
+            for x, y in zip(ref, cur):
+                assert np.array_equal(x, y)
 
 
 def test_walk_toy_and_shell_parity(nsgw):
