@@ -30,7 +30,7 @@ thread_local std::string g_init_error;
 // One CTA shape for every bin sweep (likelihood batch and walk): the same particle then gets bit-identical logL from
 // either entry point (same per-thread bin assignment, same reduction tree).
 constexpr int kBinsThreads = 256;
-constexpr int kWalkThreads = 256;
+constexpr int kWalkThreads = 128;
 
 // ======================================================================================================
 // Device state of the sampler
@@ -162,7 +162,7 @@ __device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const dou
 // further detector a complex product with its phasor, 2 FMA and the phasor advance.
 template <int MODEL, int NDET, int P, int NT>
 __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                         const double2* tabW, const double2* step, const double2* lut, const bool* active,
+                                         const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
                                          const int* slot /*smem [P]: coefficient-block / phasor-table slot of particle p*/,
                                          double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
   using AL = AccLayout<MODEL, NDET>;
@@ -205,9 +205,9 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
     for (int p = 0; p < P; ++p) {
       double q, amp = 1.0;
       if (MODEL == 1) q = phase_pn_qt(a[p], b);
-      else { phenom_bin(cbp[p], b, q, amp); q *= 64.0; }
+      else { phenom_bin(cbp[p], b, mt, q, amp); q *= 64.0; }
       double sn, cs;
-      sincos_lut(q, lut, sn, cs);
+      sincos_lut(q, mt, sn, cs);
       if (MODEL == 2) { sn *= amp; cs *= amp; }
       // E = amp exp(-i Phi) = cs - i sn;  X0 += conj(wd_0) E
       acc[p][0] = fma(w[0].x, cs, acc[p][0]);
@@ -287,12 +287,12 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   __shared__ __align__(16) double cbs[P * CB_SIZE];
   __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
   __shared__ double red[NW * NV], out[NV];
-  __shared__ double2 lut[256];
+  __shared__ MathTables mtab;
   __shared__ bool active[P];
   __shared__ int slot[P];
   const DevCfg& cfg = *cfgp;
   const long long p0 = (long long)blockIdx.x * P;
-  build_sincos_lut(lut, threadIdx.x, NT);
+  build_math_tables(&mtab, threadIdx.x, NT);
   if (threadIdx.x < P) slot[threadIdx.x] = threadIdx.x;
   for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
     long long p = p0 + e / CB_SIZE;
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   build_phasor_tables<NDET, NT>(cfg, cbs, P, tabL, tabW, step);
   __syncthreads();
   double acc[P][AL::N];
-  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, acc);
+  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, acc);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < P; ++p)
@@ -338,11 +338,11 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
   using AL = AccLayout<1, NDET>;
   constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) LpSmem<NDET, KR> sm;
-  __shared__ double2 lut[256];
+  __shared__ MathTables mtab;
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x;
   const int nf = cfg.n_freq;
-  build_sincos_lut(lut, tid, NT);
+  build_math_tables(&mtab, tid, NT);
   for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
     const long long grp = task / nranges;
     const int rng = (int)(task % nranges);
@@ -398,7 +398,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       for (int j = 0; j < PP; ++j) {
         const double q = phase_pn_qt(a[j], b);
         double sn, cs;
-        sincos_lut(q, lut, sn, cs);
+        sincos_lut(q, &mtab, sn, cs);
         acc[j][0] = fma(w[0].x, cs, acc[j][0]);
         acc[j][1] = fma(-w[0].x, sn, acc[j][1]);
         acc[j][0] = fma(-w[0].y, sn, acc[j][0]);
@@ -446,7 +446,9 @@ __global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restri
 template <int MODEL>
 __global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ theta, double* out) {
   __shared__ double cb[CB_SIZE];
+  __shared__ MathTables mtab;
   const DevCfg& cfg = *cfgp;
+  build_math_tables(&mtab, threadIdx.x, blockDim.x);
   if (threadIdx.x == 0) {
     double th[11];
     for (int d = 0; d < 11; ++d) th[d] = theta[d];
@@ -458,7 +460,7 @@ __global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const dou
     BinBasis b = make_basis(tb, k, MODEL == 2);
     double q, amp = 1.0;
     if (MODEL == 1) q = phase_pn_qt(cb + CB_PH, b);
-    else phenom_bin(cb, b, q, amp);
+    else phenom_bin(cb, b, &mtab, q, amp);
     double a76 = b.y3 * sqrt(b.y);   // f^-7/6
     for (int d = 0; d < cfg.n_det; ++d) {
       double s, c;
@@ -598,12 +600,12 @@ constexpr int kWalkPG = 2;     // particles per bin sweep
 
 template <int MODEL, int NDET, int PG, int NT>
 __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                            const double2* tabW, const double2* step, const double2* lut, const bool* active,
+                                            const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
                                             const int* slot, double* red, double* out /*smem [PG][N]*/) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NV = PG * AL::N;
   double acc[PG][AL::N];
-  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, acc);
+  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, mt, active, slot, acc);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < PG; ++p)
@@ -613,13 +615,13 @@ __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb,
 }
 
 template <int MODEL, int NDET>
-__global__ void __launch_bounds__(kWalkThreads, 2) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+__global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NT = kWalkThreads, NW = NT / 32, DM = kWalkDMax, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) double cbs[DM * CB_SIZE];
   __shared__ double2 tabL[DM * ND1 * 32], tabW[DM * ND1 * NW], step[DM * ND1];
   __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DM];
-  __shared__ double2 lut[256];
+  __shared__ MathTables mtab;
   __shared__ bool active[PG];
   __shared__ int slot[PG];
   __shared__ double s_cur[kMaxDim], s_prop[DM][kMaxDim], s_curl;
@@ -634,7 +636,7 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_gw(const DevCfg* __res
   const int tid = threadIdx.x;
   const long long row = blockIdx.x;
   int na = 0, ne = 0, no = 0;   // thread 0's counters
-  build_sincos_lut(lut, tid, NT);
+  build_math_tables(&mtab, tid, NT);
   if (tid == 0) {
     for (int d = 0; d < D; ++d) s_cur[d] = a.u[row * D + d];
     s_curl = a.logl[row];
@@ -683,8 +685,8 @@ __global__ void __launch_bounds__(kWalkThreads, 2) k_walk_gw(const DevCfg* __res
           active[tid] = mine >= 0;
         }
         __syncthreads();
-        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, red, out);
-        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, lut, active, slot, red, out);
+        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
+        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
         if (tid < ng) s_logl[slot[tid]] = finish_logl<MODEL, NDET>(cfg, cbs + slot[tid] * CB_SIZE, out + tid * AL::N, nullptr);
         __syncthreads();
       }

@@ -117,28 +117,37 @@ __device__ __forceinline__ void sincos_qt(double q, double& s, double& c) {
   c = __hiloint2double(c_hi, c_lo);
 }
 
-// Table-driven variant for the hot loops: the angle is given in units of 1/256 turn (u = 64 q), k = rint(u) selects
-// exp(2 pi i k / 256) from a 256-entry table in shared memory (built with sincos_qt, exact arguments) and the remainder
+// Table-driven variant for the hot loops (sincos_lut): the angle is given in units of 1/256 turn (u = 64 q), k = rint(u) selects
+// exp(2 pi i k / 256) from a 256-entry table in shared memory (MathTables::sc, built with sincos_qt on exact arguments) and the remainder
 // |r| <= 1/2 unit (|alpha| <= pi/256) needs three-term polynomials (truncation 8e-18 / 1e-20).  Compared with sincos_qt it
 // trades the quadrant selects (10 ALU instructions) and 8 FMAs for one LDS.128 and a complex product: 14 FP64 instructions
 // instead of 18, 3 integer instructions instead of 10.
 // ------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void build_sincos_lut(double2* lut /*smem [256]*/, int tid, int nthreads) {
+// Shared-memory tables of the hot loops (4.9 KB per CTA), built once per CTA.
+struct MathTables {
+  double2 sc[256];   // exp(2 pi i k / 256) = (cos, sin)
+  double e2[64];     // 2^(j/64)
+  double at[34];     // atan(j/32), j = 0..32 (+ pad)
+};
+
+__device__ __forceinline__ void build_math_tables(MathTables* mt, int tid, int nthreads) {
   for (int i = tid; i < 256; i += nthreads) {
     double s, c;
     sincos_qt(i * (1.0 / 64.0), s, c);
-    lut[i] = make_double2(c, s);
+    mt->sc[i] = make_double2(c, s);
   }
+  for (int i = tid; i < 64; i += nthreads) mt->e2[i] = exp2(i * (1.0 / 64.0));
+  for (int i = tid; i < 34; i += nthreads) mt->at[i] = atan(i * (1.0 / 32.0));
 }
 
-__device__ __forceinline__ void sincos_lut(double u, const double2* lut, double& s, double& c) {
+__device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, double& s, double& c) {
   const double magic = 6755399441055744.0;  // 1.5 * 2^52
   double kk = u + magic;
   const int ki = __double2loint(kk);
   kk -= magic;
   const double r = u - kk;
   const double z = r * r;
-  const double2 T = lut[ki & 255];
+  const double2 T = mt->sc[ki & 255];
   constexpr double h = 0.024543692606170259675;   // 2 pi / 256
   double ps = fma(z, h * h * h * h * h / 120.0, -h * h * h / 6.0);
   double pc = fma(z, -h * h * h * h * h * h / 720.0, h * h * h * h / 24.0);
@@ -148,6 +157,66 @@ __device__ __forceinline__ void sincos_lut(double u, const double2* lut, double&
   pc = fma(pc, z, 1.0);
   c = fma(T.x, pc, -(T.y * ps));
   s = fma(T.y, pc, T.x * ps);
+}
+
+// 1/d for finite normal d well inside the exponent range (no special cases): MUFU.RCP64H seed (>= 20 bits) and two Newton
+// steps (relative error 2^-20 -> 2^-40 -> 2^-80, i.e. rounding-limited).  The hot loops only divide by sums of squares of
+// O(1..1e6) magnitude.
+__device__ __forceinline__ double rcp_nr(double d) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  double e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-d, y, 1.0);
+  y = fma(y, e, y);
+  return y;
+}
+
+// exp(x) for |x| <= 700: n = rint(64 x / ln 2), r = x - n ln2/64 (two-term Cody-Waite, |r| <= 0.0055), degree-5 Taylor
+// (truncation 3.4e-17 relative), 2^(n/64) from the table and an exponent-field add.
+__device__ __forceinline__ double exp_tab(double x, const MathTables* mt) {
+  const double magic = 6755399441055744.0;
+  double t = fma(x, 92.33248261689366, magic);
+  const int n = __double2loint(t);
+  t -= magic;
+  double r = fma(t, -0.010830424696905538, x);
+  r = fma(t, 6.563929801064195e-13, r);
+  double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
+  p = fma(p, r, 1.0 / 6.0);
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  const double v = mt->e2[n & 63] * p;
+  return __hiloint2double(__double2hiint(v) + ((n >> 6) << 20), __double2loint(v));
+}
+
+// atan(y), any finite y: |y| >= 1 goes through atan(y) = sgn(y) pi/2 + atan(-1/y) written as the fraction n/d = -1/y (no
+// division); a 20-bit estimate of n/d picks the table point c = j/32, and atan(n/d) = atan(c) + atan((n - c d)/(d + c n))
+// with |t| <= 1/64 + 2^-19, so five odd Taylor terms suffice (t^11/11 < 1.3e-21).  One full reciprocal (d + c n >= 1 in
+// magnitude by construction).
+__device__ __forceinline__ double atan_tab(double y, const MathTables* mt) {
+  const int hi = __double2hiint(y);
+  const bool big = (hi & 0x7fffffff) >= 0x3ff00000;      // |y| >= 1
+  const double n = big ? -1.0 : y;
+  const double d = big ? y : 1.0;
+  const double base = big ? __hiloint2double((hi & 0x80000000) | 0x3ff921fb, 0x54442d18) : 0.0;   // sgn(y) pi/2
+  double r0;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r0) : "d"(d));
+  const double magic = 6755399441055744.0;
+  double jq = fma(n * r0, 32.0, magic);                   // j = rint(32 n/d), |j| <= 32
+  const int j = __double2loint(jq);
+  jq -= magic;
+  const double c = jq * (1.0 / 32.0);
+  const double num = fma(-c, d, n), den = fma(c, n, d);
+  const double t = num * rcp_nr(den);
+  const double z = t * t;
+  double p = fma(z, 1.0 / 9.0, -1.0 / 7.0);
+  p = fma(p, z, 0.2);
+  p = fma(p, z, -1.0 / 3.0);
+  const double at = fma(t * z, p, t);
+  const int ja = j < 0 ? -j : j;
+  const double tj = mt->at[ja];
+  return base + ((j < 0 ? -tj : tj) + at);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -483,7 +552,7 @@ __device__ __forceinline__ double phase_pn_qt(const double* a, const BinBasis& b
 }
 
 // PhenomD-form: phase [quarter turns] and amplitude factor for one bin.
-__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, double& q, double& amp) {
+__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, const MathTables* mt, double& q, double& amp) {
   const double f = b.f;
   if (f < cb[CB_FP1]) {
     const double* a = cb + CB_PH;
@@ -503,7 +572,7 @@ __device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, 
     q = fma(p[1], f, p[0]);
     q = fma(p[2], b.y3, q);
     q = fma(p[3], b.f34, q);
-    q = fma(p[4], atan((f - p[5]) * p[6]), q);
+    q = fma(p[4], atan_tab((f - p[5]) * p[6], mt), q);
   }
   if (f < cb[CB_FA1]) {
     const double* c = cb + CB_AI;
@@ -523,7 +592,7 @@ __device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, 
   } else {
     const double* c = cb + CB_AM;
     double fx = f - c[0];
-    amp = c[1] / fma(fx, fx, c[2]) * exp(c[3] * fx);
+    amp = c[1] * rcp_nr(fma(fx, fx, c[2])) * exp_tab(c[3] * fx, mt);
   }
 }
 
