@@ -192,44 +192,88 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
   }
   if (!any) return;   // block-uniform: nothing to evaluate (all proposals of this CTA were out of bounds)
   const int nf = cfg.n_freq;
-  for (int k = tid; k < nf; k += NT) {
+  // shared tail of a (particle, bin): E = amp exp(-i Phi) and the accumulations
+  auto tail = [&](int p, double q, double amp, const double2 (&w)[NDET], const double (&wsv)[NDET]) {
+    double sn, cs;
+    sincos_lut(q, mt, sn, cs);
+    if (MODEL == 2) { sn *= amp; cs *= amp; }
+    // E = cs - i sn;  X0 += conj(wd_0) E
+    acc[p][0] = fma(w[0].x, cs, acc[p][0]);
+    acc[p][1] = fma(-w[0].x, sn, acc[p][1]);
+    acc[p][0] = fma(-w[0].y, sn, acc[p][0]);
+    acc[p][1] = fma(-w[0].y, cs, acc[p][1]);
+    if (MODEL == 2) {
+      const double a2 = amp * amp;
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) acc[p][AL::kHh + d] = fma(a2, wsv[d], acc[p][AL::kHh + d]);
+    }
+#pragma unroll
+    for (int d = 0; d < ND1; ++d) {
+      const double rx = R[p][d].x, ry = R[p][d].y;
+      // G = E R_d;  dh_d += Re(conj(wd_d) G)
+      const double gr = fma(cs, rx, sn * ry);
+      const double gi = fma(cs, ry, -(sn * rx));
+      acc[p][AL::kDh + d] = fma(w[d + 1].x, gr, acc[p][AL::kDh + d]);
+      acc[p][AL::kDh + d] = fma(w[d + 1].y, gi, acc[p][AL::kDh + d]);
+      // advance the detector phasor by one sweep
+      R[p][d].x = fma(rx, St[p][d].x, -(ry * St[p][d].y));
+      R[p][d].y = fma(rx, St[p][d].y, ry * St[p][d].x);
+    }
+  };
+  // PhenomD-form: from the first sweep whose bins all lie in the merger-ringdown region of BOTH phase and amplitude for every
+  // particle of this group (about 80 % of the band), a branch-free loop with that region's 11 coefficients in registers.
+  int k_mr = nf;   // first bin of the specialised loop (multiple of NT)
+  if (MODEL == 2) {
+    double fs = 0.0;
+#pragma unroll
+    for (int p = 0; p < P; ++p) fs = fmax(fs, fmax(cbp[p][CB_FP2], cbp[p][CB_FA2]));
+    const double ks = (fs - cfg.f_min) / cfg.df + 2.0;          // two bins of margin against rounding of f_k
+    if (ks < (double)nf) k_mr = ((int)fmax(ks, 0.0) + NT - 1) / NT * NT;
+  }
+  const int k_gen = (MODEL == 2) ? min(nf, k_mr) : nf;
+  for (int k = tid; k < k_gen; k += NT) {
     const BinBasis b = make_basis(tb, k, MODEL == 2);
     double2 w[NDET];
     double wsv[NDET];
 #pragma unroll
     for (int d = 0; d < NDET; ++d) {
       w[d] = __ldg(tb.wd[d] + k);
-      if (MODEL == 2) wsv[d] = __ldg(tb.ws[d] + k);
+      wsv[d] = (MODEL == 2) ? __ldg(tb.ws[d] + k) : 0.0;
     }
 #pragma unroll
     for (int p = 0; p < P; ++p) {
       double q, amp = 1.0;
       if (MODEL == 1) q = phase_pn_qt(a[p], b);
       else { phenom_bin(cbp[p], b, mt, q, amp); q *= 64.0; }
-      double sn, cs;
-      sincos_lut(q, mt, sn, cs);
-      if (MODEL == 2) { sn *= amp; cs *= amp; }
-      // E = amp exp(-i Phi) = cs - i sn;  X0 += conj(wd_0) E
-      acc[p][0] = fma(w[0].x, cs, acc[p][0]);
-      acc[p][1] = fma(-w[0].x, sn, acc[p][1]);
-      acc[p][0] = fma(-w[0].y, sn, acc[p][0]);
-      acc[p][1] = fma(-w[0].y, cs, acc[p][1]);
-      if (MODEL == 2) {
-        const double a2 = amp * amp;
+      tail(p, q, amp, w, wsv);
+    }
+  }
+  if (MODEL == 2 && k_mr < nf) {
+    double pm[P][7], am[P][4];
 #pragma unroll
-        for (int d = 0; d < NDET; ++d) acc[p][AL::kHh + d] = fma(a2, wsv[d], acc[p][AL::kHh + d]);
-      }
+    for (int p = 0; p < P; ++p) {
 #pragma unroll
-      for (int d = 0; d < ND1; ++d) {
-        const double rx = R[p][d].x, ry = R[p][d].y;
-        // G = E R_d;  dh_d += Re(conj(wd_d) G)
-        const double gr = fma(cs, rx, sn * ry);
-        const double gi = fma(cs, ry, -(sn * rx));
-        acc[p][AL::kDh + d] = fma(w[d + 1].x, gr, acc[p][AL::kDh + d]);
-        acc[p][AL::kDh + d] = fma(w[d + 1].y, gi, acc[p][AL::kDh + d]);
-        // advance the detector phasor by one sweep
-        R[p][d].x = fma(rx, St[p][d].x, -(ry * St[p][d].y));
-        R[p][d].y = fma(rx, St[p][d].y, ry * St[p][d].x);
+      for (int i = 0; i < 5; ++i) pm[p][i] = 64.0 * cbp[p][CB_PM + i];     // phase in 1/256 turn (exact scaling)
+      pm[p][5] = cbp[p][CB_PM + 5]; pm[p][6] = cbp[p][CB_PM + 6];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) am[p][i] = cbp[p][CB_AM + i];
+    }
+    for (int k = k_mr + tid; k < nf; k += NT) {
+      const double f = __ldg(tb.f + k), f34 = __ldg(tb.f34 + k);
+      const double y3 = __ldg(tb.t01 + k).y;       // 1/f
+      double2 w[NDET];
+      double wsv[NDET];
+#pragma unroll
+      for (int d = 0; d < NDET; ++d) { w[d] = __ldg(tb.wd[d] + k); wsv[d] = __ldg(tb.ws[d] + k); }
+#pragma unroll
+      for (int p = 0; p < P; ++p) {
+        double q = fma(pm[p][1], f, pm[p][0]);
+        q = fma(pm[p][2], y3, q);
+        q = fma(pm[p][3], f34, q);
+        q = fma(pm[p][4], atan_tab((f - pm[p][5]) * pm[p][6], mt), q);
+        const double fx = f - am[p][0];
+        const double amp = am[p][1] * rcp_nr(fma(fx, fx, am[p][2])) * exp_tab(am[p][3] * fx, mt);
+        tail(p, q, amp, w, wsv);
       }
     }
   }
