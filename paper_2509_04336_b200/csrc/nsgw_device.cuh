@@ -123,6 +123,14 @@ __device__ __forceinline__ void sincos_qt(double q, double& s, double& c) {
 // trades the quadrant selects (10 ALU instructions) and 8 FMAs for one LDS.128 and a complex product: 14 FP64 instructions
 // instead of 18, 3 integer instructions instead of 10.
 // ------------------------------------------------------------------------------------------------------
+// Polynomial / reduction constants of the table-driven functions, in constant memory for the same reason as kSinQ/kCosQ.
+// kLutC: sin (h, -h^3/6, h^5/120) and cos (-h^2/2, h^4/24, -h^6/720) Taylor coefficients for h = 2 pi / 256.
+// kExpC: 64/ln2, ln2/64 (hi, lo), 1/120, 1/24, 1/6.   kAtanC: 1/9, -1/7, 1/5, -1/3.
+__constant__ double kLutC[6] = {0.02454369260617026, -2.464157476448998e-06, 7.421954185344934e-11,
+                                -0.0003011964233730883, 1.511988090879011e-08, -3.0360360343697477e-13};
+__constant__ double kExpC[6] = {92.33248261689366, -0.010830424696905538, 6.563929801064195e-13, 1.0 / 120.0, 1.0 / 24.0, 1.0 / 6.0};
+__constant__ double kAtanC[4] = {1.0 / 9.0, -1.0 / 7.0, 0.2, -1.0 / 3.0};
+
 // Shared-memory tables of the hot loops (4.9 KB per CTA), built once per CTA.
 struct MathTables {
   double2 sc[256];   // exp(2 pi i k / 256) = (cos, sin)
@@ -148,11 +156,10 @@ __device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, doubl
   const double r = u - kk;
   const double z = r * r;
   const double2 T = mt->sc[ki & 255];
-  constexpr double h = 0.024543692606170259675;   // 2 pi / 256
-  double ps = fma(z, h * h * h * h * h / 120.0, -h * h * h / 6.0);
-  double pc = fma(z, -h * h * h * h * h * h / 720.0, h * h * h * h / 24.0);
-  ps = fma(ps, z, h);
-  pc = fma(pc, z, -h * h / 2.0);
+  double ps = fma(z, kLutC[2], kLutC[1]);
+  double pc = fma(z, kLutC[5], kLutC[4]);
+  ps = fma(ps, z, kLutC[0]);
+  pc = fma(pc, z, kLutC[3]);
   ps *= r;
   pc = fma(pc, z, 1.0);
   c = fma(T.x, pc, -(T.y * ps));
@@ -176,13 +183,13 @@ __device__ __forceinline__ double rcp_nr(double d) {
 // (truncation 3.4e-17 relative), 2^(n/64) from the table and an exponent-field add.
 __device__ __forceinline__ double exp_tab(double x, const MathTables* mt) {
   const double magic = 6755399441055744.0;
-  double t = fma(x, 92.33248261689366, magic);
+  double t = fma(x, kExpC[0], magic);
   const int n = __double2loint(t);
   t -= magic;
-  double r = fma(t, -0.010830424696905538, x);
-  r = fma(t, 6.563929801064195e-13, r);
-  double p = fma(r, 1.0 / 120.0, 1.0 / 24.0);
-  p = fma(p, r, 1.0 / 6.0);
+  double r = fma(t, kExpC[1], x);
+  r = fma(t, kExpC[2], r);
+  double p = fma(r, kExpC[3], kExpC[4]);
+  p = fma(p, r, kExpC[5]);
   p = fma(p, r, 0.5);
   p = fma(p, r, 1.0);
   p = fma(p, r, 1.0);
@@ -210,9 +217,9 @@ __device__ __forceinline__ double atan_tab(double y, const MathTables* mt) {
   const double num = fma(-c, d, n), den = fma(c, n, d);
   const double t = num * rcp_nr(den);
   const double z = t * t;
-  double p = fma(z, 1.0 / 9.0, -1.0 / 7.0);
-  p = fma(p, z, 0.2);
-  p = fma(p, z, -1.0 / 3.0);
+  double p = fma(z, kAtanC[0], kAtanC[1]);
+  p = fma(p, z, kAtanC[2]);
+  p = fma(p, z, kAtanC[3]);
   const double at = fma(t * z, p, t);
   const int ja = j < 0 ? -j : j;
   const double tj = mt->at[ja];
