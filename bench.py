@@ -221,8 +221,11 @@ def run_ours(args):
         fp64_burst = nsgw.measure_fp64_peak(1 << 17)
         flops_launch = float(B) * n_freq * alg_flops_per_bin(n_det)
         ach = flops_launch / (kern_ms / kern_n * 1e-3) / 1e12
+        # DRAM bytes per launch of the dominant kernel: dram__bytes_read.sum + dram__bytes_write.sum of the committed
+        # `ncu --set full` capture of this same command (profiles/r01n_k_bins_lp_ncu_full.txt); only valid for the default batch
+        traffic = (19322624 + 6656) if (B == 65536 and n_freq == 4017) else None
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
-                "traffic": None, "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic 96 B x B = %d" % (96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
                 "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
                 "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,
@@ -281,11 +284,12 @@ def run_ours(args):
         th_np = theta[:nb].cpu().numpy()
         Pc.gw_loglike(th_np[:64])
         t0 = time.perf_counter()
-        lo = Pc.gw_loglike(th_np)
-        dt = time.perf_counter() - t0
+        for _ in range(args.cpu_passes):
+            lo = Pc.gw_loglike(th_np)
+        dt = (time.perf_counter() - t0) / args.cpu_passes
         lg = logl[:nb].cpu().numpy()
         line["cpu_baseline"] = {"value": nb / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-                                "sample": f"first {nb} of the {B} rows, OpenMP over rows, {dt:.1f} s",
+                                "sample": f"first {nb} of the {B} rows x {args.cpu_passes} passes, OpenMP over rows, {dt * args.cpu_passes:.1f} s of CPU work",
                                 "max_abs_dlogl_vs_gpu": float(np.max(np.abs(lg - lo)))}
     if rank == 0:
         print(json.dumps(line), flush=True)
@@ -312,7 +316,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--batch", type=int, default=65536)
     ap.add_argument("--ref-batch", type=int, default=1024)
-    ap.add_argument("--cpu-rows", type=int, default=16384)
+    ap.add_argument("--cpu-rows", type=int, default=65536)
+    ap.add_argument("--cpu-passes", type=int, default=3)
     ap.add_argument("--quick", action="store_true", help="skip the walk / full-run extras")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

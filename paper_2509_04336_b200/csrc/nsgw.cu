@@ -365,7 +365,7 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
 // sums in registers for the whole task), and the CTA walks a range of KR bins whose table values are staged once in shared
 // memory and read with warp-uniform (broadcast) LDS.  No per-bin global traffic, no cross-thread reduction, no phasor
 // tables: a task costs each thread 2 sincos per extra detector plus KR x (the same per-bin arithmetic as bin_loop).
-// Task = (group of NT particles, range of KR bins); partial[B][n_ranges][N] is summed in range order by k_finish.
+// Task = (group of NT PP particles, range of kr bins); partial[n_ranges][N][B] is summed in range order by k_finish.
 // Built for TaylorF2 (no per-particle branches in the bin loop; PhenomD-form's piecewise regions would diverge across lanes).
 // ------------------------------------------------------------------------------------------------------
 template <int NDET, int KR>
@@ -464,13 +464,13 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       const long long p = (grp * PP + j) * NT + tid;
       if (p < B) {
 #pragma unroll
-        for (int i = 0; i < AL::N; ++i) partial[(p * nranges + rng) * AL::N + i] = acc[j][i];
+        for (int i = 0; i < AL::N; ++i) partial[((long long)rng * AL::N + i) * B + p] = acc[j][i];   // [range][N][B]: coalesced
       }
     }
   }
 }
 
-// Adds the per-chunk partial sums in chunk order and finishes logL.
+// Adds the per-range partial sums in range order and finishes logL.
 template <int MODEL, int NDET>
 __global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restrict__ cbs_g, const double* __restrict__ partial, int nchunks,
                          long long B, double* logl, double* parts) {
@@ -482,7 +482,7 @@ __global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restri
   for (int i = 0; i < AL::N; ++i) sums[i] = 0.0;
   for (int c = 0; c < nchunks; ++c)
 #pragma unroll
-    for (int i = 0; i < AL::N; ++i) sums[i] += partial[(p * nchunks + c) * AL::N + i];
+    for (int i = 0; i < AL::N; ++i) sums[i] += partial[((long long)c * AL::N + i) * B + p];
   logl[p] = finish_logl<MODEL, NDET>(*cfgp, cbs_g + p * CB_SIZE, sums, parts ? parts + p * 2 * NDET : nullptr);
 }
 
@@ -964,7 +964,7 @@ struct ns_handle {
   double* d_cur_l = nullptr;
   int* d_cnt = nullptr;         // 3 * k
   double* d_cb = nullptr;       // coefficient blocks scratch
-  double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [B][n_ranges][N]
+  double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [n_ranges][N][B]
   size_t partial_cap = 0;
   int n_sm = 148;
   int opt_walk_spec = 0;        // 0 auto (from the acceptance rate), 1..8 fixed speculative chunk length
