@@ -274,6 +274,44 @@ def run_ours(args):
                                     "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
                                     "evals_per_s": st["n_eval_total"] / wall}
         h3.close()
+        if args.full_extras:
+            # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
+            spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
+            h4 = nsgw.Handle(spec4, smp4, seed=1)
+            t0 = time.perf_counter()
+            nit, st = h4.run(smp4["term_kind"], smp4["term_tol"], 4000)
+            logz, err, H = h4.finalize_evidence()
+            wall = time.perf_counter() - t0
+            extras["ns_run_config4"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
+                                        "logz_err": err, "H": H, "walk_len_last": st["walk_len"],
+                                        "accept_mean_last": st["accept_mean"], "evals_per_s": st["n_eval_total"] / wall}
+            h4.close()
+            # config 5: divergence and saturation sweep (H1+L1+V1, 16 s at 4096 Hz, 32449 bins); B walkers, live set of 2B points
+            spec5 = W.config5(wf_cuda_for(nsgw, torch))
+            h5 = nsgw.Handle(spec5)
+            sweep = []
+            for Bw in (256, 1024, 4096, 16384, 65536, 131072):
+                u5 = torch.as_tensor(W.config5_live(spec5, 2 * Bw)).cuda()
+                l5 = h5.loglike_u_batch(u5)
+                order = torch.argsort(l5)
+                donors = u5[order[Bw:]].contiguous()
+                lstar = float(l5[order[Bw - 1]])
+                for Wl in (20, 60, 200):
+                    if Bw * Wl > 131072 * 20:          # keep the sweep within ~1 min: larger products are extrapolations of these
+                        continue
+                    uw, lw = donors.clone(), l5[order[Bw:]].clone()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    cnt = h5.walk_batch(donors, uw, lw, lstar, Wl, 4321, 9)
+                    b.record(stream)
+                    torch.cuda.synchronize()
+                    ne, na = int(cnt["n_eval"].sum()), cnt["n_accept"].double()
+                    wms = a.elapsed_time(b)
+                    sweep.append({"B": Bw, "W": Wl, "ms": wms, "evals": ne, "evals_per_s": ne / (wms * 1e-3),
+                                  "accept_mean": float(na.mean()), "accept_std": float(na.std()), "accept_min": int(na.min()),
+                                  "accept_max": int(na.max()), "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl)})
+            extras["config5_sweep"] = sweep
+            h5.close()
         line["extras"] = extras
 
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample of the same rows (rank 0, N=1)
@@ -319,6 +357,7 @@ def main():
     ap.add_argument("--cpu-rows", type=int, default=65536)
     ap.add_argument("--cpu-passes", type=int, default=3)
     ap.add_argument("--quick", action="store_true", help="skip the walk / full-run extras")
+    ap.add_argument("--full-extras", action="store_true", help="also run the config-4 nested-sampling run and the config-5 sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":

@@ -38,7 +38,7 @@ constexpr int kWalkThreads = 128;
 struct DevState {
   double logx, logz, h, walks, delay, lstar;
   long long iter, n_eval_total;
-  int W, naccept, maxmcmc, spec;   // spec: speculative steps per chunk of the next walk
+  int W, naccept, maxmcmc, pad;
   ns_stats stats;
 };
 
@@ -536,8 +536,8 @@ struct WalkArgs {
   int* n_accept; int* n_eval; int* n_oob;
   uint8_t* tflags; double* tlogl;
   int trace_stride;
-  int spec;                 // speculative steps per chunk (1..kWalkDMax)
-  const int* spec_dev;      // if non-null overrides spec
+  int spec;                 // speculative steps per chunk: cap (1..kWalkDMax) of the per-walker adaptive length ...
+  int spec_fixed;           // ... or, if non-zero, the fixed length
 };
 
 // DE proposal for one walker (footnote P:120; R:L8-L10).  Returns false if out of bounds.
@@ -637,8 +637,8 @@ __global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
 // the in-bounds ones are swept together (PG particles per pass share every table load and supply ILP), and thread 0 then walks
 // through the D outcomes in order: out-of-bounds -> counted; logL' > L* -> accepted, and the steps after it are DISCARDED (they
 // started from a stale point) and redone in the next chunk from t0 + j + 1.  The decisions, counters and trace are exactly those
-// of the sequential algorithm (oracle_walk); only work is wasted, never semantics changed.  D is a launch argument (1 = no
-// speculation) chosen from the previous batch's acceptance rate.
+// of the sequential algorithm (oracle_walk); only work is wasted, never semantics changed.  Each walker adapts its own D
+// (start 2; halved after a chunk cut short by an acceptance, doubled up to 8 after one that was not), or D is fixed by option.
 constexpr int kWalkDMax = 8;   // speculative steps per chunk
 constexpr int kWalkPG = 2;     // particles per bin sweep
 
@@ -670,11 +670,12 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
   __shared__ int slot[PG];
   __shared__ double s_cur[kMaxDim], s_prop[DM][kMaxDim], s_curl;
   __shared__ int s_flag[DM];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
-  __shared__ int s_t0;
+  __shared__ int s_t0, s_d;
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const int W = a.W_dev ? *a.W_dev : a.W;
-  const int spec = max(1, min(DM, a.spec_dev ? *a.spec_dev : a.spec));
+  const int spec = max(1, min(DM, a.spec));   // cap of the chunk length (a.spec < 0: fixed length -a.spec)
+  const bool spec_fixed = a.spec_fixed != 0;
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
   const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
   const int tid = threadIdx.x;
@@ -685,12 +686,13 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
     for (int d = 0; d < D; ++d) s_cur[d] = a.u[row * D + d];
     s_curl = a.logl[row];
     s_t0 = 0;
+    s_d = spec_fixed ? spec : min(spec, 2);
   }
   __syncthreads();
   while (true) {
     const int t0 = s_t0;
     if (t0 >= W) break;
-    const int nd = min(spec, W - t0);
+    const int nd = min(s_d, W - t0);
     // ---- phase A: nd proposals from the current point, side by side
     if (tid < nd) {
       const int j = tid;
@@ -738,6 +740,7 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
     // ---- phase C: the nd outcomes in order; the first acceptance invalidates the rest of the chunk
     if (tid == 0) {
       int used = nd;
+      bool hit = false;
       for (int j = 0; j < nd; ++j) {
         const int t = t0 + j;
         const int fl = s_flag[j];
@@ -757,9 +760,12 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
         }
         if (a.tflags) a.tflags[row * a.trace_stride + t] = tf;
         if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
-        if (acc_) { used = j + 1; break; }
+        if (acc_) { used = j + 1; hit = true; break; }
       }
       s_t0 = t0 + used;
+      // per-walker chunk length: halve after a chunk that ended in an acceptance (the rest of it was wasted), double after one
+      // that did not; a function of the walker's own chain only, so still deterministic
+      if (!spec_fixed) s_d = hit ? max(1, s_d >> 1) : min(spec, s_d << 1);
     }
     __syncthreads();
   }
@@ -903,11 +909,6 @@ __global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __r
     double r = fmax(0.5, amean) / W;
     double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
     st->walks = walks;
-    // speculative chunk length of the next walk: keep the expected waste (steps after an acceptance) near 1/8 of the work
-    {
-      const double per_step = fmax(amean, 0.05) / W;
-      st->spec = max(1, min(kWalkDMax, (int)floor(0.25 / per_step)));
-    }
     st->n_eval_total += s_e[0];
     double lse = lmax + log(s_d[0]);
     ns_stats& o_ = st->stats;
@@ -1292,7 +1293,7 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
   memset(&hs, 0, sizeof(hs));
   hs.logx = 0.0; hs.logz = -INFINITY; hs.h = 0.0; hs.walks = cfg->walks0;
   hs.delay = (n > 0) ? (cfg->delay >= 0.0 ? cfg->delay : std::max((double)n / (10.0 * k) - 1.0, 0.0)) : 0.0;
-  hs.iter = 0; hs.n_eval_total = n; hs.W = 1; hs.spec = 2; hs.naccept = cfg->naccept; hs.maxmcmc = cfg->maxmcmc;
+  hs.iter = 0; hs.n_eval_total = n; hs.W = 1; hs.naccept = cfg->naccept; hs.maxmcmc = cfg->maxmcmc;
   INIT_CHECK(cudaMemcpyAsync(h->d_state, &hs, sizeof(hs), cudaMemcpyHostToDevice, s), -2);
   if (n > 0) {
     INIT_CHECK(cudaMalloc(&h->d_live_u, sizeof(double) * (size_t)n * D), -2);
@@ -1387,6 +1388,7 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
   a.n_accept = n_accept_dev; a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.tflags = trace_flags_dev; a.tlogl = trace_logl_dev;
   a.trace_stride = walk_len;
   a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
+  a.spec_fixed = h->opt_walk_spec > 0;
   return launch_walk(h, a, (cudaStream_t)stream);
 }
 
@@ -1407,7 +1409,8 @@ int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) 
   memset(&a, 0, sizeof(a));
   a.donors = h->d_surv; a.m = m; a.u = h->d_cur_u; a.logl = h->d_cur_l; a.B = k;
   a.lstar_dev = &h->d_state->lstar; a.W_dev = &h->d_state->W; a.iter_dev = &h->d_state->iter;
-  if (h->opt_walk_spec > 0) a.spec = h->opt_walk_spec; else a.spec_dev = &h->d_state->spec;
+  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
+  a.spec_fixed = h->opt_walk_spec > 0;
   a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
   a.n_accept = h->d_cnt; a.n_eval = h->d_cnt + k; a.n_oob = h->d_cnt + 2 * k;
   int rc = launch_walk(h, a, s);
