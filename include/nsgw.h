@@ -150,8 +150,8 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
 #define NSGW_OPT_BINS_KERNEL 0
 /* key NSGW_OPT_WALK_SPEC: speculative chunk length of the GW walk kernel (k_walk_gw evaluates that many consecutive steps of a
  * walker at once from its current point and discards the ones after an acceptance; results are identical for every value):
- * 0 = automatic (every walker adapts its own length between 1 and 8 from its chain: halved after an acceptance, doubled after
- * a chunk without one), 1..8 = fixed (1 = one step at a time). */
+ * 0 = automatic (every walker adapts its own length between 1 and 32 from its chain: halved after an acceptance, doubled
+ * after a chunk without one), 1..32 = fixed (1 = one step at a time). */
 #define NSGW_OPT_WALK_SPEC 1
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 

@@ -638,8 +638,8 @@ __global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
 // through the D outcomes in order: out-of-bounds -> counted; logL' > L* -> accepted, and the steps after it are DISCARDED (they
 // started from a stale point) and redone in the next chunk from t0 + j + 1.  The decisions, counters and trace are exactly those
 // of the sequential algorithm (oracle_walk); only work is wasted, never semantics changed.  Each walker adapts its own D
-// (start 2; halved after a chunk cut short by an acceptance, doubled up to 8 after one that was not), or D is fixed by option.
-constexpr int kWalkDMax = 8;   // speculative steps per chunk
+// (start 2; halved after a chunk cut short by an acceptance, doubled up to 32 after one that was not), or D is fixed by option.
+constexpr int kWalkDMax = 32;   // speculative steps per chunk (cap): one warp builds them side by side
 constexpr int kWalkPG = 2;     // particles per bin sweep
 
 template <int MODEL, int NDET, int PG, int NT>
@@ -658,17 +658,28 @@ __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb,
   block_reduce<NV, NT>(v, red, out);
 }
 
+template <int NDET>
+struct WalkSmem {
+  static constexpr int ND1 = NDET > 1 ? NDET - 1 : 1, NW = kWalkThreads / 32;
+  static constexpr size_t kBytes = sizeof(double2) * kWalkDMax * ND1 * (32 + NW + 1) + sizeof(double) * kWalkDMax * (CB_SIZE + kMaxDim);
+};
+
 template <int MODEL, int NDET>
 __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NT = kWalkThreads, NW = NT / 32, DM = kWalkDMax, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
-  __shared__ __align__(16) double cbs[DM * CB_SIZE];
-  __shared__ double2 tabL[DM * ND1 * 32], tabW[DM * ND1 * NW], step[DM * ND1];
+  // per-chunk buffers in dynamic shared memory (WalkSmem<NDET>::kBytes): coefficient blocks, phasor tables, proposals
+  extern __shared__ __align__(16) unsigned char walk_smem[];
+  double2* tabL = reinterpret_cast<double2*>(walk_smem);          // [DM][ND1][32]
+  double2* tabW = tabL + DM * ND1 * 32;                            // [DM][ND1][NW]
+  double2* step = tabW + DM * ND1 * NW;                            // [DM][ND1]
+  double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
+  double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
   __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DM];
   __shared__ MathTables mtab;
   __shared__ bool active[PG];
   __shared__ int slot[PG];
-  __shared__ double s_cur[kMaxDim], s_prop[DM][kMaxDim], s_curl;
+  __shared__ double s_cur[kMaxDim], s_curl;
   __shared__ int s_flag[DM];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
   __shared__ int s_t0, s_d;
   const DevCfg& cfg = *cfgp;
@@ -968,7 +979,7 @@ struct ns_handle {
   double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [n_ranges][N][B]
   size_t partial_cap = 0;
   int n_sm = 148;
-  int opt_walk_spec = 0;        // 0 auto (from the acceptance rate), 1..8 fixed speculative chunk length
+  int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
@@ -1139,7 +1150,13 @@ int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cuda
 
 template <int MODEL, int NDET>
 int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
-  k_walk_gw<MODEL, NDET><<<(unsigned)a.B, kWalkThreads, 0, s>>>(h->d_cfg, h->tb, a);
+  auto kern = k_walk_gw<MODEL, NDET>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WalkSmem<NDET>::kBytes));
+    attr_set = true;
+  }
+  kern<<<(unsigned)a.B, kWalkThreads, WalkSmem<NDET>::kBytes, s>>>(h->d_cfg, h->tb, a);
   LAUNCH_CHECK(h);
   return 0;
 }

@@ -241,7 +241,7 @@ def test_walk_speculation_is_invisible(nsgw):
     lstar = float(np.quantile(ld, 0.2))
     start = rng.integers(0, m, B)
     ref = None
-    for spec_len in (1, 2, 5, 8, 0):
+    for spec_len in (1, 2, 5, 8, 32, 0):
         h.set_option(1, spec_len)
         ug, lg_ = dev(donors[start]), dev(ld[start])
         res = h.walk_batch(dev(donors), ug, lg_, lstar, Wlen, 77, (5 << 24) | 3, slot0=0, trace=True)
