@@ -559,7 +559,9 @@ __device__ __forceinline__ double phase_pn_qt(const double* a, const BinBasis& b
 }
 
 // PhenomD-form: phase [quarter turns] and amplitude factor for one bin.
-__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, const MathTables* mt, double& q, double& amp) {
+// `ex` = exp(-gamma2 (f - f_RD)/w) of this bin, supplied by the caller (the bin loops carry it as a geometric sequence along a
+// thread's bins; k_waveform evaluates it directly).
+__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, const MathTables* mt, double ex, double& q, double& amp) {
   const double f = b.f;
   if (f < cb[CB_FP1]) {
     const double* a = cb + CB_PH;
@@ -599,7 +601,7 @@ __device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, 
   } else {
     const double* c = cb + CB_AM;
     double fx = f - c[0];
-    amp = c[1] * rcp_nr(fma(fx, fx, c[2])) * exp_tab(c[3] * fx, mt);
+    amp = c[1] * rcp_nr(fma(fx, fx, c[2])) * ex;
   }
 }
 
