@@ -548,6 +548,7 @@ struct WalkArgs {
   int trace_stride;
   int spec;                 // speculative steps per chunk: cap (1..kWalkDMax) of the per-walker adaptive length ...
   int spec_fixed;           // ... or, if non-zero, the fixed length
+  int spec_cap;             // chunk buffers in shared memory hold this many steps (>= spec)
 };
 
 // DE proposal for one walker (footnote P:120; R:L8-L10).  Returns false if out of bounds.
@@ -668,16 +669,20 @@ __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb,
   block_reduce<NV, NT>(v, red, out);
 }
 
-template <int NDET>
-struct WalkSmem {
-  static constexpr int ND1 = NDET > 1 ? NDET - 1 : 1, NW = kWalkThreads / 32;
-  static constexpr size_t kBytes = sizeof(double2) * kWalkDMax * ND1 * (32 + NW + 1) + sizeof(double) * kWalkDMax * (CB_SIZE + kMaxDim);
-};
+// dynamic shared memory of k_walk_gw for a chunk cap of dm steps
+template <int NDET, int NT>
+constexpr size_t walk_smem_bytes(int dm) {
+  return sizeof(double2) * dm * (NDET > 1 ? NDET - 1 : 1) * (32 + NT / 32 + 1) + sizeof(double) * dm * (CB_SIZE + kMaxDim);
+}
 
-template <int MODEL, int NDET>
-__global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+// NT threads per walker: 128 when all walkers of the batch are resident at 4 CTAs per SM, 96 (5 per SM) or 64 (8 per SM) when
+// that keeps a larger batch in one wave (config 4: k = 700 on 148 SMs).
+template <int MODEL, int NDET, int NT>
+__global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
   using AL = AccLayout<MODEL, NDET>;
-  constexpr int NT = kWalkThreads, NW = NT / 32, DM = kWalkDMax, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
+  constexpr int NW = NT / 32, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
+  constexpr int DMX = kWalkDMax;
+  const int DM = max(1, min(DMX, a.spec_cap));   // buffers are carved for this many steps per chunk
   // per-chunk buffers in dynamic shared memory (WalkSmem<NDET>::kBytes): coefficient blocks, phasor tables, proposals
   extern __shared__ __align__(16) unsigned char walk_smem[];
   double2* tabL = reinterpret_cast<double2*>(walk_smem);          // [DM][ND1][32]
@@ -685,12 +690,12 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
   double2* step = tabW + DM * ND1 * NW;                            // [DM][ND1]
   double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
   double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
-  __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DM];
+  __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DMX];
   __shared__ MathTables mtab;
   __shared__ bool active[PG];
   __shared__ int slot[PG];
   __shared__ double s_cur[kMaxDim], s_curl;
-  __shared__ int s_flag[DM];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
+  __shared__ int s_flag[DMX];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
   __shared__ int s_t0, s_d;
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
@@ -731,7 +736,7 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
     // the proposals that need a sweep, in order (every thread counts them the same way)
     int n_in = 0;
 #pragma unroll
-    for (int j = 0; j < DM; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
+    for (int j = 0; j < DMX; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
     if (n_in > 0) {
       build_phasor_tables<NDET, NT>(cfg, cbs, nd, tabL, tabW, step);
       __syncthreads();
@@ -741,7 +746,7 @@ __global__ void __launch_bounds__(kWalkThreads, 4) k_walk_gw(const DevCfg* __res
         if (tid < PG) {
           int cnt = 0, mine = -1, first = 0;
 #pragma unroll
-          for (int j = 0; j < DM; ++j) {
+          for (int j = 0; j < DMX; ++j) {
             if (j < nd && s_flag[j] == 2) {
               if (cnt == g) first = j;
               if (cnt == g + tid) mine = j;
@@ -1158,17 +1163,37 @@ int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cuda
   return loglike_theta(h, h->d_theta, B, logl, nullptr, s);
 }
 
-template <int MODEL, int NDET>
-int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
-  auto kern = k_walk_gw<MODEL, NDET>;
+template <int MODEL, int NDET, int NT>
+int launch_walk_gw_nt(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
+  auto kern = k_walk_gw<MODEL, NDET, NT>;
   static bool attr_set = false;
   if (!attr_set) {
-    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)WalkSmem<NDET>::kBytes));
+    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)walk_smem_bytes<NDET, NT>(kWalkDMax)));
     attr_set = true;
   }
-  kern<<<(unsigned)a.B, kWalkThreads, WalkSmem<NDET>::kBytes, s>>>(h->d_cfg, h->tb, a);
+  a.spec_cap = dm;
+  a.spec = std::min(a.spec, dm);
+  kern<<<(unsigned)a.B, NT, walk_smem_bytes<NDET, NT>(dm), s>>>(h->d_cfg, h->tb, a);
   LAUNCH_CHECK(h);
   return 0;
+}
+
+// Longest chunk buffers (32, 16 or 8 steps) with which `ctas` CTAs of the kernel still fit the SM's shared memory.
+template <int NDET, int NT>
+int walk_chunk_cap(int ctas) {
+  for (int dm = kWalkDMax; dm > 8; dm /= 2)
+    if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + 6656) <= (size_t)225 * 1024) return dm;
+  return 8;
+}
+
+// Geometry by batch size: the widest CTA (and the longest chunk buffers) that still keeps every walker resident at once.
+template <int MODEL, int NDET>
+int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
+  const long long sm = h->n_sm;
+  if (a.B <= 4 * sm || a.B > 8 * sm)   // <= 4 walkers per SM, or many waves anyway
+    return launch_walk_gw_nt<MODEL, NDET, 128>(h, a, walk_chunk_cap<NDET, 128>(4), s);
+  if (a.B <= 5 * sm) return launch_walk_gw_nt<MODEL, NDET, 96>(h, a, walk_chunk_cap<NDET, 96>(5), s);
+  return launch_walk_gw_nt<MODEL, NDET, 64>(h, a, walk_chunk_cap<NDET, 64>(8), s);
 }
 
 int launch_walk(ns_handle* h, const WalkArgs& a, cudaStream_t s) {

@@ -191,7 +191,9 @@ def _compare_traces(res_g, res_o, lstar, W_):
 # and the ones after an acceptance discarded, 3 = chunks that do not divide the walk length.  Results must not depend on it.
 @pytest.mark.parametrize("kind,B,Wlen,spec_len", [(W.LIKE_TAYLORF2, 37, 12, 8), (W.LIKE_TAYLORF2, 37, 12, 1),
                                                   (W.LIKE_PHENOMD, 2051, 3, 8), (W.LIKE_PHENOMD, 70, 10, 3),
-                                                  (W.LIKE_PHENOMD, 70, 10, 0)])
+                                                  (W.LIKE_PHENOMD, 70, 10, 0),
+                                                  # batch sizes that select the 96- and 64-thread walker CTAs (5 and 8 per SM)
+                                                  (W.LIKE_PHENOMD, 700, 4, 0), (W.LIKE_TAYLORF2, 900, 4, 0)])
 def test_walk_decision_parity(nsgw, kind, B, Wlen, spec_len):
     spec = W.gw_spec(kind, ["H1", "L1"], 4.0, 256.0, (20.0, 40.0))
     spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
