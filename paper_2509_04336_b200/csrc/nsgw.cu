@@ -67,6 +67,8 @@ __global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const d
   }
 }
 
+__global__ void k_math_tables(MathTables* mt) { build_math_tables(mt, threadIdx.x, blockDim.x); }
+
 // I_{7/3} per detector: deterministic single-CTA tree sum.
 __global__ void k_i73(DevCfg* cfg, const double* __restrict__ ws) {
   __shared__ double sh[256];
@@ -346,7 +348,7 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   __shared__ int slot[P];
   const DevCfg& cfg = *cfgp;
   const long long p0 = (long long)blockIdx.x * P;
-  build_math_tables(&mtab, threadIdx.x, NT);
+  load_math_tables(&mtab, tb.mt, threadIdx.x, NT);
   if (threadIdx.x < P) slot[threadIdx.x] = threadIdx.x;
   for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
     long long p = p0 + e / CB_SIZE;
@@ -396,7 +398,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x;
   const int nf = cfg.n_freq;
-  build_math_tables(&mtab, tid, NT);
+  load_math_tables(&mtab, tb.mt, tid, NT);
   for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
     const long long grp = task / nranges;
     const int rng = (int)(task % nranges);
@@ -502,7 +504,7 @@ __global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const dou
   __shared__ double cb[CB_SIZE];
   __shared__ MathTables mtab;
   const DevCfg& cfg = *cfgp;
-  build_math_tables(&mtab, threadIdx.x, blockDim.x);
+  load_math_tables(&mtab, tb.mt, threadIdx.x, blockDim.x);
   if (threadIdx.x == 0) {
     double th[11];
     for (int d = 0; d < 11; ++d) th[d] = theta[d];
@@ -707,7 +709,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   const int tid = threadIdx.x;
   const long long row = blockIdx.x;
   int na = 0, ne = 0, no = 0;   // thread 0's counters
-  build_math_tables(&mtab, tid, NT);
+  load_math_tables(&mtab, tb.mt, tid, NT);
   if (tid == 0) {
     for (int d = 0; d < D; ++d) s_cur[d] = a.u[row * D + d];
     s_curl = a.logl[row];
@@ -981,6 +983,7 @@ struct ns_handle {
   DevState* d_state = nullptr;
   Tables tb{};
   double* d_tab = nullptr;      // four double2 pair tables, f, f34 (10 * nf doubles)
+  MathTables* d_mtab = nullptr; // sin/cos, exp2, atan tables
   double2* d_wd = nullptr;      // [n_det][nf]
   double* d_ws = nullptr;       // [n_det][nf]
   double* d_live_u = nullptr;   // [n_live][D]
@@ -1064,7 +1067,7 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 
 // Lane-per-particle kernel (k_bins_lp): geometry and the batch size from which it is used (TaylorF2 only).
 constexpr int kLpNT = 128, kLpKR = 256, kLpPP = 2, kLpUNR = 4, kLpOCC = 3;
-constexpr long long kLpMinBatch = 4096;   // below this the CTA-per-particle kernel fills the machine better
+constexpr long long kLpMinBatch = 8192;   // below this the CTA-per-particle kernel fills the machine better
 
 int ensure_partial(ns_handle* h, size_t n) {
   if (n > h->partial_cap) {
@@ -1082,9 +1085,17 @@ int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaS
   constexpr int NT = kLpNT, PP = kLpPP;
   const long long ngroups = (B + NT * PP - 1) / (NT * PP);
   const long long grid_max = (long long)h->n_sm * kLpOCC;
-  // bins per task: as large as keeps >= 6 tasks per resident CTA (tail balance), never below 32
+  // bins per task (multiple of the unroll, 32..256): the value that minimises rounds x (bins per task + per-task overhead),
+  // rounds = ceil(tasks / resident CTAs) -- large tiles amortise the per-task set-up, small ones balance the last round
   int kr = kLpKR;
-  while (kr > 32 && ngroups * ((h->cfg.n_freq + kr - 1) / kr) < 6 * grid_max) kr /= 2;
+  {
+    double best = 1e300;
+    for (int c = 32; c <= kLpKR; c += kLpUNR) {
+      const long long nt = ngroups * ((h->cfg.n_freq + c - 1) / c);
+      const double cost = (double)((nt + grid_max - 1) / grid_max) * (c + 8);
+      if (cost < best - 1e-9) { best = cost; kr = c; }
+    }
+  }
   const int nranges = (h->cfg.n_freq + kr - 1) / kr;
   const long long ntasks = ngroups * nranges;
   const long long grid = std::min<long long>(ntasks, grid_max);
@@ -1226,7 +1237,7 @@ int64_t nsgw_launch_count(void) { return g_launches.load(); }
 
 void ns_free(ns_handle* h) {
   if (!h) return;
-  cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_wd); cudaFree(h->d_ws);
+  cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_mtab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
   cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
   if (h->h_stats) cudaFreeHost(h->h_stats);
@@ -1330,6 +1341,10 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
     k_tables<<<(unsigned)((nf + 255) / 256), 256, 0, s>>>(h->d_cfg, strain_dev, psd_dev, t2, t2 + nf, t2 + 2 * nf, t2 + 3 * nf,
                                                           h->d_tab + 8 * nf, h->d_tab + 9 * nf, h->d_wd, h->d_ws);
     g_launches.fetch_add(1);
+    INIT_CHECK(cudaMalloc(&h->d_mtab, sizeof(MathTables)), -2);
+    k_math_tables<<<1, 256, 0, s>>>(h->d_mtab);
+    g_launches.fetch_add(1);
+    h->tb.mt = h->d_mtab;
     k_i73<<<1, 256, 0, s>>>(h->d_cfg, h->d_ws);
     g_launches.fetch_add(1);
     INIT_CHECK(cudaGetLastError(), -2);

@@ -48,6 +48,7 @@ struct Tables {
   const double* f34;    // f^3/4
   const double2* wd[kMaxDet];  // 4 df d_k f_k^-7/6 / S_k   (complex)
   const double* ws[kMaxDet];   // 4 df f_k^-7/3 / S_k
+  const struct MathTables* mt; // sin/cos, 2^(j/64), atan(j/32) tables (built once per handle; CTAs copy them to shared memory)
 };
 
 // ------------------------------------------------------------------------------------------------------
@@ -146,6 +147,14 @@ __device__ __forceinline__ void build_math_tables(MathTables* mt, int tid, int n
   }
   for (int i = tid; i < 64; i += nthreads) mt->e2[i] = exp2(i * (1.0 / 64.0));
   for (int i = tid; i < 34; i += nthreads) mt->at[i] = atan(i * (1.0 / 32.0));
+}
+
+// CTA-wide copy of the handle's tables into shared memory (617 doubles).
+__device__ __forceinline__ void load_math_tables(MathTables* dst, const MathTables* __restrict__ src, int tid, int nthreads) {
+  static_assert(sizeof(MathTables) % sizeof(double) == 0, "MathTables is an array of doubles");
+  double* d = reinterpret_cast<double*>(dst);
+  const double* g = reinterpret_cast<const double*>(src);
+  for (int i = tid; i < (int)(sizeof(MathTables) / sizeof(double)); i += nthreads) d[i] = __ldg(g + i);
 }
 
 __device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, double& s, double& c) {
