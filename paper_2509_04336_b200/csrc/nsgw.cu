@@ -1067,7 +1067,7 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 
 // Lane-per-particle kernel (k_bins_lp): geometry and the batch size from which it is used (TaylorF2 only).
 constexpr int kLpNT = 128, kLpKR = 256, kLpPP = 2, kLpUNR = 4, kLpOCC = 3;
-constexpr long long kLpMinBatch = 8192;   // below this the CTA-per-particle kernel fills the machine better
+constexpr long long kLpMinBatch = 2048;   // below this the CTA-per-particle kernel fills the machine better
 
 int ensure_partial(ns_handle* h, size_t n) {
   if (n > h->partial_cap) {
