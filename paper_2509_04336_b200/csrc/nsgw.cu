@@ -269,6 +269,7 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
 #pragma unroll
       for (int i = 0; i < 4; ++i) am[p][i] = cbp[p][CB_AM + i];
     }
+#pragma unroll 2
     for (int k = k_mr + tid; k < nf; k += NT) {
       const double f = __ldg(tb.f + k), f34 = __ldg(tb.f34 + k);
       const double y3 = __ldg(tb.t01 + k).y;       // 1/f
