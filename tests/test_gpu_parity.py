@@ -155,6 +155,51 @@ def test_phenomd_three_detector_long_segment_parity(nsgw, kern):
 
 
 @pytest.mark.parametrize("kind", [W.LIKE_TAYLORF2, W.LIKE_PHENOMD])
+@pytest.mark.parametrize("dets,f_max,T", [(["H1"], 64.0, 4.0),            # one detector, 177 bins (fewer than a CTA has threads)
+                                          (["L1"], 20.25, 4.0),           # 2 bins: degenerate grid
+                                          (["H1", "L1", "V1"], 85.0, 2.0),  # three detectors, 131 bins (one ragged tile)
+                                          (["V1", "H1"], 532.5, 2.0)])    # 1026 bins: tiles of 256 plus a 2-bin tail
+def test_loglike_edge_grids_parity(nsgw, kind, dets, f_max, T):
+    spec = W.gw_spec(kind, dets, T, f_max, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 9.0, wf)
+    P = O.OracleProblem(spec)
+    th = P.prior_transform(W.uniforms(300, 11, 31))
+    logl_o, parts_o = P.gw_loglike(th, parts=True)
+    for kern in KERNELS:
+        h = nsgw.Handle(spec)
+        h.set_option(0, kern)
+        logl_g, parts_g = h.gw_loglike_batch(dev(th), parts=True)
+        _check_logl(logl_g.cpu().numpy(), parts_g.cpu().numpy(), logl_o, parts_o, len(dets))
+
+
+def test_walk_single_detector_and_three_detectors(nsgw):
+    rng = np.random.default_rng(21)
+    for dets in (["H1"], ["H1", "L1", "V1"]):
+        spec = W.gw_spec(W.LIKE_PHENOMD, dets, 4.0, 128.0, (20.0, 40.0))
+        spec = W.make_data(spec, W.INJ_C3, 10.0, wf)
+        P = O.OracleProblem(spec)
+        h = nsgw.Handle(spec)
+        m, B, Wlen = 120, 33, 9
+        u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+        donors = u_inj[None, :] + rng.normal(0, 1, (m, 11)) * np.array(W.C5_SIGMA) * 0.5
+        per = np.array(spec["periodic"], bool)
+        donors[:, per] -= np.floor(donors[:, per])
+        donors[:, ~per] = np.clip(donors[:, ~per], 1e-6, 1 - 1e-6)
+        ld = P.loglike_u(donors)
+        lstar = float(np.median(ld))
+        start = rng.integers(0, m, B)
+        u0, l0 = donors[start].copy(), ld[start].copy()
+        res_o = P.walk(donors, u0, l0, lstar, Wlen, 99, (5 << 24) | 1, slot0=0, trace=True)
+        ug, lg_ = dev(u0), dev(l0)
+        res_g = h.walk_batch(dev(donors), ug, lg_, lstar, Wlen, 99, (5 << 24) | 1, slot0=0, trace=True)
+        clean, n_exc, n_steps = _compare_traces(res_g, res_o, lstar, Wlen)
+        assert n_exc <= 2
+        for key in ("n_accept", "n_eval", "n_oob"):
+            assert np.array_equal(res_g[key].cpu().numpy()[clean], res_o[key][clean])
+        np.testing.assert_allclose(ug.cpu().numpy()[clean], res_o["u"][clean], rtol=0, atol=1e-13)
+
+
+@pytest.mark.parametrize("kind", [W.LIKE_TAYLORF2, W.LIKE_PHENOMD])
 def test_waveform_parity(nsgw, kind):
     spec = W.gw_spec(kind, ["H1", "L1", "V1"], 4.0, 1024.0, (20.0, 40.0))
     spec = W.make_data(spec, W.INJ_C3, 20.0, wf)
