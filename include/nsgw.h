@@ -126,6 +126,16 @@ int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream);
 int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host, double* dead_dev,
                void* stream);
 
+/* Runs n_runs independent samplers concurrently on one GPU (the paper's population studies, are many
+ * independent runs).  Each handle steps on a stream of its own, so the walk kernels of different runs share the SMs: one run with
+ * k = n_live/2 walkers leaves SM slots empty (3.4 walkers per SM at k = 500) and its kernels have tails; several runs fill them.
+ * Every run is bit-identical to the same handle driven by ns_run.  All runs use the same termination rule; a finished run stops
+ * stepping.  last_host[n_runs], iters_host[n_runs] (either may be NULL) receive each run's last statistics and iteration count;
+ * dead_dev (may be NULL, and so may its entries) holds one [max_iter * k, ndim+3] device buffer per run.  Synchronises once per
+ * round.  Returns the total number of iterations performed, or a negative error code. */
+int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host,
+                    int64_t* iters_host, double** dead_dev);
+
 /* Copies the live set out: u_dev [n_live, ndim], logl_dev [n_live] (either may be NULL). */
 int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream);
 

@@ -984,6 +984,7 @@ struct ns_handle {
   DevState* d_state = nullptr;
   Tables tb{};
   double* d_tab = nullptr;      // four double2 pair tables, f, f34 (10 * nf doubles)
+  cudaStream_t s_own = nullptr; // ns_run_many: this run's stream
   MathTables* d_mtab = nullptr; // sin/cos, exp2, atan tables
   double2* d_wd = nullptr;      // [n_det][nf]
   double* d_ws = nullptr;       // [n_det][nf]
@@ -1241,6 +1242,7 @@ void ns_free(ns_handle* h) {
   cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_mtab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
   cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
+  if (h->s_own) cudaStreamDestroy(h->s_own);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -1460,10 +1462,11 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
   return launch_walk(h, a, (cudaStream_t)stream);
 }
 
-int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) {
-  if (!h) return -3;
-  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
-  cudaStream_t s = (cudaStream_t)stream;
+}  // extern "C"
+
+namespace {
+// One nested-sampling iteration enqueued on stream s (no synchronisation, no host read-back).
+int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
   const int n = h->cfg.n_live, k = h->cfg.n_delete, D = h->cfg.ndim, m = n - k;
   const uint32_t k0 = (uint32_t)(h->seed & 0xFFFFFFFFull), k1 = (uint32_t)(h->seed >> 32);
   k_rank<<<(n + 255) / 256, 256, 0, s>>>(h->d_live_l, n, h->d_order);
@@ -1487,6 +1490,18 @@ int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) 
   LAUNCH_CHECK(h);
   k_adapt<<<1, 256, 0, s>>>(h->d_state, h->d_cnt, h->d_cnt + k, h->d_cnt + 2 * k, k, h->d_live_l, n);
   LAUNCH_CHECK(h);
+  return 0;
+}
+}  // namespace
+
+extern "C" {
+
+int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) {
+  if (!h) return -3;
+  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = step_enqueue(h, dead_dev, s);
+  if (rc) return rc;
   if (stats_host) {
     CU_CHECK(h, cudaMemcpyAsync(h->h_stats, &h->d_state->stats, sizeof(ns_stats), cudaMemcpyDeviceToHost, s));
     CU_CHECK(h, cudaStreamSynchronize(s));
@@ -1511,6 +1526,49 @@ int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_ite
   }
   if (last_host) *last_host = st;
   return it;
+}
+
+int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host,
+                    int64_t* iters_host, double** dead_dev) {
+  if (!hs || n_runs < 1 || term_kind < 0 || term_kind > 1 || max_iter < 0) return -1;
+  for (int r = 0; r < n_runs; ++r) {
+    if (!hs[r]) return -3;
+    if (hs[r]->cfg.n_live <= 0) return fail(hs[r], -3, "handle has no live set");
+    if (!hs[r]->s_own && cudaStreamCreateWithFlags(&hs[r]->s_own, cudaStreamNonBlocking) != cudaSuccess)
+      return fail(hs[r], -2, "cudaStreamCreate");
+  }
+  std::vector<char> active(n_runs, 1);
+  std::vector<int64_t> it(n_runs, 0);
+  std::vector<ns_stats> st(n_runs);
+  memset(st.data(), 0, sizeof(ns_stats) * n_runs);
+  int64_t total = 0;
+  int n_active = max_iter > 0 ? n_runs : 0;
+  while (n_active > 0) {
+    // enqueue one iteration of every unfinished run on its own stream: the runs' kernels overlap on the device and fill the
+    // SM slots a single run with k = n_live/2 walkers leaves empty (and one another's tails)
+    for (int r = 0; r < n_runs; ++r) {
+      if (!active[r]) continue;
+      ns_handle* h = hs[r];
+      const size_t stride = (size_t)h->cfg.n_delete * (h->cfg.ndim + 3);
+      int rc = step_enqueue(h, (dead_dev && dead_dev[r]) ? dead_dev[r] + it[r] * stride : nullptr, h->s_own);
+      if (rc) return rc;
+      CU_CHECK(h, cudaMemcpyAsync(h->h_stats, &h->d_state->stats, sizeof(ns_stats), cudaMemcpyDeviceToHost, h->s_own));
+    }
+    for (int r = 0; r < n_runs; ++r) {
+      if (!active[r]) continue;
+      ns_handle* h = hs[r];
+      CU_CHECK(h, cudaStreamSynchronize(h->s_own));
+      st[r] = *h->h_stats;
+      ++it[r]; ++total;
+      const bool done = (term_kind == 0) ? (st[r].dlogz < term_tol) : (st[r].live_frac_log < std::log(term_tol));
+      if (done || it[r] >= max_iter) { active[r] = 0; --n_active; }
+    }
+  }
+  for (int r = 0; r < n_runs; ++r) {
+    if (last_host) last_host[r] = st[r];
+    if (iters_host) iters_host[r] = it[r];
+  }
+  return total;
 }
 
 int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream) {

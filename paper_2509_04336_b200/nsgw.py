@@ -43,7 +43,7 @@ class NsStats(C.Structure):
 
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
-           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_get_live", "ns_finalize_evidence",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_get_live", "ns_finalize_evidence",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 _lib = None
@@ -60,6 +60,7 @@ def lib():
         L.ns_last_error.restype = C.c_char_p
         L.ns_last_error.argtypes = [C.c_void_p]
         L.ns_run.restype = C.c_int64
+        L.ns_run_many.restype = C.c_int64
         L.nsgw_launch_count.restype = C.c_int64
         L.ns_free.restype = None
         L.ns_free.argtypes = [C.c_void_p]
@@ -244,6 +245,22 @@ class Handle:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         self._check(lib().ns_finalize_evidence(self._h, C.byref(a), C.byref(b), C.byref(c), _stream()), "ns_finalize_evidence")
         return a.value, b.value, c.value
+
+
+def run_many(handles, term_kind, term_tol, max_iter, dead=None):
+    """ns_run_many: steps the handles' samplers concurrently (one stream each).  Returns (iterations per run, stats per run)."""
+    n = len(handles)
+    hs = (C.c_void_p * n)(*[h._h for h in handles])
+    st = (NsStats * n)()
+    its = (C.c_int64 * n)()
+    dd = None
+    if dead is not None:
+        dd = (C.c_void_p * n)(*[C.c_void_p(d.data_ptr()) if d is not None else C.c_void_p(0) for d in dead])
+    rc = lib().ns_run_many(hs, C.c_int32(n), C.c_int32(term_kind), C.c_double(term_tol), C.c_int64(max_iter), st, its, dd)
+    if rc < 0:
+        msgs = "; ".join(lib().ns_last_error(h._h).decode() for h in handles)
+        raise NsgwError(f"ns_run_many failed ({rc}): {msgs}")
+    return [int(x) for x in its], [s_.as_dict() for s_ in st]
 
 
 def measure_fp64_peak(iters=1 << 18):

@@ -537,6 +537,32 @@ def test_gw_full_run_vs_oracle_run_statistics(nsgw):
     assert min(pvals) > 0.01 / len(free), pvals
 
 
+def test_run_many_equals_single_runs(nsgw):
+    """ns_run_many steps several samplers concurrently on streams of their own; every run must be bit-identical to the same
+    handle driven alone by ns_run (toy and GW problems mixed in one call, different lengths)."""
+    spec1, smp1, _ = W.config1()
+    specg = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 128.0, (20.0, 40.0))
+    specg = W.make_data(specg, W.INJ_C3, 10.0, wf)
+    smpg = dict(n_live=300, n_delete=150, naccept=10, maxmcmc=200, walks0=20.0, delay=-1.0)
+    jobs = [(spec1, smp1, 3), (specg, smpg, 4), (spec1, smp1, 5), (specg, smpg, 6)]
+    max_it = 90
+    single = []
+    for spec, smp, seed in jobs:
+        h = nsgw.Handle(spec, smp, seed=seed)
+        n, st = h.run(0, 0.5, max_it)
+        single.append((n, st, h.finalize_evidence(), h.get_live()[0].cpu().numpy()))
+    hs = [nsgw.Handle(spec, smp, seed=seed) for spec, smp, seed in jobs]
+    dead = [torch.zeros(max_it * smp["n_delete"], spec["ndim"] + 3, dtype=torch.float64, device="cuda") for spec, smp, _ in jobs]
+    its, sts = nsgw.run_many(hs, 0, 0.5, max_it, dead=dead)
+    assert len(set(its)) > 1                                          # runs of different lengths in one call
+    for h, n_m, st_m, (n_s, st_s, fin_s, live_s), d, (spec, smp, _) in zip(hs, its, sts, single, dead, jobs):
+        assert n_m == n_s and st_m == st_s
+        assert h.finalize_evidence() == fin_s
+        assert np.array_equal(h.get_live()[0].cpu().numpy(), live_s)
+        rows = d.cpu().numpy()[: n_m * smp["n_delete"]]
+        assert np.all(np.diff(rows[:, spec["ndim"]]) >= 0)            # dead points come out in ascending logL
+
+
 def test_error_codes(nsgw, c2):
     import ctypes as C
     h = nsgw.Handle(c2)
