@@ -275,6 +275,19 @@ def run_ours(args):
                                     "evals_per_s": st["n_eval_total"] / wall}
         h3.close()
         if args.full_extras:
+            # four config-3 runs with different seeds at once (ns_run_many): the runs' walk kernels share the SMs
+            hs = [nsgw.Handle(spec3, smp3, seed=sd) for sd in (1, 2, 3, 4)]
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            its, sts = nsgw.run_many(hs, smp3["term_kind"], smp3["term_tol"], 4000)
+            fins = [hh.finalize_evidence() for hh in hs]
+            wall = time.perf_counter() - t0
+            ev = sum(st_["n_eval_total"] for st_ in sts)
+            extras["ns_run_many_4x_config3"] = {"wall_s": wall, "iterations": its, "n_eval_total": ev, "evals_per_s": ev / wall,
+                                                "logz": [f_[0] for f_ in fins], "logz_err": [f_[1] for f_ in fins],
+                                                "wall_s_per_run": wall / len(hs)}
+            for hh in hs:
+                hh.close()
             # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
             spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
             h4 = nsgw.Handle(spec4, smp4, seed=1)
