@@ -158,10 +158,11 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * PhenomD-form the value 2 falls back to 1).  Both compute the same sums in a different, fixed order.
  * Returns -1 for an unknown key or value. */
 #define NSGW_OPT_BINS_KERNEL 0
-/* key NSGW_OPT_WALK_SPEC: speculative chunk length of the GW walk kernel (k_walk_gw evaluates that many consecutive steps of a
- * walker at once from its current point and discards the ones after an acceptance; results are identical for every value):
- * 0 = automatic (every walker adapts its own length between 1 and 32 from its chain: halved after an acceptance, doubled
- * after a chunk without one), 1..32 = fixed (1 = one step at a time). */
+/* key NSGW_OPT_WALK_SPEC: speculative chunk size of the GW walk kernel.  k_walk_gw proposes consecutive steps of a walker from
+ * its current point until that many of them are in bounds (at most 128 steps), sets those up and evaluates them together, and
+ * discards the steps after the first acceptance; results are identical for every value.  0 = automatic (every walker adapts
+ * its own size between 1 and 32 from its chain: halved after a chunk with an acceptance, doubled after one without),
+ * 1..32 = fixed (1 = one likelihood evaluation at a time, the sequential algorithm). */
 #define NSGW_OPT_WALK_SPEC 1
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 

@@ -646,15 +646,17 @@ __global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
 //
 // A walker's chain is serial (proposal t+1 starts from the point accepted at t), and one step is: propose + transform + ~3 kflop
 // of serial waveform set-up by ONE thread, then a bin sweep.  With acceptance rates of 0.1-10 % per step the outcome "rejected" is
-// almost certain, so the kernel evaluates the next D steps AT ONCE, all from the current point: lanes 0..D-1 of warp 0 build the
-// D proposals (Philox counters t0..t0+D-1) and their coefficient blocks side by side (SIMT: D set-ups for the latency of one),
-// the in-bounds ones are swept together (PG particles per pass share every table load and supply ILP), and thread 0 then walks
-// through the D outcomes in order: out-of-bounds -> counted; logL' > L* -> accepted, and the steps after it are DISCARDED (they
-// started from a stale point) and redone in the next chunk from t0 + j + 1.  The decisions, counters and trace are exactly those
-// of the sequential algorithm (oracle_walk); only work is wasted, never semantics changed.  Each walker adapts its own D
-// (start 2; halved after a chunk cut short by an acceptance, doubled up to 32 after one that was not), or D is fixed by option.
-constexpr int kWalkDMax = 32;   // speculative steps per chunk (cap): one warp builds them side by side
+// almost certain, so the kernel works on a CHUNK of future steps at once, all proposed from the current point: warp 0 draws the
+// proposals of steps t0, t0+1, ... 32 at a time (Philox counters are per step) until E of them are in bounds, builds the E
+// coefficient blocks side by side (SIMT: E set-ups for the latency of one), the physical ones are swept PG at a time (shared
+// table loads, ILP), and thread 0 then walks through the chunk's steps in order: out-of-bounds -> counted; logL' > L* -> accepted,
+// and the steps after it are DISCARDED (they started from a stale point) and redone in the next chunk from t0 + j + 1.  The
+// decisions, counters and trace are exactly those of the sequential algorithm (oracle_walk); only work is wasted, never semantics
+// changed.  Each walker adapts its own E (start 2; halved after a chunk with an acceptance, doubled up to the slot cap after one
+// without), or E is fixed by option.
+constexpr int kWalkDMax = 32;   // evaluations per chunk (cap): one warp sets them up side by side
 constexpr int kWalkPG = 2;     // particles per bin sweep
+constexpr int kWalkSteps = 128;   // steps per chunk (cap): proposals are drawn 32 at a time until enough are in bounds
 
 template <int MODEL, int NDET, int PG, int NT>
 __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
@@ -698,16 +700,18 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   __shared__ bool active[PG];
   __shared__ int slot[PG];
   __shared__ double s_cur[kMaxDim], s_curl;
-  __shared__ int s_flag[DMX];   // 0 out of bounds, 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
-  __shared__ int s_t0, s_d;
+  __shared__ double s_stage[32][kMaxDim];       // phase A1: one proposal per lane of warp 0
+  __shared__ int s_flag[DMX];                   // per slot: 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
+  __shared__ unsigned char s_step[kWalkSteps];  // per step of the chunk: 0 out of bounds, else slot + 1
+  __shared__ int s_t0, s_d, s_nsteps, s_nslots;
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const int W = a.W_dev ? *a.W_dev : a.W;
-  const int spec = max(1, min(DM, a.spec));   // cap of the chunk length (a.spec < 0: fixed length -a.spec)
+  const int spec = max(1, min(DM, a.spec));   // cap of the evaluations per chunk
   const bool spec_fixed = a.spec_fixed != 0;
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
   const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid & 31;
   const long long row = blockIdx.x;
   int na = 0, ne = 0, no = 0;   // thread 0's counters
   load_math_tables(&mtab, tb.mt, tid, NT);
@@ -721,21 +725,44 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   while (true) {
     const int t0 = s_t0;
     if (t0 >= W) break;
-    const int nd = min(s_d, W - t0);
-    // ---- phase A: nd proposals from the current point, side by side
-    if (tid < nd) {
-      const int j = tid;
-      bool inb = de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur, s_prop[j]);
-      int fl = 0;
-      if (inb) {
+    // ---- phase A (warp 0).  A1: propose steps t0, t0+1, ... 32 at a time from the current point until s_d of them are in
+    // bounds (out-of-bounds steps cost a Philox block and 11 FMAs, nothing else) or the step cap is reached; the chunk ends with
+    // the step of the last collected in-bounds proposal.  A2: the expensive part -- prior transform and waveform set-up -- for the
+    // collected proposals, one per lane, all lanes busy.
+    if (tid < 32) {
+      const int emax = s_d;
+      int nslots = 0, nsteps = 0;
+      while (nslots < emax && nsteps < kWalkSteps && t0 + nsteps < W) {
+        const int j = nsteps + lane;
+        const bool live = j < kWalkSteps && t0 + j < W;
+        const bool inb = live && de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur, s_stage[lane]);
+        const unsigned bal = __ballot_sync(0xffffffffu, inb);
+        const int rank = __popc(bal & ((1u << lane) - 1u));
+        const int room = emax - nslots, cnt = __popc(bal);
+        int consumed = min(32, min(kWalkSteps - nsteps, W - t0 - nsteps));
+        if (cnt > room) {   // more in-bounds proposals than slots left: stop right after the room-th one
+          const unsigned m2 = __ballot_sync(0xffffffffu, inb && rank == room - 1);
+          consumed = __ffs(m2);
+        }
+        if (lane < consumed) {
+          s_step[j] = inb ? (unsigned char)(nslots + rank + 1) : 0;
+          if (inb)
+            for (int d = 0; d < D; ++d) s_prop[nslots + rank][d] = s_stage[lane][d];
+        }
+        nslots += min(cnt, room);
+        nsteps += consumed;
+        __syncwarp();
+      }
+      if (lane == 0) { s_nsteps = nsteps; s_nslots = nslots; }
+      if (lane < nslots) {
         double th[11];
 #pragma unroll
-        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[j][d]);
-        fl = setup_particle<MODEL>(cfg, th, cbs + j * CB_SIZE) ? 2 : 1;
+        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[lane][d]);
+        s_flag[lane] = setup_particle<MODEL>(cfg, th, cbs + lane * CB_SIZE) ? 2 : 1;
       }
-      s_flag[j] = fl;
     }
     __syncthreads();
+    const int nd = s_nslots, nsteps = s_nsteps;
     // the proposals that need a sweep, in order (every thread counts them the same way)
     int n_in = 0;
 #pragma unroll
@@ -766,25 +793,25 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
         __syncthreads();
       }
     }
-    // ---- phase C: the nd outcomes in order; the first acceptance invalidates the rest of the chunk
+    // ---- phase C: the chunk's steps in order; the first acceptance invalidates the rest of the chunk
     if (tid == 0) {
-      int used = nd;
+      int used = nsteps;
       bool hit = false;
-      for (int j = 0; j < nd; ++j) {
+      for (int j = 0; j < nsteps; ++j) {
         const int t = t0 + j;
-        const int fl = s_flag[j];
-        if (fl == 0) {
+        const int sl = (int)s_step[j] - 1;
+        if (sl < 0) {
           ++no;
           if (a.tflags) a.tflags[row * a.trace_stride + t] = 1;
           if (a.tlogl) a.tlogl[row * a.trace_stride + t] = nan("");
           continue;
         }
         ++ne;
-        const double pl = (fl == 2) ? s_logl[j] : -INFINITY;
+        const double pl = (s_flag[sl] == 2) ? s_logl[sl] : -INFINITY;
         uint8_t tf = 4;
         const bool acc_ = pl > lstar;
         if (acc_) {
-          for (int d = 0; d < D; ++d) s_cur[d] = s_prop[j][d];
+          for (int d = 0; d < D; ++d) s_cur[d] = s_prop[sl][d];
           s_curl = pl; ++na; tf |= 2;
         }
         if (a.tflags) a.tflags[row * a.trace_stride + t] = tf;
@@ -792,8 +819,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
         if (acc_) { used = j + 1; hit = true; break; }
       }
       s_t0 = t0 + used;
-      // per-walker chunk length: halve after a chunk that ended in an acceptance (the rest of it was wasted), double after one
-      // that did not; a function of the walker's own chain only, so still deterministic
+      // per-walker chunk size (evaluations): halve after a chunk that ended in an acceptance (the rest of it was wasted), double
+      // after one that did not; a function of the walker's own chain only, so still deterministic
       if (!spec_fixed) s_d = hit ? max(1, s_d >> 1) : min(spec, s_d << 1);
     }
     __syncthreads();
@@ -1195,7 +1222,7 @@ int launch_walk_gw_nt(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
 template <int NDET, int NT>
 int walk_chunk_cap(int ctas) {
   for (int dm = kWalkDMax; dm > 8; dm /= 2)
-    if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + 6656) <= (size_t)225 * 1024) return dm;
+    if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + 10496) <= (size_t)225 * 1024) return dm;
   return 8;
 }
 
