@@ -440,8 +440,16 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       for (int i = 0; i < AL::N; ++i) acc[j][i] = 0.0;
     }
     __syncthreads();
+    // Detectors d >= 1: sum_k conj(wd_k) E_k R_k with R_k = R_0 rho^k is evaluated as R_0 * Horner(rho) over the tile's bins in
+    // DESCENDING order, S <- S rho + conj(wd_k) E_k (8 FP64 instructions per bin instead of 10 for product + accumulate + phasor
+    // advance).  The zero-weight padding bins come first and leave S = 0.
+    double2 S[PP][ND1s];
+#pragma unroll
+    for (int j = 0; j < PP; ++j)
+#pragma unroll
+      for (int d = 0; d < ND1s; ++d) S[j][d] = make_double2(0.0, 0.0);
 #pragma unroll UNR
-    for (int kk = 0; kk < nk2; ++kk) {
+    for (int kk = nk2 - 1; kk >= 0; --kk) {
       BinBasis b;
       { const double2 v = sm.t01[kk]; b.y5 = v.x; b.y3 = v.y; }
       { const double2 v = sm.t23[kk]; b.y2 = v.x; b.y = v.y; }
@@ -462,16 +470,18 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
         acc[j][1] = fma(-w[0].y, cs, acc[j][1]);
 #pragma unroll
         for (int d = 0; d < ND1; ++d) {
-          const double rx = R[j][d].x, ry = R[j][d].y;
-          const double gr = fma(cs, rx, sn * ry);
-          const double gi = fma(cs, ry, -(sn * rx));
-          acc[j][AL::kDh + d] = fma(w[d + 1].x, gr, acc[j][AL::kDh + d]);
-          acc[j][AL::kDh + d] = fma(w[d + 1].y, gi, acc[j][AL::kDh + d]);
-          R[j][d].x = fma(rx, St[j][d].x, -(ry * St[j][d].y));
-          R[j][d].y = fma(rx, St[j][d].y, ry * St[j][d].x);
+          const double ax = fma(w[d + 1].x, cs, -(w[d + 1].y * sn));      // conj(wd) E, E = cs - i sn
+          const double ay = -fma(w[d + 1].x, sn, w[d + 1].y * cs);
+          const double sx = S[j][d].x, sy = S[j][d].y;
+          S[j][d].x = fma(sx, St[j][d].x, fma(-sy, St[j][d].y, ax));
+          S[j][d].y = fma(sx, St[j][d].y, fma(sy, St[j][d].x, ay));
         }
       }
     }
+#pragma unroll
+    for (int j = 0; j < PP; ++j)
+#pragma unroll
+      for (int d = 0; d < ND1; ++d) acc[j][AL::kDh + d] = fma(R[j][d].x, S[j][d].x, -(R[j][d].y * S[j][d].y));   // Re(R_0 S)
 #pragma unroll
     for (int j = 0; j < PP; ++j) {
       const long long p = (grp * PP + j) * NT + tid;
