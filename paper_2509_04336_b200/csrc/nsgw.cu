@@ -1105,7 +1105,14 @@ int ensure_theta(ns_handle* h, long long B) {
 int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 
 // Lane-per-particle kernel (k_bins_lp): geometry and the batch size from which it is used (TaylorF2 only).
-constexpr int kLpNT = 128, kLpKR = 256, kLpPP = 2, kLpUNR = 4, kLpOCC = 3;
+// (the four numbers can be overridden at compile time for tuning sweeps)
+#ifndef NSGW_LP_NT
+#define NSGW_LP_NT 128
+#define NSGW_LP_PP 2
+#define NSGW_LP_UNR 4
+#define NSGW_LP_OCC 3
+#endif
+constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
 constexpr long long kLpMinBatch = 2048;   // below this the CTA-per-particle kernel fills the machine better
 
 int ensure_partial(ns_handle* h, size_t n) {
