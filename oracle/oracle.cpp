@@ -827,3 +827,185 @@ int64_t orc_run(orc_state* s, int32_t term_kind, double tol, int64_t max_iter, o
 double orc_neff(int32_t n, int32_t k) { return k / std::log((double)n / (double)(n - k)); }
 
 }  // extern "C"
+
+// =============================================================================================
+// Relative binning ("heterodyned likelihood"; P:155 says the paper does NOT use it, P:172, P:338 and P:503 name it as the remedy
+// for the bins x samples cost).  The paper gives no formula: DESIGN.md reading R:L24 restates the published scheme
+// (Zackay, Dai & Venumadhav 2018, as in bilby's relative-binning likelihood) and this is that reading, step by step:
+//  1. fiducial theta0 -> h0_d(f_k) on the full grid;
+//  2. bin edges: Delta(f) = 2 pi chi sum_gamma sgn(gamma) (f / f*_gamma)^gamma, gamma in {-5/3, -2/3, 1, 5/3, 7/3}, f*_gamma = f_min
+//     for gamma < 0 and f_max for gamma > 0 (monotone increasing); N_b = max(1, floor((Delta(f_max) - Delta(f_min)) / eps)) bins
+//     equally spaced in Delta; edge i = first grid index with Delta(f_k) - Delta(f_0) >= i (Delta_tot / N_b); edge N_b = N_f - 1;
+//     duplicates removed;
+//  3. summary data per detector and bin b (grid indices [e_b, e_b+1), the last bin also holds e_Nb), f_m = (f_lo + f_hi)/2:
+//     A0 = 4 df sum d conj(h0)/S, A1 = 4 df sum d conj(h0)/S (f - f_m), B0 = 4 df sum |h0|^2/S, B1 = 4 df sum |h0|^2/S (f - f_m);
+//  4. for theta: r = h(f_e; theta)/h0(f_e) at the edges, per bin r0 = (r_lo + r_hi)/2, r1 = (r_hi - r_lo)/(f_hi - f_lo);
+//     <d,h> ~ Re sum_b [A0 conj(r0) + A1 conj(r1)],  <h,h> ~ sum_b [B0 |r0|^2 + 2 B1 Re(r0 conj(r1))].
+// It is an approximation: exact when r is constant (same waveform up to amplitude/phase: the d_L and phase directions) and second
+// order in the bin width otherwise.  Pins: tests/test_oracle_relbin.py.
+// =============================================================================================
+namespace {
+
+struct RelBin {
+  int n_det = 0, n_bins = 0;
+  std::vector<int> edge;            // [n_bins + 1] grid indices
+  std::vector<double> fe;           // [n_bins + 1]
+  std::vector<double> h0;           // [n_det][n_bins + 1][2]
+  std::vector<double> A0, A1;       // [n_det][n_bins][2]
+  std::vector<double> B0, B1;       // [n_det][n_bins]
+};
+
+double relbin_delta(double f, double f_lo, double f_hi, double chi) {
+  const double g[5] = {-5.0 / 3.0, -2.0 / 3.0, 1.0, 5.0 / 3.0, 7.0 / 3.0};
+  double s = 0.0;
+  for (int i = 0; i < 5; ++i) s += (g[i] < 0.0) ? -std::pow(f / f_lo, g[i]) : std::pow(f / f_hi, g[i]);
+  return 2.0 * PI * chi * s;
+}
+
+// detector-frame waveform of theta at one frequency for every detector: out[n_det][2]
+void waveform_at(const orc_problem* p, const Waveform& w, const double* th, const double* fp, const double* fx, const double* dt,
+                 double f, double* out) {
+  double amp, psi0;
+  waveform_amp_phase(w, f, &amp, &psi0);
+  const double ci = std::cos(th[5]);
+  for (int det = 0; det < p->n_det; ++det) {
+    double cre = fp[det] * 0.5 * (1.0 + ci * ci), cim = -fx[det] * ci;
+    double Phi = psi0 + 2.0 * PI * f * (th[8] + dt[det]);
+    double c = std::cos(Phi), s_ = std::sin(Phi);
+    out[2 * det] = amp * (cre * c + cim * s_);
+    out[2 * det + 1] = amp * (cim * c - cre * s_);
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+void* orc_relbin_create(const orc_problem* p, const double* theta0, double chi, double eps) {
+  if (!theta_physical(theta0) || !(eps > 0.0) || !(chi > 0.0) || p->n_freq < 2) return nullptr;
+  RelBin* rb = new RelBin();
+  const int nf = p->n_freq, nd = p->n_det;
+  rb->n_det = nd;
+  const double f_lo = p->f_min, f_hi = p->f_min + (nf - 1) * p->df;
+  const double d0 = relbin_delta(f_lo, f_lo, f_hi, chi), dtot = relbin_delta(f_hi, f_lo, f_hi, chi) - d0;
+  const int nb_req = std::max(1, (int)std::floor(dtot / eps));
+  // step 2: edges
+  std::vector<int> e;
+  e.push_back(0);
+  int k = 0;
+  for (int i = 1; i < nb_req; ++i) {
+    const double target = i * (dtot / nb_req);
+    while (k < nf - 1 && relbin_delta(p->f_min + k * p->df, f_lo, f_hi, chi) - d0 < target) ++k;
+    if (k > e.back() && k < nf - 1) e.push_back(k);
+  }
+  e.push_back(nf - 1);
+  rb->edge = e;
+  rb->n_bins = (int)e.size() - 1;
+  const int nb = rb->n_bins;
+  rb->fe.resize(nb + 1);
+  for (int i = 0; i <= nb; ++i) rb->fe[i] = p->f_min + e[i] * p->df;
+  // step 1: fiducial waveform on the grid
+  Waveform w0 = make_waveform(p, theta0);
+  std::vector<double> fp(nd), fx(nd), dt(nd);
+  for (int det = 0; det < nd; ++det) detector_response(p, det, theta0[9], theta0[10], theta0[6], &fp[det], &fx[det], &dt[det]);
+  std::vector<double> hk(2 * nd);
+  rb->h0.assign((size_t)nd * (nb + 1) * 2, 0.0);
+  for (int i = 0; i <= nb; ++i) {
+    waveform_at(p, w0, theta0, fp.data(), fx.data(), dt.data(), rb->fe[i], hk.data());
+    for (int det = 0; det < nd; ++det) {
+      rb->h0[((size_t)det * (nb + 1) + i) * 2] = hk[2 * det];
+      rb->h0[((size_t)det * (nb + 1) + i) * 2 + 1] = hk[2 * det + 1];
+    }
+  }
+  // step 3: summary data
+  rb->A0.assign((size_t)nd * nb * 2, 0.0); rb->A1.assign((size_t)nd * nb * 2, 0.0);
+  rb->B0.assign((size_t)nd * nb, 0.0); rb->B1.assign((size_t)nd * nb, 0.0);
+  for (int b = 0; b < nb; ++b) {
+    const int k_lo = e[b], k_hi = (b == nb - 1) ? e[b + 1] + 1 : e[b + 1];
+    const double fm = 0.5 * (rb->fe[b] + rb->fe[b + 1]);
+    std::vector<long double> a0r(nd, 0.0L), a0i(nd, 0.0L), a1r(nd, 0.0L), a1i(nd, 0.0L), b0(nd, 0.0L), b1(nd, 0.0L);
+    for (int kk = k_lo; kk < k_hi; ++kk) {
+      const double f = p->f_min + kk * p->df;
+      waveform_at(p, w0, theta0, fp.data(), fx.data(), dt.data(), f, hk.data());
+      for (int det = 0; det < nd; ++det) {
+        const double dr = p->strain[((size_t)det * nf + kk) * 2], di = p->strain[((size_t)det * nf + kk) * 2 + 1];
+        const double S = p->psd[(size_t)det * nf + kk];
+        const double hr = hk[2 * det], hi = hk[2 * det + 1];
+        // d conj(h0) / S
+        const double zr = (dr * hr + di * hi) / S, zi = (di * hr - dr * hi) / S;
+        const double h2 = (hr * hr + hi * hi) / S;
+        a0r[det] += zr; a0i[det] += zi; a1r[det] += zr * (f - fm); a1i[det] += zi * (f - fm);
+        b0[det] += h2; b1[det] += h2 * (f - fm);
+      }
+    }
+    for (int det = 0; det < nd; ++det) {
+      const size_t ib = (size_t)det * nb + b;
+      rb->A0[2 * ib] = (double)(4.0L * p->df * a0r[det]); rb->A0[2 * ib + 1] = (double)(4.0L * p->df * a0i[det]);
+      rb->A1[2 * ib] = (double)(4.0L * p->df * a1r[det]); rb->A1[2 * ib + 1] = (double)(4.0L * p->df * a1i[det]);
+      rb->B0[ib] = (double)(4.0L * p->df * b0[det]); rb->B1[ib] = (double)(4.0L * p->df * b1[det]);
+    }
+  }
+  return rb;
+}
+
+void orc_relbin_free(void* h) { delete static_cast<RelBin*>(h); }
+int32_t orc_relbin_nbins(const void* h) { return static_cast<const RelBin*>(h)->n_bins; }
+void orc_relbin_edges(const void* h, int32_t* out) {
+  const RelBin* rb = static_cast<const RelBin*>(h);
+  for (int i = 0; i <= rb->n_bins; ++i) out[i] = rb->edge[i];
+}
+// summary data: A0, A1 [n_det][n_bins][2]; B0, B1 [n_det][n_bins]
+void orc_relbin_summary(const void* h, double* A0, double* A1, double* B0, double* B1) {
+  const RelBin* rb = static_cast<const RelBin*>(h);
+  std::copy(rb->A0.begin(), rb->A0.end(), A0); std::copy(rb->A1.begin(), rb->A1.end(), A1);
+  std::copy(rb->B0.begin(), rb->B0.end(), B0); std::copy(rb->B1.begin(), rb->B1.end(), B1);
+}
+
+static double relbin_loglike_one(const orc_problem* p, const RelBin* rb, const double* th, double* parts) {
+  const int nd = p->n_det, nb = rb->n_bins;
+  if (!theta_physical(th)) {
+    if (parts) for (int i = 0; i < 2 * nd; ++i) parts[i] = std::numeric_limits<double>::quiet_NaN();
+    return NEG_INF;
+  }
+  Waveform w = make_waveform(p, th);
+  std::vector<double> fp(nd), fx(nd), dt(nd);
+  for (int det = 0; det < nd; ++det) detector_response(p, det, th[9], th[10], th[6], &fp[det], &fx[det], &dt[det]);
+  // step 4: ratios at the edges
+  std::vector<double> r((size_t)nd * (nb + 1) * 2), hk(2 * nd);
+  for (int i = 0; i <= nb; ++i) {
+    waveform_at(p, w, th, fp.data(), fx.data(), dt.data(), rb->fe[i], hk.data());
+    for (int det = 0; det < nd; ++det) {
+      const double ar = hk[2 * det], ai = hk[2 * det + 1];
+      const double br = rb->h0[((size_t)det * (nb + 1) + i) * 2], bi = rb->h0[((size_t)det * (nb + 1) + i) * 2 + 1];
+      const double den = br * br + bi * bi;
+      r[((size_t)det * (nb + 1) + i) * 2] = (ar * br + ai * bi) / den;
+      r[((size_t)det * (nb + 1) + i) * 2 + 1] = (ai * br - ar * bi) / den;
+    }
+  }
+  double logl = 0.0;
+  for (int det = 0; det < nd; ++det) {
+    long double dh = 0.0L, hh = 0.0L;
+    for (int b = 0; b < nb; ++b) {
+      const double* rl = &r[((size_t)det * (nb + 1) + b) * 2];
+      const double* rh = rl + 2;
+      const double w_ = rb->fe[b + 1] - rb->fe[b];
+      const double r0r = 0.5 * (rl[0] + rh[0]), r0i = 0.5 * (rl[1] + rh[1]);
+      const double r1r = (rh[0] - rl[0]) / w_, r1i = (rh[1] - rl[1]) / w_;
+      const size_t ib = (size_t)det * nb + b;
+      // Re(A conj(r)) = Ar rr + Ai ri
+      dh += (long double)(rb->A0[2 * ib] * r0r + rb->A0[2 * ib + 1] * r0i + rb->A1[2 * ib] * r1r + rb->A1[2 * ib + 1] * r1i);
+      hh += (long double)(rb->B0[ib] * (r0r * r0r + r0i * r0i) + 2.0 * rb->B1[ib] * (r0r * r1r + r0i * r1i));
+    }
+    if (parts) { parts[2 * det] = (double)dh; parts[2 * det + 1] = (double)hh; }
+    logl += (double)dh - 0.5 * (double)hh;
+  }
+  return logl;
+}
+
+void orc_relbin_loglike(const orc_problem* p, const void* h, const double* theta, int64_t B, double* logl, double* parts, int threads) {
+  const RelBin* rb = static_cast<const RelBin*>(h);
+#pragma omp parallel for schedule(dynamic, 4) num_threads(threads > 0 ? threads : omp_get_max_threads_safe())
+  for (int64_t i = 0; i < B; ++i) logl[i] = relbin_loglike_one(p, rb, theta + i * 11, parts ? parts + i * 2 * p->n_det : nullptr);
+}
+
+}  // extern "C"

@@ -144,6 +144,10 @@ class OracleProblem:
         _lib.orc_gw_loglike(C.byref(self.p), _dp(theta), C.c_int64(B), _dp(logl), _dp(pr), C.c_int(threads))
         return (logl, pr) if parts else logl
 
+    # ---- relative binning (DESIGN.md R:L24) ----------------------------------------------------------
+    def relbin(self, theta0, chi=1.0, eps=0.5):
+        return OracleRelBin(self, theta0, chi, eps)
+
     def loglike_u(self, u, threads=0):
         u = _f64(u).reshape(-1, self.ndim)
         logl = np.empty(u.shape[0])
@@ -212,6 +216,44 @@ class OracleSampler:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         _lib.orc_finalize(self.h, C.byref(a), C.byref(b), C.byref(c))
         return a.value, b.value, c.value  # logZ, err, H
+
+
+class OracleRelBin:
+    """Relative-binning summary data about a fiducial theta0 and the approximate likelihood built on them."""
+
+    def __init__(self, problem, theta0, chi, eps):
+        self.P = problem
+        _lib.orc_relbin_create.restype = C.c_void_p
+        self.h = C.c_void_p(_lib.orc_relbin_create(C.byref(problem.p), _dp(_f64(theta0)), C.c_double(chi), C.c_double(eps)))
+        if not self.h.value:
+            raise ValueError("orc_relbin_create failed (unphysical theta0 or bad chi/eps)")
+        _lib.orc_relbin_nbins.restype = C.c_int32
+        self.n_bins = int(_lib.orc_relbin_nbins(self.h))
+
+    def __del__(self):
+        if getattr(self, "h", None) and self.h.value:
+            _lib.orc_relbin_free(self.h)
+            self.h = C.c_void_p(0)
+
+    def edges(self):
+        e = np.empty(self.n_bins + 1, dtype=np.int32)
+        _lib.orc_relbin_edges(self.h, e.ctypes.data_as(C.POINTER(C.c_int32)))
+        return e
+
+    def summary(self):
+        nd, nb = self.P.n_det, self.n_bins
+        A0, A1 = np.empty((nd, nb, 2)), np.empty((nd, nb, 2))
+        B0, B1 = np.empty((nd, nb)), np.empty((nd, nb))
+        _lib.orc_relbin_summary(self.h, _dp(A0), _dp(A1), _dp(B0), _dp(B1))
+        return A0, A1, B0, B1
+
+    def loglike(self, theta, parts=False, threads=0):
+        theta = _f64(theta).reshape(-1, 11)
+        B = theta.shape[0]
+        logl = np.empty(B)
+        pr = np.empty((B, 2 * self.P.n_det)) if parts else None
+        _lib.orc_relbin_loglike(C.byref(self.P.p), self.h, _dp(theta), C.c_int64(B), _dp(logl), _dp(pr), C.c_int(threads))
+        return (logl, pr) if parts else logl
 
 
 # ---- free functions ---------------------------------------------------------------------------
