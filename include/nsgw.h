@@ -136,6 +136,24 @@ int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_ite
 int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host,
                     int64_t* iters_host, double** dead_dev);
 
+/* ---- Relative binning ("heterodyned likelihood"; the paper names it as the remedy for the bins x samples cost,
+ * P:172, and gives no formula: DESIGN.md reading R:L24 restates the published scheme). ----
+ * ns_relbin_setup builds, on the device, the summary data about the fiducial parameters theta0_host[11] (physical, Table-1 order):
+ * bin edges equally spaced in Delta(f) = 2 pi chi sum_gamma sgn(gamma) (f/f*_gamma)^gamma with floor(Delta_tot/eps) bins (or the
+ * caller's edges_host[n_edges]: strictly increasing grid indices from 0 to n_freq-1; pass NULL, 0 for the default), and per
+ * detector and bin A0, A1 (complex), B0, B1.  Replaces any earlier set-up of the handle.  Synchronises.  *n_bins_host (may be
+ * NULL) receives the number of bins.  Errors: -1 bad chi/eps/edges or unphysical theta0, -3 no GW likelihood.
+ * ns_relbin_get copies out the edges [n_bins+1] and/or the summary data laid out A0[n_det][n_bins][2], A1[n_det][n_bins][2],
+ * B0[n_det][n_bins], B1[n_det][n_bins] (host pointers, either may be NULL).  Synchronises.
+ * gw_loglike_relbin_batch: as gw_loglike_batch, with <d,h> ~ Re sum_b [A0 conj(r0) + A1 conj(r1)] and
+ * <h,h> ~ sum_b [B0 |r0|^2 + 2 B1 Re(r0 conj(r1))], r = h(theta)/h(theta0) at the bin edges: the waveform is evaluated at
+ * n_bins+1 frequencies per row instead of n_freq.  An approximation of gw_loglike_batch: exact when r is constant (distance,
+ * phase), second order in the bin width otherwise.  parts_dev as in gw_loglike_batch. */
+int ns_relbin_setup(ns_handle* h, const double* theta0_host, double chi, double eps, const int32_t* edges_host, int32_t n_edges,
+                    int32_t* n_bins_host, void* stream);
+int ns_relbin_get(ns_handle* h, int32_t* edges_host, double* summary_host, void* stream);
+int gw_loglike_relbin_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream);
+
 /* Copies the live set out: u_dev [n_live, ndim], logl_dev [n_live] (either may be NULL). */
 int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream);
 

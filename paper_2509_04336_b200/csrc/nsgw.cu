@@ -541,6 +541,200 @@ __global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const dou
 }
 
 // ======================================================================================================
+// Relative binning (heterodyned likelihood; DESIGN.md R:L24): summary data about a fiducial theta0 on N_b
+// coarse bins, then per evaluation the waveform at the N_b + 1 bin edges only.
+// ======================================================================================================
+struct RbDev {
+  const int* edge;        // [nb + 1] grid indices of the bin edges
+  const double2* A0;      // [n_det][nb]  sum wd conj(g0)              (g = h f^{7/6}: the f^{-7/6} of the amplitude lives in wd, ws)
+  const double2* A1;      // [n_det][nb]  sum wd conj(g0) (f - f_m)
+  const double* B0;       // [n_det][nb]  sum ws |g0|^2
+  const double* B1;       // [n_det][nb]  sum ws |g0|^2 (f - f_m)
+  const double2* ig0;     // [n_det][nb + 1]  1 / g0 at the edges
+  const double* inv_w;    // [nb]  1 / (f_hi - f_lo)
+  int nb;
+};
+
+// g_d(f_k) = amp C_d exp(-i Phi_d) for every detector at grid bin k (Phi_d = common phase - relative delay; the same pieces as
+// the bin loops, with a direct sincos per detector because the edges are not equally spaced).
+template <int MODEL, int NDET, class CB>
+__device__ __forceinline__ void gw_g_at(const CB& cb, const Tables& tb, int k, const MathTables* mt, double2 (&g)[NDET]) {
+  const BinBasis b = make_basis(tb, k, MODEL == 2);
+  double q, amp = 1.0;
+  if (MODEL == 1) {
+    q = fma(cb(CB_PH + 0), b.y5, cb(CB_PH + 4));
+    q = fma(cb(CB_PH + 1), b.y3, q);
+    q = fma(cb(CB_PH + 2), b.y2, q);
+    q = fma(cb(CB_PH + 3), b.y, q);
+    q = fma(cb(CB_PH + 5), b.L, q);
+    q = fma(cb(CB_PH + 6), b.x, q);
+    q = fma(cb(CB_PH + 7), b.xL, q);
+    q = fma(cb(CB_PH + 8), b.x2, q);
+    q = fma(cb(CB_PH + 9), b.f, q);
+  } else {
+    phenom_bin_t(cb, b, mt, exp_tab(cb(CB_AM + 3) * (b.f - cb(CB_AM + 0)), mt), q, amp);
+  }
+#pragma unroll
+  for (int d = 0; d < NDET; ++d) {
+    double sn, cs;
+    sincos_lut(64.0 * fma(-cb(CB_DET + 4 * d + 2), b.f, q), mt, sn, cs);
+    const double cr = cb(CB_DET + 4 * d), ci = cb(CB_DET + 4 * d + 1);
+    g[d] = make_double2(amp * fma(cr, cs, ci * sn), amp * fma(ci, cs, -(cr * sn)));
+  }
+}
+
+// Delta(f_k) of reading L24, one thread per grid bin.
+__global__ void k_rb_delta(const DevCfg* __restrict__ cfg, double chi, double* delta) {
+  const int nf = cfg->n_freq;
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= nf) return;
+  const double f = cfg->f_min + k * cfg->df, f_lo = cfg->f_min, f_hi = cfg->f_min + (nf - 1) * cfg->df;
+  const double g[5] = {-5.0 / 3.0, -2.0 / 3.0, 1.0, 5.0 / 3.0, 7.0 / 3.0};
+  double s = 0.0;
+  for (int i = 0; i < 5; ++i) s += (g[i] < 0.0) ? -pow(f / f_lo, g[i]) : pow(f / f_hi, g[i]);
+  delta[k] = 2.0 * kPi * chi * s;
+}
+
+// Bin edges equally spaced in Delta (sequential, as the reading states it; N_f steps in total).  out[0] = number of bins.
+__global__ void k_rb_select(const DevCfg* __restrict__ cfg, const double* __restrict__ delta, double eps, int cap, int* nb_out, int* edge) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  const int nf = cfg->n_freq;
+  const double d0 = delta[0], dtot = delta[nf - 1] - d0;
+  const double want = floor(dtot / eps);
+  if (!(want <= 4.0 * nf)) { *nb_out = -1; return; }     // eps far below what the grid resolves
+  const int nb_req = max(1, (int)want);
+  int n = 0, k = 0;
+  edge[n++] = 0;
+  for (int i = 1; i < nb_req && n < cap - 1; ++i) {
+    const double target = i * (dtot / nb_req);
+    while (k < nf - 1 && delta[k] - d0 < target) ++k;
+    if (k > edge[n - 1] && k < nf - 1) edge[n++] = k;
+  }
+  edge[n++] = nf - 1;
+  *nb_out = n - 1;
+}
+
+// Summary data: CTA b sums grid bins [e_b, e_b+1) (the last one up to and including e_nb) for every detector; fixed-order
+// reduction.  Also 1/g0 at the edges and 1/(bin width).
+template <int MODEL, int NDET>
+__global__ void __launch_bounds__(128) k_rb_summary(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cb0_g,
+                                                    const int* __restrict__ edge, int nb, double2* A0, double2* A1, double* B0, double* B1,
+                                                    double2* ig0, double* inv_w) {
+  constexpr int NT = 128, NW = NT / 32, NV = 6 * NDET;
+  __shared__ MathTables mtab;
+  __shared__ double cb0[CB_SIZE];
+  __shared__ double red[NW * NV], out[NV];
+  const int tid = threadIdx.x, b = blockIdx.x;
+  load_math_tables(&mtab, tb.mt, tid, NT);
+  for (int i = tid; i < CB_SIZE; i += NT) cb0[i] = cb0_g[i];
+  __syncthreads();
+  const CbPtr cb{cb0};
+  const int k_lo = edge[b], k_hi = (b == nb - 1) ? edge[b + 1] + 1 : edge[b + 1];
+  const double f_lo = __ldg(tb.f + edge[b]), f_hi = __ldg(tb.f + edge[b + 1]);
+  const double fm = 0.5 * (f_lo + f_hi);
+  double v[NV];
+#pragma unroll
+  for (int i = 0; i < NV; ++i) v[i] = 0.0;
+  for (int k = k_lo + tid; k < k_hi; k += NT) {
+    double2 g[NDET];
+    gw_g_at<MODEL, NDET>(cb, tb, k, &mtab, g);
+    const double df_ = __ldg(tb.f + k) - fm;
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      const double2 w = __ldg(tb.wd[d] + k);
+      // wd conj(g0)
+      const double zr = fma(w.x, g[d].x, w.y * g[d].y), zi = fma(w.y, g[d].x, -(w.x * g[d].y));
+      const double h2 = __ldg(tb.ws[d] + k) * fma(g[d].x, g[d].x, g[d].y * g[d].y);
+      v[6 * d + 0] += zr; v[6 * d + 1] += zi;
+      v[6 * d + 2] = fma(zr, df_, v[6 * d + 2]); v[6 * d + 3] = fma(zi, df_, v[6 * d + 3]);
+      v[6 * d + 4] += h2; v[6 * d + 5] = fma(h2, df_, v[6 * d + 5]);
+    }
+  }
+  block_reduce<NV, NT>(v, red, out);
+  if (tid < NDET) {
+    const int d = tid;
+    A0[(size_t)d * nb + b] = make_double2(out[6 * d + 0], out[6 * d + 1]);
+    A1[(size_t)d * nb + b] = make_double2(out[6 * d + 2], out[6 * d + 3]);
+    B0[(size_t)d * nb + b] = out[6 * d + 4];
+    B1[(size_t)d * nb + b] = out[6 * d + 5];
+  }
+  if (tid == 32) inv_w[b] = 1.0 / (f_hi - f_lo);
+  if (tid == 64 || (tid == 96 && b == nb - 1)) {
+    const int i = (tid == 64) ? b : nb;
+    double2 g[NDET];
+    gw_g_at<MODEL, NDET>(cb, tb, edge[i], &mtab, g);
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      const double den = 1.0 / fma(g[d].x, g[d].x, g[d].y * g[d].y);
+      ig0[(size_t)d * (nb + 1) + i] = make_double2(g[d].x * den, -g[d].y * den);
+    }
+  }
+}
+
+// Evaluation: one thread per particle, loop over the N_b + 1 edges (all lanes at the same edge: table and summary loads are
+// warp-uniform), ratio r = g/g0 at the edge, then the bin between the previous edge and this one.
+constexpr int kRbThreads = 128;
+
+template <int MODEL, int NDET>
+__global__ void __launch_bounds__(kRbThreads) k_relbin(const DevCfg* __restrict__ cfgp, Tables tb, RbDev rb, const double* __restrict__ cbs_g,
+                                                        long long B, double* logl, double* parts) {
+  constexpr int NT = kRbThreads;
+  __shared__ MathTables mtab;
+  extern __shared__ __align__(16) double rb_cbT[];   // PhenomD-form: [CB_SIZE][NT] coefficient blocks, transposed
+  const int tid = threadIdx.x;
+  const long long p0 = (long long)blockIdx.x * NT, p = p0 + tid;
+  const bool have = p < B;
+  load_math_tables(&mtab, tb.mt, tid, NT);
+  // coefficient block of this thread's particle: TaylorF2 -> registers through a 16-entry local copy; PhenomD-form -> shared
+  double cbl[MODEL == 1 ? 30 : 1];
+  if (MODEL == 1) {
+#pragma unroll
+    for (int i = 0; i < 30; ++i) cbl[i] = have ? __ldg(cbs_g + p * CB_SIZE + i) : 0.0;
+  } else {
+    for (int e = tid; e < NT * CB_SIZE; e += NT) {
+      const int part = e % NT, i = e / NT;
+      rb_cbT[i * NT + part] = (p0 + part < B) ? __ldg(cbs_g + (p0 + part) * CB_SIZE + i) : 0.0;
+    }
+  }
+  __syncthreads();
+  double2 prev[NDET];
+  double dh[NDET], hh[NDET];
+#pragma unroll
+  for (int d = 0; d < NDET; ++d) { dh[d] = 0.0; hh[d] = 0.0; prev[d] = make_double2(0.0, 0.0); }
+  const int nb = rb.nb;
+  for (int i = 0; i <= nb; ++i) {
+    const int k = __ldg(rb.edge + i);
+    double2 g[NDET];
+    if (MODEL == 1) gw_g_at<MODEL, NDET>(CbPtr{cbl}, tb, k, &mtab, g);
+    else gw_g_at<MODEL, NDET>(CbStrided{rb_cbT + tid, NT}, tb, k, &mtab, g);
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      const double2 ig = __ldg(rb.ig0 + (size_t)d * (nb + 1) + i);
+      const double2 r = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
+      if (i > 0) {
+        const size_t ib = (size_t)d * nb + (i - 1);
+        const double iw = __ldg(rb.inv_w + (i - 1));
+        const double r0r = 0.5 * (prev[d].x + r.x), r0i = 0.5 * (prev[d].y + r.y);
+        const double r1r = (r.x - prev[d].x) * iw, r1i = (r.y - prev[d].y) * iw;
+        const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
+        dh[d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
+        hh[d] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
+      }
+      prev[d] = r;
+    }
+  }
+  if (!have) return;
+  const bool valid = ((MODEL == 1) ? cbl[CB_VALID] : rb_cbT[CB_VALID * NT + tid]) != 0.0;
+  double l = 0.0;
+#pragma unroll
+  for (int d = 0; d < NDET; ++d) {
+    if (parts) { parts[p * 2 * NDET + 2 * d] = valid ? dh[d] : nan(""); parts[p * 2 * NDET + 2 * d + 1] = valid ? hh[d] : nan(""); }
+    l += dh[d] - 0.5 * hh[d];
+  }
+  logl[p] = valid ? l : -INFINITY;
+}
+
+// ======================================================================================================
 // K2: acceptance walk
 // ======================================================================================================
 struct WalkArgs {
@@ -1022,6 +1216,11 @@ struct ns_handle {
   Tables tb{};
   double* d_tab = nullptr;      // four double2 pair tables, f, f34 (10 * nf doubles)
   cudaStream_t s_own = nullptr; // ns_run_many: this run's stream
+  // relative binning (ns_relbin_setup)
+  int rb_nb = 0;
+  int* d_rb_edge = nullptr;      // [rb_nb + 1]
+  double* d_rb_buf = nullptr;    // A0, A1 (complex), B0, B1, ig0 (complex), inv_w, cb0, theta0
+  RbDev rb{};
   MathTables* d_mtab = nullptr; // sin/cos, exp2, atan tables
   double2* d_wd = nullptr;      // [n_det][nf]
   double* d_ws = nullptr;       // [n_det][nf]
@@ -1287,6 +1486,7 @@ void ns_free(ns_handle* h) {
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
   cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
   if (h->s_own) cudaStreamDestroy(h->s_own);
+  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -1613,6 +1813,128 @@ int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double te
     if (iters_host) iters_host[r] = it[r];
   }
   return total;
+}
+
+int ns_relbin_setup(ns_handle* h, const double* theta0_host, double chi, double eps, const int32_t* edges_host, int32_t n_edges,
+                    int32_t* n_bins_host, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (!theta0_host || !(chi > 0.0) || !(eps > 0.0) || h->cfg.n_freq < 2) return fail(h, -1, "bad arguments");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int nf = h->cfg.n_freq, nd = h->cfg.n_det;
+  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
+  h->d_rb_edge = nullptr; h->d_rb_buf = nullptr; h->rb_nb = 0;
+  // ---- bin edges: given, or equally spaced in Delta(f) (reading L24)
+  std::vector<int> edge;
+  if (edges_host) {
+    if (n_edges < 2 || edges_host[0] != 0 || edges_host[n_edges - 1] != nf - 1) return fail(h, -1, "edges must run from 0 to n_freq - 1");
+    for (int i = 1; i < n_edges; ++i)
+      if (edges_host[i] <= edges_host[i - 1]) return fail(h, -1, "edges must increase strictly");
+    edge.assign(edges_host, edges_host + n_edges);
+  } else {
+    double* d_delta = nullptr;
+    int* d_sel = nullptr;
+    CU_CHECK(h, cudaMalloc(&d_delta, sizeof(double) * nf));
+    if (cudaMalloc(&d_sel, sizeof(int) * ((size_t)nf + 2)) != cudaSuccess) { cudaFree(d_delta); return fail(h, -4, "cudaMalloc"); }
+    k_rb_delta<<<(nf + 127) / 128, 128, 0, s>>>(h->d_cfg, chi, d_delta);
+    k_rb_select<<<1, 1, 0, s>>>(h->d_cfg, d_delta, eps, nf + 1, d_sel, d_sel + 1);
+    g_launches.fetch_add(2);
+    std::vector<int> sel((size_t)nf + 2);
+    cudaError_t e_ = cudaMemcpyAsync(sel.data(), d_sel, sizeof(int) * ((size_t)nf + 2), cudaMemcpyDeviceToHost, s);
+    if (e_ == cudaSuccess) e_ = cudaStreamSynchronize(s);
+    cudaFree(d_delta); cudaFree(d_sel);
+    if (e_ != cudaSuccess) return fail(h, -2, std::string("relbin edges: ") + cudaGetErrorString(e_));
+    if (sel[0] < 1) return fail(h, -1, "eps too small for this grid (more than 4 n_freq bins requested)");
+    edge.assign(sel.begin() + 1, sel.begin() + 2 + sel[0]);
+  }
+  const int nb = (int)edge.size() - 1;
+  // ---- device buffers: A0, A1 [nd][nb] complex, B0, B1 [nd][nb], ig0 [nd][nb+1] complex, inv_w [nb], cb0 [CB_SIZE], theta0 [16]
+  const size_t n_buf = (size_t)nd * nb * 6 + (size_t)nd * (nb + 1) * 2 + nb + CB_SIZE + 16;
+  CU_CHECK(h, cudaMalloc(&h->d_rb_edge, sizeof(int) * (nb + 1)));
+  CU_CHECK(h, cudaMalloc(&h->d_rb_buf, sizeof(double) * n_buf));
+  double* b = h->d_rb_buf;
+  double2* A0 = reinterpret_cast<double2*>(b); b += (size_t)nd * nb * 2;
+  double2* A1 = reinterpret_cast<double2*>(b); b += (size_t)nd * nb * 2;
+  double2* ig0 = reinterpret_cast<double2*>(b); b += (size_t)nd * (nb + 1) * 2;
+  double* B0 = b; b += (size_t)nd * nb;
+  double* B1 = b; b += (size_t)nd * nb;
+  double* inv_w = b; b += nb;
+  double* cb0 = b; b += CB_SIZE;
+  double* th0 = b;
+  CU_CHECK(h, cudaMemcpyAsync(h->d_rb_edge, edge.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, s));
+  CU_CHECK(h, cudaMemcpyAsync(th0, theta0_host, sizeof(double) * 11, cudaMemcpyHostToDevice, s));
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  if (tf2) k_setup<1><<<1, 32, 0, s>>>(h->d_cfg, th0, 1, cb0);
+  else k_setup<2><<<1, 32, 0, s>>>(h->d_cfg, th0, 1, cb0);
+  LAUNCH_CHECK(h);
+#define RB_SUMMARY(M, N) k_rb_summary<M, N><<<nb, 128, 0, s>>>(h->d_cfg, h->tb, cb0, h->d_rb_edge, nb, A0, A1, B0, B1, ig0, inv_w)
+  if (tf2) { if (nd == 1) RB_SUMMARY(1, 1); else if (nd == 2) RB_SUMMARY(1, 2); else RB_SUMMARY(1, 3); }
+  else { if (nd == 1) RB_SUMMARY(2, 1); else if (nd == 2) RB_SUMMARY(2, 2); else RB_SUMMARY(2, 3); }
+#undef RB_SUMMARY
+  LAUNCH_CHECK(h);
+  double valid = 0.0;
+  CU_CHECK(h, cudaMemcpyAsync(&valid, cb0 + CB_VALID, sizeof(double), cudaMemcpyDeviceToHost, s));
+  CU_CHECK(h, cudaStreamSynchronize(s));
+  if (valid == 0.0) {
+    cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
+    h->d_rb_edge = nullptr; h->d_rb_buf = nullptr;
+    return fail(h, -1, "fiducial theta0 is unphysical");
+  }
+  h->rb_nb = nb;
+  h->rb.edge = h->d_rb_edge; h->rb.A0 = A0; h->rb.A1 = A1; h->rb.B0 = B0; h->rb.B1 = B1; h->rb.ig0 = ig0; h->rb.inv_w = inv_w; h->rb.nb = nb;
+  if (n_bins_host) *n_bins_host = nb;
+  return 0;
+}
+
+int ns_relbin_get(ns_handle* h, int32_t* edges_host, double* summary_host, void* stream) {
+  if (!h) return -3;
+  if (h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int nb = h->rb_nb, nd = h->cfg.n_det;
+  if (edges_host) CU_CHECK(h, cudaMemcpyAsync(edges_host, h->d_rb_edge, sizeof(int) * (nb + 1), cudaMemcpyDeviceToHost, s));
+  if (summary_host) {   // A0 [nd][nb][2], A1 [nd][nb][2], B0 [nd][nb], B1 [nd][nb]
+    CU_CHECK(h, cudaMemcpyAsync(summary_host, h->rb.A0, sizeof(double) * (size_t)nd * nb * 4, cudaMemcpyDeviceToHost, s));
+    CU_CHECK(h, cudaMemcpyAsync(summary_host + (size_t)nd * nb * 4, h->rb.B0, sizeof(double) * (size_t)nd * nb * 2, cudaMemcpyDeviceToHost, s));
+  }
+  CU_CHECK(h, cudaStreamSynchronize(s));
+  return 0;
+}
+
+int gw_loglike_relbin_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");
+  if (B < 0 || (B > 0 && (!theta_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  if (B == 0) return 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  int rc = ensure_cb(h, B);
+  if (rc) return rc;
+  const unsigned gs = (unsigned)((B + 127) / 128), gr = (unsigned)((B + kRbThreads - 1) / kRbThreads);
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  const int nd = h->cfg.n_det;
+  if (tf2) k_setup<1><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+  else k_setup<2><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+  LAUNCH_CHECK(h);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof && h->prof_ev.size() < 4096) {
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, s);
+  }
+  constexpr size_t kSm2 = sizeof(double) * CB_SIZE * kRbThreads;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    attr_set = true;
+  }
+#define RB_EVAL(M, N, SM) k_relbin<M, N><<<gr, kRbThreads, SM, s>>>(h->d_cfg, h->tb, h->rb, h->d_cb, B, logl_dev, parts_dev)
+  if (tf2) { if (nd == 1) RB_EVAL(1, 1, 0); else if (nd == 2) RB_EVAL(1, 2, 0); else RB_EVAL(1, 3, 0); }
+  else { if (nd == 1) RB_EVAL(2, 1, kSm2); else if (nd == 2) RB_EVAL(2, 2, kSm2); else RB_EVAL(2, 3, kSm2); }
+#undef RB_EVAL
+  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
+  LAUNCH_CHECK(h);
+  return 0;
 }
 
 int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream) {

@@ -567,51 +567,70 @@ __device__ __forceinline__ double phase_pn_qt(const double* a, const BinBasis& b
   return q;
 }
 
+// Accessors of a coefficient block: contiguous (shared or global memory, one particle) or strided (block transposed in shared
+// memory so that each lane of a warp reads its own particle without bank conflicts).
+struct CbPtr {
+  const double* p;
+  __device__ __forceinline__ double operator()(int i) const { return p[i]; }
+};
+struct CbStrided {
+  const double* p;
+  int stride;
+  __device__ __forceinline__ double operator()(int i) const { return p[i * stride]; }
+};
+
 // PhenomD-form: phase [quarter turns] and amplitude factor for one bin.
 // `ex` = exp(-gamma2 (f - f_RD)/w) of this bin, supplied by the caller (the bin loops carry it as a geometric sequence along a
-// thread's bins; k_waveform evaluates it directly).
-__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, const MathTables* mt, double ex, double& q, double& amp) {
+// thread's bins; k_waveform and the relative-binning kernels evaluate it directly).
+template <class CB>
+__device__ __forceinline__ void phenom_bin_t(const CB& cb, const BinBasis& b, const MathTables* mt, double ex, double& q, double& amp) {
   const double f = b.f;
-  if (f < cb[CB_FP1]) {
-    const double* a = cb + CB_PH;
-    q = phase_pn_qt(a, b);
+  if (f < cb(CB_FP1)) {
+    q = fma(cb(CB_PH + 0), b.y5, cb(CB_PH + 4));
+    q = fma(cb(CB_PH + 1), b.y3, q);
+    q = fma(cb(CB_PH + 2), b.y2, q);
+    q = fma(cb(CB_PH + 3), b.y, q);
+    q = fma(cb(CB_PH + 5), b.L, q);
+    q = fma(cb(CB_PH + 6), b.x, q);
+    q = fma(cb(CB_PH + 7), b.xL, q);
+    q = fma(cb(CB_PH + 8), b.x2, q);
+    q = fma(cb(CB_PH + 9), b.f, q);
     double fx = f * b.x;
-    q = fma(a[10], fx, q);
-    q = fma(a[11], fx * b.x, q);
-    q = fma(a[12], f * f, q);
-  } else if (f < cb[CB_FP2]) {
-    const double* p = cb + CB_PB;
+    q = fma(cb(CB_PH + 10), fx, q);
+    q = fma(cb(CB_PH + 11), fx * b.x, q);
+    q = fma(cb(CB_PH + 12), f * f, q);
+  } else if (f < cb(CB_FP2)) {
     double if3 = b.y3 * b.y3 * b.y3;
-    q = fma(p[1], b.L, p[0]);
-    q = fma(p[2], f, q);
-    q = fma(p[3], if3, q);
+    q = fma(cb(CB_PB + 1), b.L, cb(CB_PB + 0));
+    q = fma(cb(CB_PB + 2), f, q);
+    q = fma(cb(CB_PB + 3), if3, q);
   } else {
-    const double* p = cb + CB_PM;
-    q = fma(p[1], f, p[0]);
-    q = fma(p[2], b.y3, q);
-    q = fma(p[3], b.f34, q);
-    q = fma(p[4], atan_tab((f - p[5]) * p[6], mt), q);
+    q = fma(cb(CB_PM + 1), f, cb(CB_PM + 0));
+    q = fma(cb(CB_PM + 2), b.y3, q);
+    q = fma(cb(CB_PM + 3), b.f34, q);
+    q = fma(cb(CB_PM + 4), atan_tab((f - cb(CB_PM + 5)) * cb(CB_PM + 6), mt), q);
   }
-  if (f < cb[CB_FA1]) {
-    const double* c = cb + CB_AI;
-    double p = c[9];
+  if (f < cb(CB_FA1)) {
+    double p = cb(CB_AI + 9);
 #pragma unroll
-    for (int i = 8; i >= 0; --i) p = fma(p, b.x, c[i]);
+    for (int i = 8; i >= 0; --i) p = fma(p, b.x, cb(CB_AI + i));
     amp = p;
-  } else if (f < cb[CB_FA2]) {
-    const double* c = cb + CB_AH;
-    double xh = (f - c[0]) * c[1];
-    double p = c[6];
-    p = fma(p, xh, c[5]);
-    p = fma(p, xh, c[4]);
-    p = fma(p, xh, c[3]);
-    p = fma(p, xh, c[2]);
+  } else if (f < cb(CB_FA2)) {
+    double xh = (f - cb(CB_AH + 0)) * cb(CB_AH + 1);
+    double p = cb(CB_AH + 6);
+    p = fma(p, xh, cb(CB_AH + 5));
+    p = fma(p, xh, cb(CB_AH + 4));
+    p = fma(p, xh, cb(CB_AH + 3));
+    p = fma(p, xh, cb(CB_AH + 2));
     amp = p;
   } else {
-    const double* c = cb + CB_AM;
-    double fx = f - c[0];
-    amp = c[1] * rcp_nr(fma(fx, fx, c[2])) * ex;
+    double fx = f - cb(CB_AM + 0);
+    amp = cb(CB_AM + 1) * rcp_nr(fma(fx, fx, cb(CB_AM + 2))) * ex;
   }
+}
+
+__device__ __forceinline__ void phenom_bin(const double* cb, const BinBasis& b, const MathTables* mt, double ex, double& q, double& amp) {
+  phenom_bin_t(CbPtr{cb}, b, mt, ex, q, amp);
 }
 
 }  // namespace nsgw

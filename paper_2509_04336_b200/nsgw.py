@@ -43,7 +43,7 @@ class NsStats(C.Structure):
 
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
-           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_get_live", "ns_finalize_evidence",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 _lib = None
@@ -232,6 +232,40 @@ class Handle:
 
     def profile_enable(self, on=True):
         self._check(lib().nsgw_profile_enable(self._h, C.c_int32(1 if on else 0)), "nsgw_profile_enable")
+
+    # ---- relative binning ---------------------------------------------------------------------------
+    def relbin_setup(self, theta0, chi=1.0, eps=0.5, edges=None):
+        th = (C.c_double * 11)(*[float(x) for x in theta0])
+        nb = C.c_int32()
+        if edges is not None:
+            ed = (C.c_int32 * len(edges))(*[int(x) for x in edges])
+            rc = lib().ns_relbin_setup(self._h, th, C.c_double(chi), C.c_double(eps), ed, C.c_int32(len(edges)), C.byref(nb), _stream())
+        else:
+            rc = lib().ns_relbin_setup(self._h, th, C.c_double(chi), C.c_double(eps), None, C.c_int32(0), C.byref(nb), _stream())
+        self._check(rc, "ns_relbin_setup")
+        self.rb_n_bins = nb.value
+        return nb.value
+
+    def relbin_get(self):
+        import numpy as np
+        nb, nd = self.rb_n_bins, self.n_det
+        ed = (C.c_int32 * (nb + 1))()
+        sm = (C.c_double * (nd * nb * 6))()
+        self._check(lib().ns_relbin_get(self._h, ed, sm, _stream()), "ns_relbin_get")
+        a = np.array(sm)
+        A0 = a[: nd * nb * 2].reshape(nd, nb, 2)
+        A1 = a[nd * nb * 2: nd * nb * 4].reshape(nd, nb, 2)
+        B0 = a[nd * nb * 4: nd * nb * 5].reshape(nd, nb)
+        B1 = a[nd * nb * 5:].reshape(nd, nb)
+        return np.array(ed), A0, A1, B0, B1
+
+    def gw_loglike_relbin_batch(self, theta, parts=False, out=None):
+        B = theta.shape[0]
+        logl = out if out is not None else torch.empty(B, dtype=torch.float64, device="cuda")
+        pr = torch.empty(B, 2 * self.n_det, dtype=torch.float64, device="cuda") if parts else None
+        self._check(lib().gw_loglike_relbin_batch(self._h, _ptr(theta), C.c_int64(B), _ptr(logl), _ptr(pr), _stream()),
+                    "gw_loglike_relbin_batch")
+        return (logl, pr) if parts else logl
 
     def set_option(self, key, value):
         self._check(lib().nsgw_set_option(self._h, C.c_int32(key), C.c_int32(value)), "nsgw_set_option")

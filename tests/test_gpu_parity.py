@@ -563,6 +563,82 @@ def test_run_many_equals_single_runs(nsgw):
         assert np.all(np.diff(rows[:, spec["ndim"]]) >= 0)            # dead points come out in ascending logL
 
 
+# ------------------------------------------------------------------------------------------------------
+# Relative binning (R:L24): set-up (edges: integers, bit-exact; summary data) and evaluation against the oracle's
+# ------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind,dets,f_max,T", [(W.LIKE_TAYLORF2, ["H1", "L1"], 1024.0, 4.0),       # config-2 shape
+                                               (W.LIKE_PHENOMD, ["H1", "L1"], 1024.0, 4.0),        # config-3 shape
+                                               (W.LIKE_PHENOMD, ["H1", "L1", "V1"], 512.0, 8.0),   # three detectors
+                                               (W.LIKE_TAYLORF2, ["L1"], 128.0, 2.0)])             # one detector, short grid
+def test_relbin_parity(nsgw, kind, dets, f_max, T):
+    spec = W.gw_spec(kind, dets, T, f_max, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 15.0, wf)
+    P = O.OracleProblem(spec)
+    nd = len(dets)
+    h = nsgw.Handle(spec)
+    for eps in (0.5, 0.11):
+        rb = P.relbin(W.INJ_C3, eps=eps)
+        nb = h.relbin_setup(W.INJ_C3, eps=eps)
+        ed, A0, A1, B0, B1 = h.relbin_get()
+        assert nb == rb.n_bins and np.array_equal(ed, rb.edges())          # integer work: bit-exact
+        oA0, oA1, oB0, oB1 = rb.summary()
+        sc = np.abs(oA0).max()
+        np.testing.assert_allclose(A0, oA0, rtol=0, atol=1e-10 * sc)
+        np.testing.assert_allclose(A1, oA1, rtol=0, atol=1e-10 * np.abs(oA1).max())
+        np.testing.assert_allclose(B0, oB0, rtol=1e-11, atol=0)
+        np.testing.assert_allclose(B1, oB1, rtol=0, atol=1e-11 * np.abs(oB1).max())
+        # rows: prior draws (far from the fiducial point: large, but identical, approximation errors), posterior-like scatter,
+        # the fiducial point itself and an unphysical row
+        rng = np.random.default_rng(8)
+        u0 = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+        u = np.concatenate([W.uniforms(200, 11, 55), u0[None, :] + rng.normal(0, 1, (330, 11)) * np.array(W.C5_SIGMA) * 0.1])
+        per = np.array(spec["periodic"], bool)
+        u[:, per] -= np.floor(u[:, per])
+        u[:, ~per] = np.clip(u[:, ~per], 1e-6, 1 - 1e-6)
+        th = P.prior_transform(u)
+        th[0] = W.INJ_C3
+        th[1, 1] = 1.5
+        lo, po = rb.loglike(th, parts=True)
+        lg, pg = h.gw_loglike_relbin_batch(dev(th), parts=True)
+        lg, pg = lg.cpu().numpy(), pg.cpu().numpy()
+        assert np.isneginf(lg[1]) and np.isneginf(lo[1])
+        ok = np.isfinite(lo)
+        scale = np.maximum(1.0, np.abs(po[ok, 0::2]).sum(1) + 0.5 * np.abs(po[ok, 1::2]).sum(1))
+        assert np.max(np.abs(lg[ok] - lo[ok]) / scale) < 1e-10
+        np.testing.assert_allclose(pg[ok], po[ok], rtol=0, atol=1e-10 * scale.max())
+        # and the approximation itself: equal to the exact kernel at the fiducial point
+        exact = h.gw_loglike_batch(dev(th[:1])).cpu().numpy()[0]
+        assert abs(lg[0] - exact) < 1e-9 * max(1.0, abs(exact))
+
+
+def test_relbin_given_edges_and_errors(nsgw, c2):
+    h = nsgw.Handle(c2)
+    P = O.OracleProblem(c2)
+    with pytest.raises(nsgw.NsgwError):
+        h.gw_loglike_relbin_batch(dev(np.array([W.INJ_C3])))              # no set-up yet
+    nf = c2["n_freq"]
+    edges = [0, 5, 6, 40, 400, 2000, nf - 1]
+    assert h.relbin_setup(W.INJ_C3, edges=edges) == len(edges) - 1
+    ed, A0, A1, B0, B1 = h.relbin_get()
+    assert list(ed) == edges
+    _, parts = P.gw_loglike(np.array([W.INJ_C3]), parts=True)
+    assert abs(B0[0].sum() - parts[0, 1]) < 1e-10 * parts[0, 1]           # the bins partition <h0, h0>
+    for bad in ([1, 5, nf - 1], [0, 5, 5, nf - 1], [0, 7, nf - 2], [0]):
+        with pytest.raises(nsgw.NsgwError):
+            h.relbin_setup(W.INJ_C3, edges=bad)
+    bad_th = list(W.INJ_C3)
+    bad_th[1] = 2.0
+    with pytest.raises(nsgw.NsgwError):
+        h.relbin_setup(bad_th)
+    with pytest.raises(nsgw.NsgwError):
+        h.relbin_setup(W.INJ_C3, eps=-1.0)
+    with pytest.raises(nsgw.NsgwError):
+        h.relbin_setup(W.INJ_C3, eps=1e-9)                                # more bins than grid points
+    spec1, smp1, _ = W.config1()
+    with pytest.raises(nsgw.NsgwError):
+        nsgw.Handle(spec1, smp1).relbin_setup(W.INJ_C3)                   # not a GW handle
+
+
 def test_error_codes(nsgw, c2):
     import ctypes as C
     h = nsgw.Handle(c2)
