@@ -182,6 +182,10 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * its own size between 1 and 32 from its chain: halved after a chunk with an acceptance, doubled after one without),
  * 1..32 = fixed (1 = one likelihood evaluation at a time, the sequential algorithm). */
 #define NSGW_OPT_WALK_SPEC 1
+/* key NSGW_OPT_LIKELIHOOD: 0 = exact likelihood (default), 1 = relative binning (needs ns_relbin_setup): used by ns_step / ns_run
+ * / ns_walk_batch / ns_loglike_u_batch.  Setting it re-evaluates the live points' logL with the chosen likelihood (default
+ * stream, synchronises); do so again after a new ns_relbin_setup. */
+#define NSGW_OPT_LIKELIHOOD 2
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */

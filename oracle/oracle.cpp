@@ -78,6 +78,8 @@ struct orc_problem {
   double phenom_table[19][11];
   const double* strain;  // [n_det][n_freq][2]
   const double* psd;     // [n_det][n_freq]
+  const void* relbin;    // optional: relative-binning data (orc_relbin_create); when set, loglike_from_u -- and so the walk, the
+                         // NS step and the runs -- use the relative-binning likelihood (R:L24) instead of the exact one
 };
 
 struct orc_sampler_cfg {
@@ -495,11 +497,14 @@ double shell_loglike(const orc_problem* p, const double* u) {
   return -r;
 }
 
+double relbin_loglike_any(const orc_problem* p, const double* th);   // defined with the relative-binning code below
+
 double loglike_from_u(const orc_problem* p, const double* u) {
   if (p->like_kind == LIKE_SHELL) return shell_loglike(p, u);
   double th[16];
   prior_transform(p, u, th);
   if (p->like_kind == LIKE_GAUSS) return toy_loglike(p, th);
+  if (p->relbin) return relbin_loglike_any(p, th);
   return gw_loglike(p, th, nullptr);
 }
 
@@ -1001,6 +1006,14 @@ static double relbin_loglike_one(const orc_problem* p, const RelBin* rb, const d
   }
   return logl;
 }
+
+}  // extern "C"
+namespace {
+double relbin_loglike_any(const orc_problem* p, const double* th) {
+  return relbin_loglike_one(p, static_cast<const RelBin*>(p->relbin), th, nullptr);
+}
+}  // namespace
+extern "C" {
 
 void orc_relbin_loglike(const orc_problem* p, const void* h, const double* theta, int64_t B, double* logl, double* parts, int threads) {
   const RelBin* rb = static_cast<const RelBin*>(h);

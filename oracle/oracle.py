@@ -25,6 +25,7 @@ class Problem(C.Structure):
         ("toy_mean", C.c_double * 16), ("toy_prec", C.c_double * 256), ("toy_lognorm", C.c_double),
         ("phenom_table", (C.c_double * 11) * 19),
         ("strain", c_d_p), ("psd", c_d_p),
+        ("relbin", C.c_void_p),
     ]
 
 
@@ -147,6 +148,11 @@ class OracleProblem:
     # ---- relative binning (DESIGN.md R:L24) ----------------------------------------------------------
     def relbin(self, theta0, chi=1.0, eps=0.5):
         return OracleRelBin(self, theta0, chi, eps)
+
+    def use_relbin(self, rb):
+        """Routes loglike_u, walk and the sampler through the relative-binning likelihood `rb` (None: back to the exact one)."""
+        self._rb_in_use = rb                      # keep it alive
+        self.p.relbin = rb.h if rb is not None else None
 
     def loglike_u(self, u, threads=0):
         u = _f64(u).reshape(-1, self.ndim)

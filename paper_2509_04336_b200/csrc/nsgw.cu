@@ -886,8 +886,9 @@ constexpr size_t walk_smem_bytes(int dm) {
 
 // NT threads per walker: 128 when all walkers of the batch are resident at 4 CTAs per SM, 96 (5 per SM) or 64 (8 per SM) when
 // that keeps a larger batch in one wave (config 4: k = 700 on 148 SMs).
-template <int MODEL, int NDET, int NT>
-__global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a) {
+// RB: the likelihood of a proposal is the relative-binning one (edges instead of a full bin sweep).
+template <int MODEL, int NDET, int NT, bool RB>
+__global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a, RbDev rb) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NW = NT / 32, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
   constexpr int DMX = kWalkDMax;
@@ -899,6 +900,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   double2* step = tabW + DM * ND1 * NW;                            // [DM][ND1]
   double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
   double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
+  double2* rbuf = reinterpret_cast<double2*>(cbs + DM * (CB_SIZE + kMaxDim));              // RB: [NDET][nb + 1] ratios at the edges
   __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DMX];
   __shared__ MathTables mtab;
   __shared__ bool active[PG];
@@ -971,7 +973,49 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
     int n_in = 0;
 #pragma unroll
     for (int j = 0; j < DMX; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
-    if (n_in > 0) {
+    if (RB && n_in > 0) {
+      // ---- phase B, relative binning: per proposal, ratios r = g/g0 at the edges (edges over threads), then the bins
+      const int nbn = rb.nb;
+      for (int sl = 0; sl < nd; ++sl) {
+        if (s_flag[sl] != 2) continue;
+        const CbPtr cb{cbs + sl * CB_SIZE};
+        for (int i = tid; i <= nbn; i += NT) {
+          double2 g[NDET];
+          gw_g_at<MODEL, NDET>(cb, tb, __ldg(rb.edge + i), &mtab, g);
+#pragma unroll
+          for (int d = 0; d < NDET; ++d) {
+            const double2 ig = __ldg(rb.ig0 + (size_t)d * (nbn + 1) + i);
+            rbuf[d * (nbn + 1) + i] = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
+          }
+        }
+        __syncthreads();
+        double v[2 * NDET];
+#pragma unroll
+        for (int i = 0; i < 2 * NDET; ++i) v[i] = 0.0;
+        for (int b = tid; b < nbn; b += NT) {
+          const double iw = __ldg(rb.inv_w + b);
+#pragma unroll
+          for (int d = 0; d < NDET; ++d) {
+            const double2 lo = rbuf[d * (nbn + 1) + b], hi = rbuf[d * (nbn + 1) + b + 1];
+            const size_t ib = (size_t)d * nbn + b;
+            const double r0r = 0.5 * (lo.x + hi.x), r0i = 0.5 * (lo.y + hi.y);
+            const double r1r = (hi.x - lo.x) * iw, r1i = (hi.y - lo.y) * iw;
+            const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
+            v[2 * d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
+            v[2 * d + 1] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
+          }
+        }
+        block_reduce<2 * NDET, NT>(v, red, out);
+        if (tid == 0) {
+          double l = 0.0;
+#pragma unroll
+          for (int d = 0; d < NDET; ++d) l += out[2 * d] - 0.5 * out[2 * d + 1];
+          s_logl[sl] = l;
+        }
+        __syncthreads();
+      }
+    }
+    if (!RB && n_in > 0) {
       build_phasor_tables<NDET, NT>(cfg, cbs, nd, tabL, tabW, step);
       __syncthreads();
       // ---- phase B: sweeps, PG particles at a time (a single left-over goes through the one-particle loop)
@@ -1235,6 +1279,7 @@ struct ns_handle {
   double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [n_ranges][N][B]
   size_t partial_cap = 0;
   int n_sm = 148;
+  int opt_like = 0;             // 0 exact likelihood, 1 relative binning (sampler and ns_loglike_u_batch)
   int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
   long long cb_cap = 0;
@@ -1404,6 +1449,40 @@ int loglike_theta(ns_handle* h, const double* theta_dev, long long B, double* lo
   return launch_bins<2>(h, B, logl, parts, s);
 }
 
+// theta[B,11] -> relative-binning logL (set-up kernel + edge evaluation).
+int relbin_theta(ns_handle* h, const double* theta_dev, long long B, double* logl, double* parts, cudaStream_t s) {
+  if (B == 0) return 0;
+  int rc = ensure_cb(h, B);
+  if (rc) return rc;
+  const unsigned gs = (unsigned)((B + 127) / 128), gr = (unsigned)((B + kRbThreads - 1) / kRbThreads);
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  const int nd = h->cfg.n_det;
+  if (tf2) k_setup<1><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+  else k_setup<2><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
+  LAUNCH_CHECK(h);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof && h->prof_ev.size() < 4096) {
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, s);
+  }
+  constexpr size_t kSm2 = sizeof(double) * CB_SIZE * kRbThreads;
+  static bool attr_set = false;
+  if (!attr_set) {
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
+    attr_set = true;
+  }
+#define RB_EVAL(M, N, SM) k_relbin<M, N><<<gr, kRbThreads, SM, s>>>(h->d_cfg, h->tb, h->rb, h->d_cb, B, logl, parts)
+  if (tf2) { if (nd == 1) RB_EVAL(1, 1, 0); else if (nd == 2) RB_EVAL(1, 2, 0); else RB_EVAL(1, 3, 0); }
+  else { if (nd == 1) RB_EVAL(2, 1, kSm2); else if (nd == 2) RB_EVAL(2, 2, kSm2); else RB_EVAL(2, 3, kSm2); }
+#undef RB_EVAL
+  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+
 int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cudaStream_t s) {
   if (B == 0) return 0;
   if (!is_gw(h->cfg.like_kind)) {
@@ -1416,29 +1495,40 @@ int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cuda
   long long N = B * h->cfg.ndim;
   k_prior_transform<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(h->d_cfg, u_dev, B, h->d_theta);
   LAUNCH_CHECK(h);
+  if (h->opt_like == 1) return relbin_theta(h, h->d_theta, B, logl, nullptr, s);
   return loglike_theta(h, h->d_theta, B, logl, nullptr, s);
 }
 
-template <int MODEL, int NDET, int NT>
-int launch_walk_gw_nt(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
-  auto kern = k_walk_gw<MODEL, NDET, NT>;
+template <int MODEL, int NDET, int NT, bool RB>
+int launch_walk_gw_k(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
+  auto kern = k_walk_gw<MODEL, NDET, NT, RB>;
+  const size_t extra = RB ? sizeof(double2) * NDET * ((size_t)h->rb.nb + 1) : 0;
+  if (RB && extra > 64 * 1024) return fail(h, -5, "too many relative-binning bins for the walk kernel (n_det (n_bins + 1) <= 4096)");
   static bool attr_set = false;
   if (!attr_set) {
-    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)walk_smem_bytes<NDET, NT>(kWalkDMax)));
+    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + (RB ? 64 * 1024 : 0))));
     attr_set = true;
   }
   a.spec_cap = dm;
   a.spec = std::min(a.spec, dm);
-  kern<<<(unsigned)a.B, NT, walk_smem_bytes<NDET, NT>(dm), s>>>(h->d_cfg, h->tb, a);
+  kern<<<(unsigned)a.B, NT, walk_smem_bytes<NDET, NT>(dm) + extra, s>>>(h->d_cfg, h->tb, a, h->rb);
   LAUNCH_CHECK(h);
   return 0;
 }
 
-// Longest chunk buffers (32, 16 or 8 steps) with which `ctas` CTAs of the kernel still fit the SM's shared memory.
+template <int MODEL, int NDET, int NT>
+int launch_walk_gw_nt(ns_handle* h, const WalkArgs& a, int dm, cudaStream_t s) {
+  if (h->opt_like == 1) return launch_walk_gw_k<MODEL, NDET, NT, true>(h, a, dm, s);
+  return launch_walk_gw_k<MODEL, NDET, NT, false>(h, a, dm, s);
+}
+
+// Longest chunk buffers (32, 16 or 8 slots) with which `ctas` CTAs of the kernel still fit the SM's shared memory.
 template <int NDET, int NT>
-int walk_chunk_cap(int ctas) {
+int walk_chunk_cap(const ns_handle* h, int ctas) {
+  const size_t extra = h->opt_like == 1 ? sizeof(double2) * NDET * ((size_t)h->rb.nb + 1) : 0;
   for (int dm = kWalkDMax; dm > 8; dm /= 2)
-    if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + 10496) <= (size_t)225 * 1024) return dm;
+    if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + extra + 10496) <= (size_t)225 * 1024) return dm;
   return 8;
 }
 
@@ -1447,9 +1537,9 @@ template <int MODEL, int NDET>
 int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const long long sm = h->n_sm;
   if (a.B <= 4 * sm || a.B > 8 * sm)   // <= 4 walkers per SM, or many waves anyway
-    return launch_walk_gw_nt<MODEL, NDET, 128>(h, a, walk_chunk_cap<NDET, 128>(4), s);
-  if (a.B <= 5 * sm) return launch_walk_gw_nt<MODEL, NDET, 96>(h, a, walk_chunk_cap<NDET, 96>(5), s);
-  return launch_walk_gw_nt<MODEL, NDET, 64>(h, a, walk_chunk_cap<NDET, 64>(8), s);
+    return launch_walk_gw_nt<MODEL, NDET, 128>(h, a, walk_chunk_cap<NDET, 128>(h, 4), s);
+  if (a.B <= 5 * sm) return launch_walk_gw_nt<MODEL, NDET, 96>(h, a, walk_chunk_cap<NDET, 96>(h, 5), s);
+  return launch_walk_gw_nt<MODEL, NDET, 64>(h, a, walk_chunk_cap<NDET, 64>(h, 8), s);
 }
 
 int launch_walk(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
@@ -1905,36 +1995,7 @@ int gw_loglike_relbin_batch(ns_handle* h, const double* theta_dev, int64_t B, do
   if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
   if (h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");
   if (B < 0 || (B > 0 && (!theta_dev || !logl_dev))) return fail(h, -1, "bad arguments");
-  if (B == 0) return 0;
-  cudaStream_t s = (cudaStream_t)stream;
-  int rc = ensure_cb(h, B);
-  if (rc) return rc;
-  const unsigned gs = (unsigned)((B + 127) / 128), gr = (unsigned)((B + kRbThreads - 1) / kRbThreads);
-  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
-  const int nd = h->cfg.n_det;
-  if (tf2) k_setup<1><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
-  else k_setup<2><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, h->d_cb);
-  LAUNCH_CHECK(h);
-  cudaEvent_t e0 = nullptr, e1 = nullptr;
-  if (h->prof && h->prof_ev.size() < 4096) {
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    cudaEventRecord(e0, s);
-  }
-  constexpr size_t kSm2 = sizeof(double) * CB_SIZE * kRbThreads;
-  static bool attr_set = false;
-  if (!attr_set) {
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    attr_set = true;
-  }
-#define RB_EVAL(M, N, SM) k_relbin<M, N><<<gr, kRbThreads, SM, s>>>(h->d_cfg, h->tb, h->rb, h->d_cb, B, logl_dev, parts_dev)
-  if (tf2) { if (nd == 1) RB_EVAL(1, 1, 0); else if (nd == 2) RB_EVAL(1, 2, 0); else RB_EVAL(1, 3, 0); }
-  else { if (nd == 1) RB_EVAL(2, 1, kSm2); else if (nd == 2) RB_EVAL(2, 2, kSm2); else RB_EVAL(2, 3, kSm2); }
-#undef RB_EVAL
-  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
-  LAUNCH_CHECK(h);
-  return 0;
+  return relbin_theta(h, theta_dev, B, logl_dev, parts_dev, (cudaStream_t)stream);
 }
 
 int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream) {
@@ -1969,6 +2030,17 @@ int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (!h) return -3;
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
   if (key == NSGW_OPT_WALK_SPEC && value >= 0 && value <= kWalkDMax) { h->opt_walk_spec = value; return 0; }
+  if (key == NSGW_OPT_LIKELIHOOD && (value == 0 || value == 1)) {
+    if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+    if (value == 1 && h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");
+    h->opt_like = value;
+    if (h->cfg.n_live > 0) {   // the live points' logL must come from the likelihood the sampler will compare against
+      int rc = loglike_u(h, h->d_live_u, h->cfg.n_live, h->d_live_l, nullptr);
+      if (rc) return rc;
+      CU_CHECK(h, cudaStreamSynchronize(nullptr));
+    }
+    return 0;
+  }
   return fail(h, -1, "unknown option or value");
 }
 

@@ -331,14 +331,19 @@ def _sorted_live(u, l):
     return u[o], l[o]
 
 
-def _step_parity(nsgw, spec, smp, nsteps, seed, tol_l):
+def _step_parity(nsgw, spec, smp, nsteps, seed, tol_l, relbin_theta0=None):
     """Step-for-step comparison on the same seed and live points.  Integer work (walk length, counters) must be identical;
     floating-point state agrees to rounding drift.  Near-tied logL (a gamma = 1 proposal from a donor lands on another donor
     to 1 ulp) may be ranked in either order, so live sets are compared as sets (sorted by logL), not slot by slot."""
     P = O.OracleProblem(spec)
+    if relbin_theta0 is not None:
+        P.use_relbin(P.relbin(relbin_theta0))         # both sides sample the relative-binning likelihood (R:L24)
     S = O.OracleSampler(P, smp["n_live"], smp["n_delete"], smp["naccept"], smp["maxmcmc"], smp["walks0"], smp["delay"], seed=seed)
     u0, _ = S.live()
     h = nsgw.Handle(spec, smp, live_u=u0, seed=seed)
+    if relbin_theta0 is not None:
+        h.relbin_setup(relbin_theta0)
+        h.set_option(2, 1)
     D, k = spec["ndim"], smp["n_delete"]
     for it in range(nsteps):
         dead_g = torch.empty(k, D + 3, dtype=torch.float64, device="cuda")
@@ -609,6 +614,73 @@ def test_relbin_parity(nsgw, kind, dets, f_max, T):
         # and the approximation itself: equal to the exact kernel at the fiducial point
         exact = h.gw_loglike_batch(dev(th[:1])).cpu().numpy()[0]
         assert abs(lg[0] - exact) < 1e-9 * max(1.0, abs(exact))
+
+
+def test_ns_step_parity_gw_relbin(nsgw):
+    # the sampler on the relative-binning likelihood: step-for-step against the oracle's sampler on its relative-binning likelihood
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 256.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    smp = dict(n_live=120, n_delete=60, naccept=8, maxmcmc=60, walks0=12.0, delay=-1.0)
+    _step_parity(nsgw, spec, smp, 4, 8, 1e-8, relbin_theta0=W.INJ_C3)
+
+
+@pytest.mark.parametrize("kind,dets", [(W.LIKE_TAYLORF2, ["H1", "L1"]), (W.LIKE_PHENOMD, ["H1", "L1", "V1"])])
+def test_walk_relbin_decision_parity(nsgw, kind, dets):
+    spec = W.gw_spec(kind, dets, 4.0, 256.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    P = O.OracleProblem(spec)
+    P.use_relbin(P.relbin(W.INJ_C3, eps=0.3))
+    h = nsgw.Handle(spec)
+    h.relbin_setup(W.INJ_C3, eps=0.3)
+    h.set_option(2, 1)
+    rng = np.random.default_rng(14)
+    m, B, Wlen = 250, 300, 9
+    u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+    donors = u_inj[None, :] + rng.normal(0, 1, (m, 11)) * np.array(W.C5_SIGMA) * 0.5
+    per = np.array(spec["periodic"], bool)
+    donors[:, per] -= np.floor(donors[:, per])
+    donors[:, ~per] = np.clip(donors[:, ~per], 1e-6, 1 - 1e-6)
+    ld = P.loglike_u(donors)
+    np.testing.assert_allclose(h.loglike_u_batch(dev(donors)).cpu().numpy(), ld, rtol=0, atol=1e-9 * np.abs(ld).max())
+    lstar = float(np.median(ld))
+    start = rng.integers(0, m, B)
+    u0, l0 = donors[start].copy(), ld[start].copy()
+    res_o = P.walk(donors, u0, l0, lstar, Wlen, 4242, (5 << 24) | 2, slot0=0, trace=True)
+    ug, lg_ = dev(u0), dev(l0)
+    res_g = h.walk_batch(dev(donors), ug, lg_, lstar, Wlen, 4242, (5 << 24) | 2, slot0=0, trace=True)
+    clean, n_exc, n_steps = _compare_traces(res_g, res_o, lstar, Wlen)
+    assert n_exc <= 2
+    for key in ("n_accept", "n_eval", "n_oob"):
+        assert np.array_equal(res_g[key].cpu().numpy()[clean], res_o[key][clean])
+    np.testing.assert_allclose(ug.cpu().numpy()[clean], res_o["u"][clean], rtol=0, atol=1e-13)
+    fl = res_o["flags"]
+    assert (fl & 1).any() and (fl & 2).any()
+
+
+def test_relbin_run_agrees_with_exact_run(nsgw):
+    """A full run on the relative-binning likelihood against the same run on the exact one (same seed, same live points): the
+    evidence agrees within the nested-sampling error (the approximation error in the bulk is < 0.05, pinned on the oracle)."""
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 512.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    free = (0, 1, 4, 8)
+    kinds, lo_, hi_ = list(spec["prior_kind"]), list(spec["prior_lo"]), list(spec["prior_hi"])
+    for d in range(11):
+        if d not in free:
+            kinds[d] = W.FIXED
+            lo_[d] = hi_[d] = W.INJ_C3[d]
+    spec["prior_kind"], spec["prior_lo"], spec["prior_hi"] = kinds, lo_, hi_
+    spec["periodic"] = [0] * 11
+    smp = dict(n_live=400, n_delete=200, naccept=20, maxmcmc=2000, walks0=50.0, delay=-1.0)
+    he = nsgw.Handle(spec, smp, seed=9)
+    ne, _ = he.run(0, 0.1, 200)
+    ze, ee, _ = he.finalize_evidence()
+    hr = nsgw.Handle(spec, smp, seed=9)
+    hr.relbin_setup(W.INJ_C3)
+    hr.set_option(2, 1)
+    nr, _ = hr.run(0, 0.1, 200)
+    zr, er, _ = hr.finalize_evidence()
+    assert abs(nr - ne) <= 3
+    assert abs(zr - ze) < 3.0 * math.hypot(ee, er) + 0.05, (zr, er, ze, ee)
 
 
 def test_relbin_given_edges_and_errors(nsgw, c2):

@@ -135,3 +135,20 @@ def test_unphysical_theta_and_bad_arguments(prob):
         P.relbin(th[1])
     with pytest.raises(ValueError):
         P.relbin(W.INJ_C3, eps=0.0)
+
+
+def test_sampler_routes_through_relbin_when_asked(prob):
+    spec, P = prob
+    rb = P.relbin(W.INJ_C3)
+    u = W.uniforms(50, 11, 3)
+    exact = P.loglike_u(u)
+    P.use_relbin(rb)
+    try:
+        np.testing.assert_array_equal(P.loglike_u(u), rb.loglike(P.prior_transform(u)))
+        # a short run on the approximate likelihood works end to end and uses the same code path
+        S = O.OracleSampler(P, 60, 30, 5, 40, 10.0, -1.0, seed=2)
+        st = S.step()
+        assert st["n_eval"] > 0 and np.isfinite(st["logz"])
+    finally:
+        P.use_relbin(None)
+    np.testing.assert_array_equal(P.loglike_u(u), exact)
