@@ -275,6 +275,32 @@ def run_ours(args):
                                     "evals_per_s": st["n_eval_total"] / wall}
         h3.close()
         if args.full_extras:
+            # config 3 on the relative-binning likelihood (fiducial = the injection, eps = 0.5), and the batched
+            # relative-binning evaluation on the config-2 data
+            h3r = nsgw.Handle(spec3, smp3, seed=1)
+            nbins = h3r.relbin_setup(W.INJ_C3)
+            h3r.set_option(2, 1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            nit, st = h3r.run(smp3["term_kind"], smp3["term_tol"], 4000)
+            logz, err, H = h3r.finalize_evidence()
+            wall = time.perf_counter() - t0
+            extras["ns_run_config3_relbin"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
+                                               "logz_err": err, "H": H, "n_bins": nbins, "walk_len_last": st["walk_len"],
+                                               "accept_mean_last": st["accept_mean"], "evals_per_s": st["n_eval_total"] / wall}
+            h3r.close()
+            nb2 = h.relbin_setup(W.INJ_C3)
+            rb_out = torch.empty(B, dtype=torch.float64, device="cuda")
+            for _ in range(3):
+                h.gw_loglike_relbin_batch(theta, out=rb_out)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            for _ in range(20):
+                h.gw_loglike_relbin_batch(theta, out=rb_out)
+            b.record(stream)
+            torch.cuda.synchronize()
+            rms = a.elapsed_time(b) / 20
+            extras["relbin_batch_config2"] = {"n_bins": nb2, "ms": rms, "evals_per_s": B / (rms * 1e-3)}
             # four config-3 runs with different seeds at once (ns_run_many): the runs' walk kernels share the SMs
             hs = [nsgw.Handle(spec3, smp3, seed=sd) for sd in (1, 2, 3, 4)]
             torch.cuda.synchronize()
