@@ -900,7 +900,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   double2* step = tabW + DM * ND1 * NW;                            // [DM][ND1]
   double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
   double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
-  double2* rbuf = reinterpret_cast<double2*>(cbs + DM * (CB_SIZE + kMaxDim));              // RB: [NDET][nb + 1] ratios at the edges
+  double2* rbuf = reinterpret_cast<double2*>(cbs + DM * (CB_SIZE + kMaxDim));              // RB: partial sums [32][NT/32][2 NDET]
   __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DMX];
   __shared__ MathTables mtab;
   __shared__ bool active[PG];
@@ -974,46 +974,55 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
 #pragma unroll
     for (int j = 0; j < DMX; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
     if (RB && n_in > 0) {
-      // ---- phase B, relative binning: per proposal, ratios r = g/g0 at the edges (edges over threads), then the bins
+      // ---- phase B, relative binning: NT/32 threads per proposal, each walks a contiguous run of bins edge by edge (ratio r = g/g0
+      // at the edge, then the bin between the previous edge and this one; the first edge of a run is recomputed by its owner), no
+      // barrier until the partial sums meet in shared memory
+      constexpr int T = NT / 32;
       const int nbn = rb.nb;
-      for (int sl = 0; sl < nd; ++sl) {
-        if (s_flag[sl] != 2) continue;
+      const int sl = tid / T, part = tid % T;
+      double v[2 * NDET];
+#pragma unroll
+      for (int i = 0; i < 2 * NDET; ++i) v[i] = 0.0;
+      if (sl < nd && s_flag[sl] == 2) {
         const CbPtr cb{cbs + sl * CB_SIZE};
-        for (int i = tid; i <= nbn; i += NT) {
+        const int per = (nbn + T - 1) / T, b0 = part * per, b1 = min(nbn, b0 + per);
+        double2 prev[NDET];
+        for (int i = b0; i <= b1 && b0 < b1; ++i) {
           double2 g[NDET];
           gw_g_at<MODEL, NDET>(cb, tb, __ldg(rb.edge + i), &mtab, g);
 #pragma unroll
           for (int d = 0; d < NDET; ++d) {
             const double2 ig = __ldg(rb.ig0 + (size_t)d * (nbn + 1) + i);
-            rbuf[d * (nbn + 1) + i] = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
+            const double2 r = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
+            if (i > b0) {
+              const size_t ib = (size_t)d * nbn + (i - 1);
+              const double iw = __ldg(rb.inv_w + (i - 1));
+              const double r0r = 0.5 * (prev[d].x + r.x), r0i = 0.5 * (prev[d].y + r.y);
+              const double r1r = (r.x - prev[d].x) * iw, r1i = (r.y - prev[d].y) * iw;
+              const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
+              v[2 * d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
+              v[2 * d + 1] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
+            }
+            prev[d] = r;
           }
         }
-        __syncthreads();
-        double v[2 * NDET];
-#pragma unroll
-        for (int i = 0; i < 2 * NDET; ++i) v[i] = 0.0;
-        for (int b = tid; b < nbn; b += NT) {
-          const double iw = __ldg(rb.inv_w + b);
-#pragma unroll
-          for (int d = 0; d < NDET; ++d) {
-            const double2 lo = rbuf[d * (nbn + 1) + b], hi = rbuf[d * (nbn + 1) + b + 1];
-            const size_t ib = (size_t)d * nbn + b;
-            const double r0r = 0.5 * (lo.x + hi.x), r0i = 0.5 * (lo.y + hi.y);
-            const double r1r = (hi.x - lo.x) * iw, r1i = (hi.y - lo.y) * iw;
-            const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
-            v[2 * d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
-            v[2 * d + 1] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
-          }
-        }
-        block_reduce<2 * NDET, NT>(v, red, out);
-        if (tid == 0) {
-          double l = 0.0;
-#pragma unroll
-          for (int d = 0; d < NDET; ++d) l += out[2 * d] - 0.5 * out[2 * d + 1];
-          s_logl[sl] = l;
-        }
-        __syncthreads();
       }
+      double* rpart = reinterpret_cast<double*>(rbuf);      // [32 slots][T][2 NDET]
+#pragma unroll
+      for (int i = 0; i < 2 * NDET; ++i) rpart[(sl * T + part) * 2 * NDET + i] = v[i];
+      __syncthreads();
+      if (part == 0 && sl < nd && s_flag[sl] == 2) {
+        double l = 0.0;
+#pragma unroll
+        for (int d = 0; d < NDET; ++d) {
+          double dh = 0.0, hh = 0.0;
+#pragma unroll
+          for (int t = 0; t < T; ++t) { dh += rpart[(sl * T + t) * 2 * NDET + 2 * d]; hh += rpart[(sl * T + t) * 2 * NDET + 2 * d + 1]; }
+          l += dh - 0.5 * hh;
+        }
+        s_logl[sl] = l;
+      }
+      __syncthreads();
     }
     if (!RB && n_in > 0) {
       build_phasor_tables<NDET, NT>(cfg, cbs, nd, tabL, tabW, step);
@@ -1502,12 +1511,11 @@ int loglike_u(ns_handle* h, const double* u_dev, long long B, double* logl, cuda
 template <int MODEL, int NDET, int NT, bool RB>
 int launch_walk_gw_k(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
   auto kern = k_walk_gw<MODEL, NDET, NT, RB>;
-  const size_t extra = RB ? sizeof(double2) * NDET * ((size_t)h->rb.nb + 1) : 0;
-  if (RB && extra > 64 * 1024) return fail(h, -5, "too many relative-binning bins for the walk kernel (n_det (n_bins + 1) <= 4096)");
+  const size_t extra = RB ? sizeof(double) * NT * 2 * NDET : 0;   // partial sums of phase B
   static bool attr_set = false;
   if (!attr_set) {
     CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + (RB ? 64 * 1024 : 0))));
+                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + extra)));
     attr_set = true;
   }
   a.spec_cap = dm;
@@ -1526,7 +1534,7 @@ int launch_walk_gw_nt(ns_handle* h, const WalkArgs& a, int dm, cudaStream_t s) {
 // Longest chunk buffers (32, 16 or 8 slots) with which `ctas` CTAs of the kernel still fit the SM's shared memory.
 template <int NDET, int NT>
 int walk_chunk_cap(const ns_handle* h, int ctas) {
-  const size_t extra = h->opt_like == 1 ? sizeof(double2) * NDET * ((size_t)h->rb.nb + 1) : 0;
+  const size_t extra = h->opt_like == 1 ? sizeof(double) * NT * 2 * NDET : 0;
   for (int dm = kWalkDMax; dm > 8; dm /= 2)
     if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + extra + 10496) <= (size_t)225 * 1024) return dm;
   return 8;
