@@ -27,10 +27,8 @@ namespace {
 std::atomic<long long> g_launches{0};
 thread_local std::string g_init_error;
 
-// One CTA shape for every bin sweep (likelihood batch and walk): the same particle then gets bit-identical logL from
-// either entry point (same per-thread bin assignment, same reduction tree).
+// CTA width of the CTA-per-particle sweep kernel (k_bins); the walk kernel chooses 128 / 96 / 64 by batch size.
 constexpr int kBinsThreads = 256;
-constexpr int kWalkThreads = 128;
 
 // ======================================================================================================
 // Device state of the sampler
@@ -1527,7 +1525,6 @@ int launch_walk_gw_k(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
 
 template <int MODEL, int NDET, int NT>
 int launch_walk_gw_nt(ns_handle* h, const WalkArgs& a, int dm, cudaStream_t s) {
-  if (h->opt_like == 1) return launch_walk_gw_k<MODEL, NDET, NT, true>(h, a, dm, s);
   return launch_walk_gw_k<MODEL, NDET, NT, false>(h, a, dm, s);
 }
 
@@ -1544,6 +1541,8 @@ int walk_chunk_cap(const ns_handle* h, int ctas) {
 template <int MODEL, int NDET>
 int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const long long sm = h->n_sm;
+  // relative binning: the sweep is 62-odd edge evaluations, residency is not what limits it -- one geometry (128 threads)
+  if (h->opt_like == 1) return launch_walk_gw_k<MODEL, NDET, 128, true>(h, a, walk_chunk_cap<NDET, 128>(h, 4), s);
   if (a.B <= 4 * sm || a.B > 8 * sm)   // <= 4 walkers per SM, or many waves anyway
     return launch_walk_gw_nt<MODEL, NDET, 128>(h, a, walk_chunk_cap<NDET, 128>(h, 4), s);
   if (a.B <= 5 * sm) return launch_walk_gw_nt<MODEL, NDET, 96>(h, a, walk_chunk_cap<NDET, 96>(h, 5), s);
