@@ -669,21 +669,78 @@ __global__ void __launch_bounds__(128) k_rb_summary(const DevCfg* __restrict__ c
   }
 }
 
-// Evaluation: one thread per particle, loop over the N_b + 1 edges (all lanes at the same edge: table and summary loads are
-// warp-uniform), ratio r = g/g0 at the edge, then the bin between the previous edge and this one.
+// Evaluation: one thread per particle, loop over the N_b + 1 edges (all lanes at the same edge).  The per-edge data -- the ten
+// basis values, f^3/4, 1/g0 per detector -- and the per-bin summary data are staged once per CTA in shared memory (18 + 8 n_det
+// and 1 + 6 n_det doubles per edge / bin) and read with warp-uniform LDS; ratio r = g/g0 at the edge, then the bin between the
+// previous edge and this one.
 constexpr int kRbThreads = 128;
+
+template <int NDET>
+struct RbEdge {           // one edge (and the bin that ends at it)
+  double y5, y3, y2, y, L, x, xL, x2, f, f34;
+  double2 ig0[NDET];      // 1 / g0 at the edge
+  double2 A0[NDET], A1[NDET];
+  double B0[NDET], B1[NDET];
+  double inv_w;
+  double pad;
+};
+
+template <int MODEL, int NDET, class CB>
+__device__ __forceinline__ void gw_g_edge(const CB& cb, const RbEdge<NDET>& e, const MathTables* mt, double2 (&g)[NDET]) {
+  BinBasis b;
+  b.y5 = e.y5; b.y3 = e.y3; b.y2 = e.y2; b.y = e.y; b.L = e.L; b.x = e.x; b.xL = e.xL; b.x2 = e.x2; b.f = e.f; b.f34 = e.f34;
+  double q, amp = 1.0;
+  if (MODEL == 1) {
+    q = fma(cb(CB_PH + 0), b.y5, cb(CB_PH + 4));
+    q = fma(cb(CB_PH + 1), b.y3, q);
+    q = fma(cb(CB_PH + 2), b.y2, q);
+    q = fma(cb(CB_PH + 3), b.y, q);
+    q = fma(cb(CB_PH + 5), b.L, q);
+    q = fma(cb(CB_PH + 6), b.x, q);
+    q = fma(cb(CB_PH + 7), b.xL, q);
+    q = fma(cb(CB_PH + 8), b.x2, q);
+    q = fma(cb(CB_PH + 9), b.f, q);
+  } else {
+    phenom_bin_t(cb, b, mt, exp_tab(cb(CB_AM + 3) * (b.f - cb(CB_AM + 0)), mt), q, amp);
+  }
+#pragma unroll
+  for (int d = 0; d < NDET; ++d) {
+    double sn, cs;
+    sincos_lut(64.0 * fma(-cb(CB_DET + 4 * d + 2), b.f, q), mt, sn, cs);
+    const double cr = cb(CB_DET + 4 * d), ci = cb(CB_DET + 4 * d + 1);
+    g[d] = make_double2(amp * fma(cr, cs, ci * sn), amp * fma(ci, cs, -(cr * sn)));
+  }
+}
 
 template <int MODEL, int NDET>
 __global__ void __launch_bounds__(kRbThreads) k_relbin(const DevCfg* __restrict__ cfgp, Tables tb, RbDev rb, const double* __restrict__ cbs_g,
                                                         long long B, double* logl, double* parts) {
   constexpr int NT = kRbThreads;
   __shared__ MathTables mtab;
-  extern __shared__ __align__(16) double rb_cbT[];   // PhenomD-form: [CB_SIZE][NT] coefficient blocks, transposed
+  extern __shared__ __align__(16) unsigned char rb_smem[];
+  const int nb = rb.nb;
+  RbEdge<NDET>* ed = reinterpret_cast<RbEdge<NDET>*>(rb_smem);                    // [nb + 1]
+  double* rb_cbT = reinterpret_cast<double*>(ed + (nb + 1));                       // PhenomD-form: [CB_SIZE][NT], transposed
   const int tid = threadIdx.x;
   const long long p0 = (long long)blockIdx.x * NT, p = p0 + tid;
   const bool have = p < B;
   load_math_tables(&mtab, tb.mt, tid, NT);
-  // coefficient block of this thread's particle: TaylorF2 -> registers through a 16-entry local copy; PhenomD-form -> shared
+  for (int i = tid; i <= nb; i += NT) {
+    const int k = __ldg(rb.edge + i);
+    const BinBasis b = make_basis(tb, k, MODEL == 2);
+    RbEdge<NDET> e;
+    e.y5 = b.y5; e.y3 = b.y3; e.y2 = b.y2; e.y = b.y; e.L = b.L; e.x = b.x; e.xL = b.xL; e.x2 = b.x2; e.f = b.f; e.f34 = b.f34;
+    e.inv_w = (i > 0) ? __ldg(rb.inv_w + (i - 1)) : 0.0;
+    e.pad = 0.0;
+#pragma unroll
+    for (int d = 0; d < NDET; ++d) {
+      e.ig0[d] = __ldg(rb.ig0 + (size_t)d * (nb + 1) + i);
+      const size_t ib = (size_t)d * nb + (i > 0 ? i - 1 : 0);
+      e.A0[d] = __ldg(rb.A0 + ib); e.A1[d] = __ldg(rb.A1 + ib); e.B0[d] = __ldg(rb.B0 + ib); e.B1[d] = __ldg(rb.B1 + ib);
+    }
+    ed[i] = e;
+  }
+  // coefficient block of this thread's particle: TaylorF2 -> registers; PhenomD-form -> shared memory, transposed
   double cbl[MODEL == 1 ? 30 : 1];
   if (MODEL == 1) {
 #pragma unroll
@@ -699,24 +756,23 @@ __global__ void __launch_bounds__(kRbThreads) k_relbin(const DevCfg* __restrict_
   double dh[NDET], hh[NDET];
 #pragma unroll
   for (int d = 0; d < NDET; ++d) { dh[d] = 0.0; hh[d] = 0.0; prev[d] = make_double2(0.0, 0.0); }
-  const int nb = rb.nb;
+#pragma unroll 2
   for (int i = 0; i <= nb; ++i) {
-    const int k = __ldg(rb.edge + i);
+    const RbEdge<NDET>& e = ed[i];
     double2 g[NDET];
-    if (MODEL == 1) gw_g_at<MODEL, NDET>(CbPtr{cbl}, tb, k, &mtab, g);
-    else gw_g_at<MODEL, NDET>(CbStrided{rb_cbT + tid, NT}, tb, k, &mtab, g);
+    if (MODEL == 1) gw_g_edge<MODEL, NDET>(CbPtr{cbl}, e, &mtab, g);
+    else gw_g_edge<MODEL, NDET>(CbStrided{rb_cbT + tid, NT}, e, &mtab, g);
 #pragma unroll
     for (int d = 0; d < NDET; ++d) {
-      const double2 ig = __ldg(rb.ig0 + (size_t)d * (nb + 1) + i);
+      const double2 ig = e.ig0[d];
       const double2 r = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
       if (i > 0) {
-        const size_t ib = (size_t)d * nb + (i - 1);
-        const double iw = __ldg(rb.inv_w + (i - 1));
+        const double iw = e.inv_w;
         const double r0r = 0.5 * (prev[d].x + r.x), r0i = 0.5 * (prev[d].y + r.y);
         const double r1r = (r.x - prev[d].x) * iw, r1i = (r.y - prev[d].y) * iw;
-        const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
+        const double2 a0 = e.A0[d], a1 = e.A1[d];
         dh[d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
-        hh[d] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
+        hh[d] += fma(e.B0[d], fma(r0r, r0r, r0i * r0i), 2.0 * e.B1[d] * fma(r0r, r1r, r0i * r1i));
       }
       prev[d] = r;
     }
@@ -730,6 +786,12 @@ __global__ void __launch_bounds__(kRbThreads) k_relbin(const DevCfg* __restrict_
     l += dh[d] - 0.5 * hh[d];
   }
   logl[p] = valid ? l : -INFINITY;
+}
+
+// shared memory of k_relbin: the staged edges (+ the transposed coefficient blocks for PhenomD-form)
+template <int MODEL, int NDET>
+size_t relbin_smem_bytes(int nb) {
+  return sizeof(RbEdge<NDET>) * ((size_t)nb + 1) + (MODEL == 2 ? sizeof(double) * CB_SIZE * kRbThreads : 0);
 }
 
 // ======================================================================================================
@@ -1472,17 +1534,16 @@ int relbin_theta(ns_handle* h, const double* theta_dev, long long B, double* log
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  constexpr size_t kSm2 = sizeof(double) * CB_SIZE * kRbThreads;
-  static bool attr_set = false;
-  if (!attr_set) {
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    CU_CHECK(h, cudaFuncSetAttribute(k_relbin<2, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSm2));
-    attr_set = true;
-  }
-#define RB_EVAL(M, N, SM) k_relbin<M, N><<<gr, kRbThreads, SM, s>>>(h->d_cfg, h->tb, h->rb, h->d_cb, B, logl, parts)
-  if (tf2) { if (nd == 1) RB_EVAL(1, 1, 0); else if (nd == 2) RB_EVAL(1, 2, 0); else RB_EVAL(1, 3, 0); }
-  else { if (nd == 1) RB_EVAL(2, 1, kSm2); else if (nd == 2) RB_EVAL(2, 2, kSm2); else RB_EVAL(2, 3, kSm2); }
+  const int nbn = h->rb_nb;
+#define RB_EVAL(M, N)                                                                                                  \
+  do {                                                                                                                 \
+    const size_t sm_ = relbin_smem_bytes<M, N>(nbn);                                                                   \
+    if (sm_ > 200 * 1024) return fail(h, -5, "too many relative-binning bins for one CTA's shared memory");            \
+    if (sm_ > 48 * 1024) CU_CHECK(h, cudaFuncSetAttribute(k_relbin<M, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_)); \
+    k_relbin<M, N><<<gr, kRbThreads, sm_, s>>>(h->d_cfg, h->tb, h->rb, h->d_cb, B, logl, parts);                       \
+  } while (0)
+  if (tf2) { if (nd == 1) RB_EVAL(1, 1); else if (nd == 2) RB_EVAL(1, 2); else RB_EVAL(1, 3); }
+  else { if (nd == 1) RB_EVAL(2, 1); else if (nd == 2) RB_EVAL(2, 2); else RB_EVAL(2, 3); }
 #undef RB_EVAL
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
