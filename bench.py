@@ -314,6 +314,21 @@ def run_ours(args):
                                                 "wall_s_per_run": wall / len(hs)}
             for hh in hs:
                 hh.close()
+            # sequential limit: config 1 with k = 1 against the batched k = 50 (same n_live, same rule)
+            spec1, smp1, logz_true = W.config1()
+            seq = {}
+            for kdel in (50, 1):
+                smp_k = dict(smp1, n_delete=kdel)
+                hk = nsgw.Handle(spec1, smp_k, seed=1)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                nit, st = hk.run(smp1["term_kind"], smp1["term_tol"], 200000)
+                lz, le, _ = hk.finalize_evidence()
+                seq[f"k={kdel}"] = {"wall_s": time.perf_counter() - t0, "iterations": nit, "n_eval_total": st["n_eval_total"],
+                                    "logz": lz, "logz_err": le, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"]}
+                hk.close()
+            seq["logz_closed_form"] = logz_true["logz_exact"]
+            extras["config1_sequential_limit"] = seq
             # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
             spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
             h4 = nsgw.Handle(spec4, smp4, seed=1)
