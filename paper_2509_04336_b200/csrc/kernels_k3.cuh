@@ -1,0 +1,170 @@
+// kernels_k3.cuh -- K3: selection (rank), evidence scan, start points, write-back, adaptation, final evidence; FP64 peak probe
+// Part of libnsgw (one translation unit): included by nsgw.cu inside its anonymous namespace, after nsgw_device.cuh.
+// See include/nsgw.h for the contract and DESIGN.md section 5 for the design of each kernel.
+#pragma once
+
+// ======================================================================================================
+// K3: selection, evidence, replacement, adaptation
+// ======================================================================================================
+// Stable rank by counting: order[rank(i)] = i with rank(i) = #{j : l_j < l_i or (l_j == l_i and j < i)}  (R:L6).
+__global__ void k_rank(const double* __restrict__ logl, int n, int* order) {
+  __shared__ double tile[256];
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  double li = (i < n) ? logl[i] : 0.0;
+  int rank = 0;
+  for (int base = 0; base < n; base += 256) {
+    int j = base + threadIdx.x;
+    tile[threadIdx.x] = (j < n) ? logl[j] : INFINITY;
+    __syncthreads();
+    int lim = min(256, n - base);
+    for (int jj = 0; jj < lim; ++jj) {
+      double lj = tile[jj];
+      rank += (lj < li) || (lj == li && (base + jj) < i);
+    }
+    __syncthreads();
+  }
+  if (i < n) order[rank] = i;
+}
+
+__device__ __forceinline__ double logaddexp_d(double a, double b) {
+  if (a == -INFINITY) return b;
+  if (b == -INFINITY) return a;
+  double m = fmax(a, b);
+  return m + log1p(exp(-fabs(a - b)));
+}
+
+__device__ __forceinline__ void evidence_update(double li, double ni, double& logx, double& logz, double& h, double& logw) {
+  logw = logx + log(-expm1(-1.0 / ni));
+  double lw = li + logw;
+  double zn = logaddexp_d(logz, lw);
+  double hn = exp(lw - zn) * li;
+  if (logz != -INFINITY) hn += exp(logz - zn) * (h + logz);
+  hn -= zn;
+  h = hn; logz = zn; logx -= 1.0 / ni;
+}
+
+// Sequential evidence scan over the k dead points in ascending logL (eq. 3-5 with the saw-tooth live count; R:L16, L17).
+__global__ void k_evidence(DevState* st, const double* __restrict__ logl, const double* __restrict__ u, const int* __restrict__ order,
+                           int n, int k, int D, double* dead) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double logx = st->logx, logz = st->logz, h = st->h;
+  for (int i = 0; i < k; ++i) {
+    int id = order[i];
+    double logw;
+    evidence_update(logl[id], (double)(n - i), logx, logz, h, logw);
+    if (dead) {
+      double* row = dead + (size_t)i * (D + 3);
+      for (int d = 0; d < D; ++d) row[d] = u[(size_t)id * D + d];
+      row[D] = logl[id]; row[D + 1] = logw; row[D + 2] = (double)(n - i);
+    }
+  }
+  st->logx = logx; st->logz = logz; st->h = h;
+  st->lstar = logl[order[k - 1]];
+  int W = (int)floor(st->walks);
+  st->W = max(1, min(W, st->maxmcmc));
+}
+
+// Survivor array in ascending-logL order + start points (uniform survivor, Philox tag 1; R:L7).
+__global__ void k_gather_start(const DevState* __restrict__ st, const double* __restrict__ u, const double* __restrict__ logl,
+                               const int* __restrict__ order, int n, int k, int D, uint32_t k0, uint32_t k1, double* surv, double* cur_u,
+                               double* cur_l) {
+  const int m = n - k;
+  int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < m) {
+    int id = order[k + i];
+    for (int d = 0; d < D; ++d) surv[(size_t)i * D + d] = u[(size_t)id * D + d];
+  }
+  if (i < k) {
+    uint32_t w[4];
+    philox4x32_10(0u, 0u, (uint32_t)i, (1u << 24) | (uint32_t)(st->iter & 0xFFFFFF), k0, k1, w);
+    int id = order[k + __umulhi(w[0], (uint32_t)m)];
+    for (int d = 0; d < D; ++d) cur_u[(size_t)i * D + d] = u[(size_t)id * D + d];
+    cur_l[i] = logl[id];
+  }
+}
+
+__global__ void k_writeback(const int* __restrict__ order, int k, int D, const double* __restrict__ cur_u, const double* __restrict__ cur_l,
+                            double* u, double* logl) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= k) return;
+  int id = order[j];
+  for (int d = 0; d < D; ++d) u[(size_t)id * D + d] = cur_u[(size_t)j * D + d];
+  logl[id] = cur_l[j];
+}
+
+// Batch-level adaptation (R:L13-L15) and termination quantities (R:L18).  Single CTA, fixed-order reductions.
+__global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __restrict__ ne, const int* __restrict__ no, int k,
+                        const double* __restrict__ logl, int n) {
+  __shared__ long long s_a[256], s_e[256], s_o[256], s_s[256];
+  __shared__ int s_min[256], s_max[256];
+  __shared__ double s_d[256];
+  const int t = threadIdx.x;
+  long long a = 0, e = 0, o = 0, s = 0;
+  int mn = INT_MAX, mx = INT_MIN;
+  for (int j = t; j < k; j += 256) {
+    a += na[j]; e += ne[j]; o += no[j]; s += (na[j] == 0);
+    mn = min(mn, na[j]); mx = max(mx, na[j]);
+  }
+  s_a[t] = a; s_e[t] = e; s_o[t] = o; s_s[t] = s; s_min[t] = mn; s_max[t] = mx;
+  double lm = -INFINITY;
+  for (int i = t; i < n; i += 256) lm = fmax(lm, logl[i]);
+  s_d[t] = lm;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (t < w) {
+      s_a[t] += s_a[t + w]; s_e[t] += s_e[t + w]; s_o[t] += s_o[t + w]; s_s[t] += s_s[t + w];
+      s_min[t] = min(s_min[t], s_min[t + w]); s_max[t] = max(s_max[t], s_max[t + w]);
+      s_d[t] = fmax(s_d[t], s_d[t + w]);
+    }
+    __syncthreads();
+  }
+  const double lmax = s_d[0];
+  __syncthreads();
+  double acc = 0.0;
+  for (int i = t; i < n; i += 256) acc += exp(logl[i] - lmax);
+  s_d[t] = acc;
+  __syncthreads();
+  for (int w = 128; w > 0; w >>= 1) {
+    if (t < w) s_d[t] += s_d[t + w];
+    __syncthreads();
+  }
+  if (t == 0) {
+    const int W = st->W;
+    double amean = (double)s_a[0] / k;
+    double r = fmax(0.5, amean) / W;
+    double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
+    st->walks = walks;
+    st->n_eval_total += s_e[0];
+    double lse = lmax + log(s_d[0]);
+    ns_stats& o_ = st->stats;
+    o_.iteration = st->iter;
+    o_.logl_star = st->lstar; o_.logx = st->logx; o_.logz = st->logz; o_.h = st->h;
+    o_.dlogz = logaddexp_d(st->logz, lmax + st->logx) - st->logz;
+    o_.live_frac_log = lse - log((double)n) + st->logx - st->logz;
+    o_.walk_len = W; o_.pad0 = 0; o_.walks_next = walks;
+    o_.accept_mean = amean; o_.accept_min = s_min[0]; o_.accept_max = s_max[0];
+    o_.n_eval = s_e[0]; o_.n_oob = s_o[0]; o_.n_stuck = s_s[0]; o_.n_eval_total = st->n_eval_total;
+    st->iter += 1;
+  }
+}
+
+// Final evidence: adds the live points with n_i = n..1 to a copy of the accumulators (R:L17).  out: logz, h.
+__global__ void k_finalize(const DevState* __restrict__ st, const double* __restrict__ logl, const int* __restrict__ order, int n,
+                           double* out) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double logx = st->logx, logz = st->logz, h = st->h, lw;
+  for (int i = 0; i < n; ++i) evidence_update(logl[order[i]], (double)(n - i), logx, logz, h, lw);
+  out[0] = logz; out[1] = h;
+}
+
+// FP64 FMA throughput probe: 8 independent chains per thread.
+__global__ void k_dfma_probe(long long iters, double* sink) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999, c = 1e-7;
+  for (long long i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+  if (s == 123.456) sink[0] = s;
+}

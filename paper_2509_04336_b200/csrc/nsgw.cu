@@ -1,12 +1,14 @@
-// nsgw.cu -- kernels and C-ABI of libnsgw.so (see include/nsgw.h for the contract, DESIGN.md for the design).
+// nsgw.cu -- host side and C-ABI of libnsgw.so (see include/nsgw.h for the contract, DESIGN.md for the design).
 //
-// Kernels
-//   k_tables          ns_init: per-bin tables and noise-weighted data (parameter independent)
-//   k_setup           theta[B,11] -> per-particle coefficient blocks (one thread per particle)
-//   k_bins            K1: CTA per P particles, bins strided over threads, shuffle + smem reduction
-//   k_walk_gw         K2: persistent lock-step acceptance walk, CTA per P walkers, W steps in-kernel
-//   k_walk_simple     K2 for bin-less likelihoods (Gaussian toy, cube shell): one thread per walker
-//   k_rank / k_evidence / k_gather_start / k_writeback / k_adapt   K3: select, evidence scan, replacement, adaptation
+// One translation unit; the kernels live in headers included below (inside the anonymous namespace):
+//   nsgw_device.cuh      Philox, prior transforms, table-driven sin/cos / exp / atan, detector response, per-particle set-up,
+//                        per-bin PhenomD-form evaluation
+//   kernels_k1.cuh       k_tables / k_i73 / k_math_tables / k_draw_live / k_prior_transform (ns_init), k_setup, k_bins (CTA per
+//                        particle pair), k_bins_lp + k_finish (lane per particle), k_waveform
+//   kernels_relbin.cuh   k_rb_delta / k_rb_select / k_rb_summary / k_relbin (relative binning, R:L24)
+//   kernels_walk.cuh     de_propose, k_walk_simple, k_walk_gw (speculative chunks; exact or relative-binning likelihood)
+//   kernels_k3.cuh       k_rank / k_evidence / k_gather_start / k_writeback / k_adapt / k_finalize, k_dfma_probe
+// This file: ns_handle, launch geometry, argument checks and the extern "C" entry points.
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -40,1282 +42,11 @@ struct DevState {
   ns_stats stats;
 };
 
-// ======================================================================================================
-// ns_init kernels
-// ======================================================================================================
-__global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const double* __restrict__ psd, double2* t01, double2* t23,
-                         double2* t45, double2* t67, double* tf, double* tf34, double2* wd, double* ws) {
-  const int nf = cfg->n_freq, nd = cfg->n_det;
-  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nf; k += gridDim.x * blockDim.x) {
-    double f = cfg->f_min + k * cfg->df;
-    double x = cbrt(f), y = 1.0 / x, L = log(f);
-    double y2 = y * y, y3 = y2 * y;
-    t01[k] = make_double2(y3 * y2, y3);
-    t23[k] = make_double2(y2, y);
-    t45[k] = make_double2(L, x);
-    t67[k] = make_double2(x * L, x * x);
-    tf[k] = f; tf34[k] = sqrt(sqrt(f * f * f));
-    double a76 = 1.0 / (f * sqrt(x));      // f^-7/6
-    for (int d = 0; d < nd; ++d) {
-      double S = psd[(size_t)d * nf + k];
-      double w = 4.0 * cfg->df / S;
-      wd[(size_t)d * nf + k] = make_double2(w * a76 * strain[((size_t)d * nf + k) * 2], w * a76 * strain[((size_t)d * nf + k) * 2 + 1]);
-      ws[(size_t)d * nf + k] = w * a76 * a76;
-    }
-  }
-}
+#include "kernels_k1.cuh"
+#include "kernels_relbin.cuh"
+#include "kernels_walk.cuh"
+#include "kernels_k3.cuh"
 
-__global__ void k_math_tables(MathTables* mt) { build_math_tables(mt, threadIdx.x, blockDim.x); }
-
-// I_{7/3} per detector: deterministic single-CTA tree sum.
-__global__ void k_i73(DevCfg* cfg, const double* __restrict__ ws) {
-  __shared__ double sh[256];
-  const int nf = cfg->n_freq;
-  for (int d = 0; d < cfg->n_det; ++d) {
-    double acc = 0.0;
-    for (int k = threadIdx.x; k < nf; k += 256) acc += ws[(size_t)d * nf + k];
-    sh[threadIdx.x] = acc;
-    __syncthreads();
-    for (int s = 128; s > 0; s >>= 1) {
-      if (threadIdx.x < s) sh[threadIdx.x] += sh[threadIdx.x + s];
-      __syncthreads();
-    }
-    if (threadIdx.x == 0) cfg->i73[d] = sh[0];
-    __syncthreads();
-  }
-}
-
-__global__ void k_draw_live(int ndim, long long n, uint32_t k0, uint32_t k1, double* u) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= n) return;
-  for (int d = 0; d < ndim; d += 2) {
-    uint32_t w[4];
-    philox4x32_10((uint32_t)(d / 2), 0u, (uint32_t)i, 2u << 24, k0, k1, w);
-    u[i * ndim + d] = u01(w[0], w[1]);
-    if (d + 1 < ndim) u[i * ndim + d + 1] = u01(w[2], w[3]);
-  }
-}
-
-__global__ void k_prior_transform(const DevCfg* __restrict__ cfg, const double* __restrict__ u, long long B, double* theta) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  const int D = cfg->ndim;
-  if (i >= B * D) return;
-  int d = (int)(i % D);
-  theta[i] = prior_transform_dim(cfg->prior_kind[d], cfg->prior_lo[d], cfg->prior_hi[d], u[i]);
-}
-
-// ======================================================================================================
-// K1: set-up + bin loop
-// ======================================================================================================
-template <int MODEL>
-__global__ void k_setup(const DevCfg* __restrict__ cfg, const double* __restrict__ theta, long long B, double* cbs) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= B) return;
-  double th[11];
-#pragma unroll
-  for (int d = 0; d < 11; ++d) th[d] = theta[i * 11 + d];
-  setup_particle<MODEL>(*cfg, th, cbs + i * CB_SIZE);
-}
-
-// Number of per-thread partial sums of one particle: X0 = sum conj(wd_0) amp E (complex; detector 0 carries no phasor, its
-// C_0 is applied once after the reduction), dh_d for d >= 1, and for PhenomD-form hh_d = sum amp^2 ws_d for every detector.
-template <int MODEL, int NDET>
-struct AccLayout {
-  static constexpr int ND1 = NDET - 1;
-  static constexpr int kDh = 2;                          // dh_d at kDh + d - 1 (d >= 1)
-  static constexpr int kHh = 2 + ND1;                    // hh_d at kHh + d (PhenomD-form only)
-  static constexpr int N = 2 + ND1 + (MODEL == 2 ? NDET : 0);
-};
-
-// Start phasors of the detectors d >= 1: for particle p, thread t (bin t of the first sweep)
-//   R = (Cr + i Ci) * exp(i * dtq * f_t)  [dtq: quarter turns per Hz relative to detector 0],
-// built as lane-table x warp-table to keep it to one sincos per entry.
-// tabL[(p*ND1+d-1)*32 + lane] = exp(i dtq df lane); tabW[(p*ND1+d-1)*NW + w] = C * exp(i dtq (f_min + 32 w df)).
-template <int NDET, int NT>
-__device__ __forceinline__ void build_phasor_tables(const DevCfg& cfg, const double* cbs /*smem [np][CB_SIZE]*/, int np, double2* tabL,
-                                                    double2* tabW, double2* step) {
-  constexpr int NW = NT / 32, ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
-  const int NE = np * ND1 * (32 + NW + 1);
-  for (int e = threadIdx.x; e < NE; e += NT) {
-    int pd = e / (32 + NW + 1), j = e % (32 + NW + 1);
-    int p = pd / ND1s, d = pd % ND1s + 1;
-    const double* cb = cbs + p * CB_SIZE;
-    double dtq = cb[CB_DET + 4 * d + 2];
-    double s, c;
-    if (j < 32) {
-      sincos_qt(dtq * (cfg.df * j), s, c);
-      tabL[pd * 32 + j] = make_double2(c, s);
-    } else if (j < 32 + NW) {
-      int w = j - 32;
-      sincos_qt(dtq * (cfg.f_min + cfg.df * (32 * w)), s, c);
-      double cr = cb[CB_DET + 4 * d], ci = cb[CB_DET + 4 * d + 1];
-      tabW[pd * NW + w] = make_double2(cr * c - ci * s, cr * s + ci * c);
-    } else {
-      sincos_qt(dtq * (cfg.df * NT), s, c);
-      step[pd] = make_double2(c, s);
-    }
-  }
-}
-
-// Bin loop for P particles held by this CTA: thread t handles bins t, t + NT, ...; the table values of a bin are loaded once
-// and used for the P particles.  Per (particle, bin): common phase (9 FMA), one sincos, 4 FMA for detector 0, and for each
-// further detector a complex product with its phasor, 2 FMA and the phasor advance.
-template <int MODEL, int NDET, int P, int NT>
-__device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                         const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
-                                         const int* slot /*smem [P]: coefficient-block / phasor-table slot of particle p*/,
-                                         double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
-  using AL = AccLayout<MODEL, NDET>;
-  constexpr int NW = NT / 32, ND1 = NDET - 1;
-  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-  double2 R[P][ND1 > 0 ? ND1 : 1], St[P][ND1 > 0 ? ND1 : 1];
-  double a[P][MODEL == 1 ? 10 : 1];
-  const double* cbp[P];
-  bool any = false;
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    const int sl = slot[p];
-    cbp[p] = cbs + sl * CB_SIZE;
-    any = any || active[p];
-#pragma unroll
-    for (int i = 0; i < AL::N; ++i) acc[p][i] = 0.0;
-#pragma unroll
-    for (int d = 0; d < ND1; ++d) {
-      double2 u = tabL[(sl * ND1 + d) * 32 + lane], v = tabW[(sl * ND1 + d) * NW + wrp];
-      R[p][d] = make_double2(u.x * v.x - u.y * v.y, u.x * v.y + u.y * v.x);
-      St[p][d] = step[sl * ND1 + d];
-    }
-    if (MODEL == 1) {
-#pragma unroll
-      for (int i = 0; i < 10; ++i) a[p][i] = 64.0 * cbp[p][CB_PH + i];   // quarter turns -> 1/256 turn (exact)
-    }
-  }
-  if (!any) return;   // block-uniform: nothing to evaluate (all proposals of this CTA were out of bounds)
-  const int nf = cfg.n_freq;
-  // shared tail of a (particle, bin): E = amp exp(-i Phi) and the accumulations
-  auto tail = [&](int p, double q, double amp, const double2 (&w)[NDET], const double (&wsv)[NDET]) {
-    double sn, cs;
-    sincos_lut(q, mt, sn, cs);
-    if (MODEL == 2) { sn *= amp; cs *= amp; }
-    // E = cs - i sn;  X0 += conj(wd_0) E
-    acc[p][0] = fma(w[0].x, cs, acc[p][0]);
-    acc[p][1] = fma(-w[0].x, sn, acc[p][1]);
-    acc[p][0] = fma(-w[0].y, sn, acc[p][0]);
-    acc[p][1] = fma(-w[0].y, cs, acc[p][1]);
-    if (MODEL == 2) {
-      const double a2 = amp * amp;
-#pragma unroll
-      for (int d = 0; d < NDET; ++d) acc[p][AL::kHh + d] = fma(a2, wsv[d], acc[p][AL::kHh + d]);
-    }
-#pragma unroll
-    for (int d = 0; d < ND1; ++d) {
-      const double rx = R[p][d].x, ry = R[p][d].y;
-      // G = E R_d;  dh_d += Re(conj(wd_d) G)
-      const double gr = fma(cs, rx, sn * ry);
-      const double gi = fma(cs, ry, -(sn * rx));
-      acc[p][AL::kDh + d] = fma(w[d + 1].x, gr, acc[p][AL::kDh + d]);
-      acc[p][AL::kDh + d] = fma(w[d + 1].y, gi, acc[p][AL::kDh + d]);
-      // advance the detector phasor by one sweep
-      R[p][d].x = fma(rx, St[p][d].x, -(ry * St[p][d].y));
-      R[p][d].y = fma(rx, St[p][d].y, ry * St[p][d].x);
-    }
-  };
-  // PhenomD-form: from the first sweep whose bins all lie in the merger-ringdown region of BOTH phase and amplitude for every
-  // particle of this group (about 80 % of the band), a branch-free loop with that region's 11 coefficients in registers.
-  int k_mr = nf;   // first bin of the specialised loop (multiple of NT)
-  if (MODEL == 2) {
-    double fs = 0.0;
-#pragma unroll
-    for (int p = 0; p < P; ++p) fs = fmax(fs, fmax(cbp[p][CB_FP2], cbp[p][CB_FA2]));
-    const double ks = (fs - cfg.f_min) / cfg.df + 2.0;          // two bins of margin against rounding of f_k
-    if (ks < (double)nf) k_mr = ((int)fmax(ks, 0.0) + NT - 1) / NT * NT;
-  }
-  const int k_gen = (MODEL == 2) ? min(nf, k_mr) : nf;
-  // PhenomD-form: exp(-gamma2 (f - f_RD)/w) along a thread's bins is a geometric sequence (ratio exp(c3 NT df)): one exp_tab per
-  // thread and particle here, one multiplication per bin in both loops below (<= 32 ulp of accumulated rounding).  The sequence
-  // starts at the thread's first bin whatever the loop split, so a particle's logL does not depend on its group partner.
-  double ex[P], exr[P];
-#pragma unroll
-  for (int p = 0; p < P; ++p) {
-    ex[p] = (MODEL == 2) ? exp_tab(cbp[p][CB_AM + 3] * (cfg.f_min + cfg.df * tid - cbp[p][CB_AM]), mt) : 1.0;
-    exr[p] = (MODEL == 2) ? exp_tab(cbp[p][CB_AM + 3] * (cfg.df * NT), mt) : 1.0;
-  }
-  for (int k = tid; k < k_gen; k += NT) {
-    const BinBasis b = make_basis(tb, k, MODEL == 2);
-    double2 w[NDET];
-    double wsv[NDET];
-#pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      w[d] = __ldg(tb.wd[d] + k);
-      wsv[d] = (MODEL == 2) ? __ldg(tb.ws[d] + k) : 0.0;
-    }
-#pragma unroll
-    for (int p = 0; p < P; ++p) {
-      double q, amp = 1.0;
-      if (MODEL == 1) q = phase_pn_qt(a[p], b);
-      else { phenom_bin(cbp[p], b, mt, ex[p], q, amp); q *= 64.0; ex[p] *= exr[p]; }
-      tail(p, q, amp, w, wsv);
-    }
-  }
-  if (MODEL == 2 && k_mr < nf) {
-    double pm[P][7], am[P][4];
-#pragma unroll
-    for (int p = 0; p < P; ++p) {
-#pragma unroll
-      for (int i = 0; i < 5; ++i) pm[p][i] = 64.0 * cbp[p][CB_PM + i];     // phase in 1/256 turn (exact scaling)
-      pm[p][5] = cbp[p][CB_PM + 5]; pm[p][6] = cbp[p][CB_PM + 6];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) am[p][i] = cbp[p][CB_AM + i];
-    }
-#pragma unroll 2
-    for (int k = k_mr + tid; k < nf; k += NT) {
-      const double f = __ldg(tb.f + k), f34 = __ldg(tb.f34 + k);
-      const double y3 = __ldg(tb.t01 + k).y;       // 1/f
-      double2 w[NDET];
-      double wsv[NDET];
-#pragma unroll
-      for (int d = 0; d < NDET; ++d) { w[d] = __ldg(tb.wd[d] + k); wsv[d] = __ldg(tb.ws[d] + k); }
-#pragma unroll
-      for (int p = 0; p < P; ++p) {
-        double q = fma(pm[p][1], f, pm[p][0]);
-        q = fma(pm[p][2], y3, q);
-        q = fma(pm[p][3], f34, q);
-        q = fma(pm[p][4], atan_tab((f - pm[p][5]) * pm[p][6], mt), q);
-        const double fx = f - am[p][0];
-        const double amp = am[p][1] * rcp_nr(fma(fx, fx, am[p][2])) * ex[p];
-        ex[p] *= exr[p];
-        tail(p, q, amp, w, wsv);
-      }
-    }
-  }
-}
-
-// Deterministic block reduction of NV values per thread: warp shuffle tree, then fixed-order sum over warps by thread 0..NV-1.
-template <int NV, int NT>
-__device__ __forceinline__ void block_reduce(double (&v)[NV], double* red /*smem [NT/32][NV]*/, double* out /*smem [NV]*/) {
-  constexpr int NW = NT / 32;
-#pragma unroll
-  for (int i = 0; i < NV; ++i) {
-    double x = v[i];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-    v[i] = x;
-  }
-  if ((threadIdx.x & 31) == 0) {
-#pragma unroll
-    for (int i = 0; i < NV; ++i) red[(threadIdx.x >> 5) * NV + i] = v[i];
-  }
-  __syncthreads();
-  if (threadIdx.x < NV) {
-    double s = 0.0;
-#pragma unroll
-    for (int w = 0; w < NW; ++w) s += red[w * NV + threadIdx.x];
-    out[threadIdx.x] = s;
-  }
-  __syncthreads();
-}
-
-// Finishes logL of one particle from its reduced sums (AccLayout order).
-template <int MODEL, int NDET>
-__device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* cb, const double* sums, double* parts) {
-  using AL = AccLayout<MODEL, NDET>;
-  if (cb[CB_VALID] == 0.0) {
-    if (parts) for (int d = 0; d < 2 * NDET; ++d) parts[d] = nan("");
-    return -INFINITY;
-  }
-  double logl = 0.0;
-#pragma unroll
-  for (int d = 0; d < NDET; ++d) {
-    double dh = (d == 0) ? fma(cb[CB_DET], sums[0], -(cb[CB_DET + 1] * sums[1])) : sums[AL::kDh + d - 1];
-    double hh = (MODEL == 1) ? cb[CB_DET + 4 * d + 3] * cfg.i73[d] : cb[CB_DET + 4 * d + 3] * sums[AL::kHh + d];
-    if (parts) { parts[2 * d] = dh; parts[2 * d + 1] = hh; }
-    logl += dh - 0.5 * hh;
-  }
-  return logl;
-}
-
-template <int MODEL, int NDET, int P>
-__global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
-                                                           long long B, double* logl, double* parts) {
-  using AL = AccLayout<MODEL, NDET>;
-  constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
-  __shared__ __align__(16) double cbs[P * CB_SIZE];
-  __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
-  __shared__ double red[NW * NV], out[NV];
-  __shared__ MathTables mtab;
-  __shared__ bool active[P];
-  __shared__ int slot[P];
-  const DevCfg& cfg = *cfgp;
-  const long long p0 = (long long)blockIdx.x * P;
-  load_math_tables(&mtab, tb.mt, threadIdx.x, NT);
-  if (threadIdx.x < P) slot[threadIdx.x] = threadIdx.x;
-  for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
-    long long p = p0 + e / CB_SIZE;
-    cbs[e] = (p < B) ? cbs_g[p * CB_SIZE + e % CB_SIZE] : 0.0;
-  }
-  __syncthreads();
-  if (threadIdx.x < P) active[threadIdx.x] = cbs[threadIdx.x * CB_SIZE + CB_VALID] != 0.0;
-  build_phasor_tables<NDET, NT>(cfg, cbs, P, tabL, tabW, step);
-  __syncthreads();
-  double acc[P][AL::N];
-  bin_loop<MODEL, NDET, P, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, acc);
-  double v[NV];
-#pragma unroll
-  for (int p = 0; p < P; ++p)
-#pragma unroll
-    for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
-  block_reduce<NV, NT>(v, red, out);
-  if (threadIdx.x < P && p0 + threadIdx.x < B) {
-    int p = threadIdx.x;
-    logl[p0 + p] = finish_logl<MODEL, NDET>(cfg, cbs + p * CB_SIZE, out + p * AL::N, parts ? parts + (p0 + p) * 2 * NDET : nullptr);
-  }
-}
-
-// ------------------------------------------------------------------------------------------------------
-// K1 for large batches, lane = particle: every thread owns ONE particle (phase coefficients, detector phasors and partial
-// sums in registers for the whole task), and the CTA walks a range of KR bins whose table values are staged once in shared
-// memory and read with warp-uniform (broadcast) LDS.  No per-bin global traffic, no cross-thread reduction, no phasor
-// tables: a task costs each thread 2 sincos per extra detector plus KR x (the same per-bin arithmetic as bin_loop).
-// Task = (group of NT PP particles, range of kr bins); partial[n_ranges][N][B] is summed in range order by k_finish.
-// Built for TaylorF2 (no per-particle branches in the bin loop; PhenomD-form's piecewise regions would diverge across lanes).
-// ------------------------------------------------------------------------------------------------------
-template <int NDET, int KR>
-struct LpSmem {
-  double2 t01[KR], t23[KR], t45[KR], t67[KR];
-  double2 wd[NDET][KR];
-  double f[KR];
-};
-
-template <int NDET, int NT, int KR, int PP, int UNR, int OCC>
-__global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
-                                                     long long B, int kr /*bins per range, <= KR, multiple of UNR*/, int nranges,
-                                                     long long ntasks, double* __restrict__ partial) {
-  using AL = AccLayout<1, NDET>;
-  constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
-  __shared__ __align__(16) LpSmem<NDET, KR> sm;
-  __shared__ MathTables mtab;
-  const DevCfg& cfg = *cfgp;
-  const int tid = threadIdx.x;
-  const int nf = cfg.n_freq;
-  load_math_tables(&mtab, tb.mt, tid, NT);
-  for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
-    const long long grp = task / nranges;
-    const int rng = (int)(task % nranges);
-    const int k0 = rng * kr;
-    const int nk = min(kr, nf - k0);
-    const int nk2 = (nk + UNR - 1) / UNR * UNR;   // padded with zero-weight bins
-    __syncthreads();   // readers of the previous tile are done
-    for (int i = tid; i < nk2; i += NT) {
-      const bool ok = i < nk;
-      const int k = k0 + (ok ? i : nk - 1);
-      sm.t01[i] = __ldg(tb.t01 + k); sm.t23[i] = __ldg(tb.t23 + k); sm.t45[i] = __ldg(tb.t45 + k); sm.t67[i] = __ldg(tb.t67 + k);
-      sm.f[i] = __ldg(tb.f + k);
-#pragma unroll
-      for (int d = 0; d < NDET; ++d) sm.wd[d][i] = ok ? __ldg(tb.wd[d] + k) : make_double2(0.0, 0.0);
-    }
-    // ---- this thread's PP particles (a warp-wide load of the table values of a bin then serves 32 PP particle-bins)
-    double a[PP][10];
-    double2 R[PP][ND1s], St[PP][ND1s];
-    double acc[PP][AL::N];
-#pragma unroll
-    for (int j = 0; j < PP; ++j) {
-      const long long p = (grp * PP + j) * NT + tid;
-      const bool have = p < B;
-      const double* cb = cbs_g + (have ? p : 0) * CB_SIZE;
-#pragma unroll
-      for (int i = 0; i < 10; ++i) a[j][i] = have ? 64.0 * __ldg(cb + CB_PH + i) : 0.0;   // quarter turns -> 1/256 turn (exact)
-#pragma unroll
-      for (int d = 0; d < ND1; ++d) {
-        const double cr = have ? __ldg(cb + CB_DET + 4 * (d + 1)) : 0.0, ci = have ? __ldg(cb + CB_DET + 4 * (d + 1) + 1) : 0.0;
-        const double dtq = have ? __ldg(cb + CB_DET + 4 * (d + 1) + 2) : 0.0;
-        double sn, cs;
-        sincos_qt(dtq * (cfg.f_min + cfg.df * k0), sn, cs);
-        R[j][d] = make_double2(cr * cs - ci * sn, cr * sn + ci * cs);
-        sincos_qt(dtq * cfg.df, sn, cs);
-        St[j][d] = make_double2(cs, sn);
-      }
-#pragma unroll
-      for (int i = 0; i < AL::N; ++i) acc[j][i] = 0.0;
-    }
-    __syncthreads();
-    // Detectors d >= 1: sum_k conj(wd_k) E_k R_k with R_k = R_0 rho^k is evaluated as R_0 * Horner(rho) over the tile's bins in
-    // DESCENDING order, S <- S rho + conj(wd_k) E_k (8 FP64 instructions per bin instead of 10 for product + accumulate + phasor
-    // advance).  The zero-weight padding bins come first and leave S = 0.
-    double2 S[PP][ND1s];
-#pragma unroll
-    for (int j = 0; j < PP; ++j)
-#pragma unroll
-      for (int d = 0; d < ND1s; ++d) S[j][d] = make_double2(0.0, 0.0);
-#pragma unroll UNR
-    for (int kk = nk2 - 1; kk >= 0; --kk) {
-      BinBasis b;
-      { const double2 v = sm.t01[kk]; b.y5 = v.x; b.y3 = v.y; }
-      { const double2 v = sm.t23[kk]; b.y2 = v.x; b.y = v.y; }
-      { const double2 v = sm.t45[kk]; b.L = v.x; b.x = v.y; }
-      { const double2 v = sm.t67[kk]; b.xL = v.x; b.x2 = v.y; }
-      b.f = sm.f[kk]; b.f34 = 0.0;
-      double2 w[NDET];
-#pragma unroll
-      for (int d = 0; d < NDET; ++d) w[d] = sm.wd[d][kk];
-#pragma unroll
-      for (int j = 0; j < PP; ++j) {
-        const double q = phase_pn_qt(a[j], b);
-        double sn, cs;
-        sincos_lut(q, &mtab, sn, cs);
-        acc[j][0] = fma(w[0].x, cs, acc[j][0]);
-        acc[j][1] = fma(-w[0].x, sn, acc[j][1]);
-        acc[j][0] = fma(-w[0].y, sn, acc[j][0]);
-        acc[j][1] = fma(-w[0].y, cs, acc[j][1]);
-#pragma unroll
-        for (int d = 0; d < ND1; ++d) {
-          const double ax = fma(w[d + 1].x, cs, -(w[d + 1].y * sn));      // conj(wd) E, E = cs - i sn
-          const double ay = -fma(w[d + 1].x, sn, w[d + 1].y * cs);
-          const double sx = S[j][d].x, sy = S[j][d].y;
-          S[j][d].x = fma(sx, St[j][d].x, fma(-sy, St[j][d].y, ax));
-          S[j][d].y = fma(sx, St[j][d].y, fma(sy, St[j][d].x, ay));
-        }
-      }
-    }
-#pragma unroll
-    for (int j = 0; j < PP; ++j)
-#pragma unroll
-      for (int d = 0; d < ND1; ++d) acc[j][AL::kDh + d] = fma(R[j][d].x, S[j][d].x, -(R[j][d].y * S[j][d].y));   // Re(R_0 S)
-#pragma unroll
-    for (int j = 0; j < PP; ++j) {
-      const long long p = (grp * PP + j) * NT + tid;
-      if (p < B) {
-#pragma unroll
-        for (int i = 0; i < AL::N; ++i) partial[((long long)rng * AL::N + i) * B + p] = acc[j][i];   // [range][N][B]: coalesced
-      }
-    }
-  }
-}
-
-// Adds the per-range partial sums in range order and finishes logL.
-template <int MODEL, int NDET>
-__global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restrict__ cbs_g, const double* __restrict__ partial, int nchunks,
-                         long long B, double* logl, double* parts) {
-  using AL = AccLayout<MODEL, NDET>;
-  long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (p >= B) return;
-  double sums[AL::N];
-#pragma unroll
-  for (int i = 0; i < AL::N; ++i) sums[i] = 0.0;
-  for (int c = 0; c < nchunks; ++c)
-#pragma unroll
-    for (int i = 0; i < AL::N; ++i) sums[i] += partial[((long long)c * AL::N + i) * B + p];
-  logl[p] = finish_logl<MODEL, NDET>(*cfgp, cbs_g + p * CB_SIZE, sums, parts ? parts + p * 2 * NDET : nullptr);
-}
-
-// Detector-frame waveform of one theta on the grid (for injections): out[n_det][n_freq][2].
-template <int MODEL>
-__global__ void k_waveform(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ theta, double* out) {
-  __shared__ double cb[CB_SIZE];
-  __shared__ MathTables mtab;
-  const DevCfg& cfg = *cfgp;
-  load_math_tables(&mtab, tb.mt, threadIdx.x, blockDim.x);
-  if (threadIdx.x == 0) {
-    double th[11];
-    for (int d = 0; d < 11; ++d) th[d] = theta[d];
-    setup_particle<MODEL>(cfg, th, cb);
-  }
-  __syncthreads();
-  const int nf = cfg.n_freq;
-  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < nf; k += gridDim.x * blockDim.x) {
-    BinBasis b = make_basis(tb, k, MODEL == 2);
-    double q, amp = 1.0;
-    if (MODEL == 1) q = phase_pn_qt(cb + CB_PH, b);
-    else phenom_bin(cb, b, &mtab, exp_tab(cb[CB_AM + 3] * (b.f - cb[CB_AM]), &mtab), q, amp);
-    double a76 = b.y3 * sqrt(b.y);   // f^-7/6
-    for (int d = 0; d < cfg.n_det; ++d) {
-      double s, c;
-      sincos_qt(q - cb[CB_DET + 4 * d + 2] * b.f, s, c);   // Phi_det = Phi_c + 2 pi f dt
-      double cr = cb[CB_DET + 4 * d] * amp * a76, ci = cb[CB_DET + 4 * d + 1] * amp * a76;
-      bool ok = cb[CB_VALID] != 0.0;
-      out[((size_t)d * nf + k) * 2] = ok ? cr * c + ci * s : nan("");
-      out[((size_t)d * nf + k) * 2 + 1] = ok ? ci * c - cr * s : nan("");
-    }
-  }
-}
-
-// ======================================================================================================
-// Relative binning (heterodyned likelihood; DESIGN.md R:L24): summary data about a fiducial theta0 on N_b
-// coarse bins, then per evaluation the waveform at the N_b + 1 bin edges only.
-// ======================================================================================================
-struct RbDev {
-  const int* edge;        // [nb + 1] grid indices of the bin edges
-  const double2* A0;      // [n_det][nb]  sum wd conj(g0)              (g = h f^{7/6}: the f^{-7/6} of the amplitude lives in wd, ws)
-  const double2* A1;      // [n_det][nb]  sum wd conj(g0) (f - f_m)
-  const double* B0;       // [n_det][nb]  sum ws |g0|^2
-  const double* B1;       // [n_det][nb]  sum ws |g0|^2 (f - f_m)
-  const double2* ig0;     // [n_det][nb + 1]  1 / g0 at the edges
-  const double* inv_w;    // [nb]  1 / (f_hi - f_lo)
-  int nb;
-};
-
-// g_d(f_k) = amp C_d exp(-i Phi_d) for every detector at grid bin k (Phi_d = common phase - relative delay; the same pieces as
-// the bin loops, with a direct sincos per detector because the edges are not equally spaced).
-template <int MODEL, int NDET, class CB>
-__device__ __forceinline__ void gw_g_at(const CB& cb, const Tables& tb, int k, const MathTables* mt, double2 (&g)[NDET]) {
-  const BinBasis b = make_basis(tb, k, MODEL == 2);
-  double q, amp = 1.0;
-  if (MODEL == 1) {
-    q = fma(cb(CB_PH + 0), b.y5, cb(CB_PH + 4));
-    q = fma(cb(CB_PH + 1), b.y3, q);
-    q = fma(cb(CB_PH + 2), b.y2, q);
-    q = fma(cb(CB_PH + 3), b.y, q);
-    q = fma(cb(CB_PH + 5), b.L, q);
-    q = fma(cb(CB_PH + 6), b.x, q);
-    q = fma(cb(CB_PH + 7), b.xL, q);
-    q = fma(cb(CB_PH + 8), b.x2, q);
-    q = fma(cb(CB_PH + 9), b.f, q);
-  } else {
-    phenom_bin_t(cb, b, mt, exp_tab(cb(CB_AM + 3) * (b.f - cb(CB_AM + 0)), mt), q, amp);
-  }
-#pragma unroll
-  for (int d = 0; d < NDET; ++d) {
-    double sn, cs;
-    sincos_lut(64.0 * fma(-cb(CB_DET + 4 * d + 2), b.f, q), mt, sn, cs);
-    const double cr = cb(CB_DET + 4 * d), ci = cb(CB_DET + 4 * d + 1);
-    g[d] = make_double2(amp * fma(cr, cs, ci * sn), amp * fma(ci, cs, -(cr * sn)));
-  }
-}
-
-// Delta(f_k) of reading L24, one thread per grid bin.
-__global__ void k_rb_delta(const DevCfg* __restrict__ cfg, double chi, double* delta) {
-  const int nf = cfg->n_freq;
-  const int k = blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= nf) return;
-  const double f = cfg->f_min + k * cfg->df, f_lo = cfg->f_min, f_hi = cfg->f_min + (nf - 1) * cfg->df;
-  const double g[5] = {-5.0 / 3.0, -2.0 / 3.0, 1.0, 5.0 / 3.0, 7.0 / 3.0};
-  double s = 0.0;
-  for (int i = 0; i < 5; ++i) s += (g[i] < 0.0) ? -pow(f / f_lo, g[i]) : pow(f / f_hi, g[i]);
-  delta[k] = 2.0 * kPi * chi * s;
-}
-
-// Bin edges equally spaced in Delta (sequential, as the reading states it; N_f steps in total).  out[0] = number of bins.
-__global__ void k_rb_select(const DevCfg* __restrict__ cfg, const double* __restrict__ delta, double eps, int cap, int* nb_out, int* edge) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  const int nf = cfg->n_freq;
-  const double d0 = delta[0], dtot = delta[nf - 1] - d0;
-  const double want = floor(dtot / eps);
-  if (!(want <= 4.0 * nf)) { *nb_out = -1; return; }     // eps far below what the grid resolves
-  const int nb_req = max(1, (int)want);
-  int n = 0, k = 0;
-  edge[n++] = 0;
-  for (int i = 1; i < nb_req && n < cap - 1; ++i) {
-    const double target = i * (dtot / nb_req);
-    while (k < nf - 1 && delta[k] - d0 < target) ++k;
-    if (k > edge[n - 1] && k < nf - 1) edge[n++] = k;
-  }
-  edge[n++] = nf - 1;
-  *nb_out = n - 1;
-}
-
-// Summary data: CTA b sums grid bins [e_b, e_b+1) (the last one up to and including e_nb) for every detector; fixed-order
-// reduction.  Also 1/g0 at the edges and 1/(bin width).
-template <int MODEL, int NDET>
-__global__ void __launch_bounds__(128) k_rb_summary(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cb0_g,
-                                                    const int* __restrict__ edge, int nb, double2* A0, double2* A1, double* B0, double* B1,
-                                                    double2* ig0, double* inv_w) {
-  constexpr int NT = 128, NW = NT / 32, NV = 6 * NDET;
-  __shared__ MathTables mtab;
-  __shared__ double cb0[CB_SIZE];
-  __shared__ double red[NW * NV], out[NV];
-  const int tid = threadIdx.x, b = blockIdx.x;
-  load_math_tables(&mtab, tb.mt, tid, NT);
-  for (int i = tid; i < CB_SIZE; i += NT) cb0[i] = cb0_g[i];
-  __syncthreads();
-  const CbPtr cb{cb0};
-  const int k_lo = edge[b], k_hi = (b == nb - 1) ? edge[b + 1] + 1 : edge[b + 1];
-  const double f_lo = __ldg(tb.f + edge[b]), f_hi = __ldg(tb.f + edge[b + 1]);
-  const double fm = 0.5 * (f_lo + f_hi);
-  double v[NV];
-#pragma unroll
-  for (int i = 0; i < NV; ++i) v[i] = 0.0;
-  for (int k = k_lo + tid; k < k_hi; k += NT) {
-    double2 g[NDET];
-    gw_g_at<MODEL, NDET>(cb, tb, k, &mtab, g);
-    const double df_ = __ldg(tb.f + k) - fm;
-#pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      const double2 w = __ldg(tb.wd[d] + k);
-      // wd conj(g0)
-      const double zr = fma(w.x, g[d].x, w.y * g[d].y), zi = fma(w.y, g[d].x, -(w.x * g[d].y));
-      const double h2 = __ldg(tb.ws[d] + k) * fma(g[d].x, g[d].x, g[d].y * g[d].y);
-      v[6 * d + 0] += zr; v[6 * d + 1] += zi;
-      v[6 * d + 2] = fma(zr, df_, v[6 * d + 2]); v[6 * d + 3] = fma(zi, df_, v[6 * d + 3]);
-      v[6 * d + 4] += h2; v[6 * d + 5] = fma(h2, df_, v[6 * d + 5]);
-    }
-  }
-  block_reduce<NV, NT>(v, red, out);
-  if (tid < NDET) {
-    const int d = tid;
-    A0[(size_t)d * nb + b] = make_double2(out[6 * d + 0], out[6 * d + 1]);
-    A1[(size_t)d * nb + b] = make_double2(out[6 * d + 2], out[6 * d + 3]);
-    B0[(size_t)d * nb + b] = out[6 * d + 4];
-    B1[(size_t)d * nb + b] = out[6 * d + 5];
-  }
-  if (tid == 32) inv_w[b] = 1.0 / (f_hi - f_lo);
-  if (tid == 64 || (tid == 96 && b == nb - 1)) {
-    const int i = (tid == 64) ? b : nb;
-    double2 g[NDET];
-    gw_g_at<MODEL, NDET>(cb, tb, edge[i], &mtab, g);
-#pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      const double den = 1.0 / fma(g[d].x, g[d].x, g[d].y * g[d].y);
-      ig0[(size_t)d * (nb + 1) + i] = make_double2(g[d].x * den, -g[d].y * den);
-    }
-  }
-}
-
-// Evaluation: one thread per particle, loop over the N_b + 1 edges (all lanes at the same edge).  The per-edge data -- the ten
-// basis values, f^3/4, 1/g0 per detector -- and the per-bin summary data are staged once per CTA in shared memory (18 + 8 n_det
-// and 1 + 6 n_det doubles per edge / bin) and read with warp-uniform LDS; ratio r = g/g0 at the edge, then the bin between the
-// previous edge and this one.
-constexpr int kRbThreads = 128;
-
-template <int NDET>
-struct RbEdge {           // one edge (and the bin that ends at it)
-  double y5, y3, y2, y, L, x, xL, x2, f, f34;
-  double2 ig0[NDET];      // 1 / g0 at the edge
-  double2 A0[NDET], A1[NDET];
-  double B0[NDET], B1[NDET];
-  double inv_w;
-  double pad;
-};
-
-template <int MODEL, int NDET, class CB>
-__device__ __forceinline__ void gw_g_edge(const CB& cb, const RbEdge<NDET>& e, const MathTables* mt, double2 (&g)[NDET]) {
-  BinBasis b;
-  b.y5 = e.y5; b.y3 = e.y3; b.y2 = e.y2; b.y = e.y; b.L = e.L; b.x = e.x; b.xL = e.xL; b.x2 = e.x2; b.f = e.f; b.f34 = e.f34;
-  double q, amp = 1.0;
-  if (MODEL == 1) {
-    q = fma(cb(CB_PH + 0), b.y5, cb(CB_PH + 4));
-    q = fma(cb(CB_PH + 1), b.y3, q);
-    q = fma(cb(CB_PH + 2), b.y2, q);
-    q = fma(cb(CB_PH + 3), b.y, q);
-    q = fma(cb(CB_PH + 5), b.L, q);
-    q = fma(cb(CB_PH + 6), b.x, q);
-    q = fma(cb(CB_PH + 7), b.xL, q);
-    q = fma(cb(CB_PH + 8), b.x2, q);
-    q = fma(cb(CB_PH + 9), b.f, q);
-  } else {
-    phenom_bin_t(cb, b, mt, exp_tab(cb(CB_AM + 3) * (b.f - cb(CB_AM + 0)), mt), q, amp);
-  }
-#pragma unroll
-  for (int d = 0; d < NDET; ++d) {
-    double sn, cs;
-    sincos_lut(64.0 * fma(-cb(CB_DET + 4 * d + 2), b.f, q), mt, sn, cs);
-    const double cr = cb(CB_DET + 4 * d), ci = cb(CB_DET + 4 * d + 1);
-    g[d] = make_double2(amp * fma(cr, cs, ci * sn), amp * fma(ci, cs, -(cr * sn)));
-  }
-}
-
-template <int MODEL, int NDET>
-__global__ void __launch_bounds__(kRbThreads) k_relbin(const DevCfg* __restrict__ cfgp, Tables tb, RbDev rb, const double* __restrict__ cbs_g,
-                                                        long long B, double* logl, double* parts) {
-  constexpr int NT = kRbThreads;
-  __shared__ MathTables mtab;
-  extern __shared__ __align__(16) unsigned char rb_smem[];
-  const int nb = rb.nb;
-  RbEdge<NDET>* ed = reinterpret_cast<RbEdge<NDET>*>(rb_smem);                    // [nb + 1]
-  double* rb_cbT = reinterpret_cast<double*>(ed + (nb + 1));                       // PhenomD-form: [CB_SIZE][NT], transposed
-  const int tid = threadIdx.x;
-  const long long p0 = (long long)blockIdx.x * NT, p = p0 + tid;
-  const bool have = p < B;
-  load_math_tables(&mtab, tb.mt, tid, NT);
-  for (int i = tid; i <= nb; i += NT) {
-    const int k = __ldg(rb.edge + i);
-    const BinBasis b = make_basis(tb, k, MODEL == 2);
-    RbEdge<NDET> e;
-    e.y5 = b.y5; e.y3 = b.y3; e.y2 = b.y2; e.y = b.y; e.L = b.L; e.x = b.x; e.xL = b.xL; e.x2 = b.x2; e.f = b.f; e.f34 = b.f34;
-    e.inv_w = (i > 0) ? __ldg(rb.inv_w + (i - 1)) : 0.0;
-    e.pad = 0.0;
-#pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      e.ig0[d] = __ldg(rb.ig0 + (size_t)d * (nb + 1) + i);
-      const size_t ib = (size_t)d * nb + (i > 0 ? i - 1 : 0);
-      e.A0[d] = __ldg(rb.A0 + ib); e.A1[d] = __ldg(rb.A1 + ib); e.B0[d] = __ldg(rb.B0 + ib); e.B1[d] = __ldg(rb.B1 + ib);
-    }
-    ed[i] = e;
-  }
-  // coefficient block of this thread's particle: TaylorF2 -> registers; PhenomD-form -> shared memory, transposed
-  double cbl[MODEL == 1 ? 30 : 1];
-  if (MODEL == 1) {
-#pragma unroll
-    for (int i = 0; i < 30; ++i) cbl[i] = have ? __ldg(cbs_g + p * CB_SIZE + i) : 0.0;
-  } else {
-    for (int e = tid; e < NT * CB_SIZE; e += NT) {
-      const int part = e % NT, i = e / NT;
-      rb_cbT[i * NT + part] = (p0 + part < B) ? __ldg(cbs_g + (p0 + part) * CB_SIZE + i) : 0.0;
-    }
-  }
-  __syncthreads();
-  double2 prev[NDET];
-  double dh[NDET], hh[NDET];
-#pragma unroll
-  for (int d = 0; d < NDET; ++d) { dh[d] = 0.0; hh[d] = 0.0; prev[d] = make_double2(0.0, 0.0); }
-#pragma unroll 2
-  for (int i = 0; i <= nb; ++i) {
-    const RbEdge<NDET>& e = ed[i];
-    double2 g[NDET];
-    if (MODEL == 1) gw_g_edge<MODEL, NDET>(CbPtr{cbl}, e, &mtab, g);
-    else gw_g_edge<MODEL, NDET>(CbStrided{rb_cbT + tid, NT}, e, &mtab, g);
-#pragma unroll
-    for (int d = 0; d < NDET; ++d) {
-      const double2 ig = e.ig0[d];
-      const double2 r = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
-      if (i > 0) {
-        const double iw = e.inv_w;
-        const double r0r = 0.5 * (prev[d].x + r.x), r0i = 0.5 * (prev[d].y + r.y);
-        const double r1r = (r.x - prev[d].x) * iw, r1i = (r.y - prev[d].y) * iw;
-        const double2 a0 = e.A0[d], a1 = e.A1[d];
-        dh[d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
-        hh[d] += fma(e.B0[d], fma(r0r, r0r, r0i * r0i), 2.0 * e.B1[d] * fma(r0r, r1r, r0i * r1i));
-      }
-      prev[d] = r;
-    }
-  }
-  if (!have) return;
-  const bool valid = ((MODEL == 1) ? cbl[CB_VALID] : rb_cbT[CB_VALID * NT + tid]) != 0.0;
-  double l = 0.0;
-#pragma unroll
-  for (int d = 0; d < NDET; ++d) {
-    if (parts) { parts[p * 2 * NDET + 2 * d] = valid ? dh[d] : nan(""); parts[p * 2 * NDET + 2 * d + 1] = valid ? hh[d] : nan(""); }
-    l += dh[d] - 0.5 * hh[d];
-  }
-  logl[p] = valid ? l : -INFINITY;
-}
-
-// shared memory of k_relbin: the staged edges (+ the transposed coefficient blocks for PhenomD-form)
-template <int MODEL, int NDET>
-size_t relbin_smem_bytes(int nb) {
-  return sizeof(RbEdge<NDET>) * ((size_t)nb + 1) + (MODEL == 2 ? sizeof(double) * CB_SIZE * kRbThreads : 0);
-}
-
-// ======================================================================================================
-// K2: acceptance walk
-// ======================================================================================================
-struct WalkArgs {
-  const double* donors;  // [m, D]
-  int m;
-  double* u;             // [B, D]
-  double* logl;          // [B]
-  long long B;
-  double lstar;
-  const double* lstar_dev;  // if non-null overrides lstar
-  int W;
-  const int* W_dev;         // if non-null overrides W
-  uint32_t k0, k1, stream_id;
-  const long long* iter_dev;  // if non-null: stream_id |= (*iter & 0xFFFFFF)
-  long long slot0;
-  int* n_accept; int* n_eval; int* n_oob;
-  uint8_t* tflags; double* tlogl;
-  int trace_stride;
-  int spec;                 // speculative steps per chunk: cap (1..kWalkDMax) of the per-walker adaptive length ...
-  int spec_fixed;           // ... or, if non-zero, the fixed length
-  int spec_cap;             // chunk buffers in shared memory hold this many steps (>= spec)
-};
-
-// DE proposal for one walker (footnote P:120; R:L8-L10).  Returns false if out of bounds.
-__device__ __forceinline__ bool de_propose(const DevCfg& cfg, const WalkArgs& a, uint32_t sid, uint32_t t, uint32_t slot,
-                                           const double* cur, double* prop) {
-  uint32_t b0[4];
-  philox4x32_10(0u, t, slot, sid, a.k0, a.k1, b0);
-  uint32_t ia = __umulhi(b0[0], (uint32_t)a.m);
-  uint32_t ib = __umulhi(b0[1], (uint32_t)(a.m - 1));
-  ib += (ib >= ia) ? 1u : 0u;
-  double gamma = 1.0;
-  if (b0[2] >= 0x80000000u) {
-    uint32_t b1[4], b2[4];
-    philox4x32_10(1u, t, slot, sid, a.k0, a.k1, b1);
-    philox4x32_10(2u, t, slot, sid, a.k0, a.k1, b2);
-    double prod = ((u01(b1[0], b1[1]) * u01(b1[2], b1[3])) * u01(b2[0], b2[1])) * u01(b2[2], b2[3]);
-    gamma = (2.38 / sqrt(2.0 * cfg.n_free)) * (-0.25 * log(prod));
-  }
-  const int D = cfg.ndim;
-  bool inb = true;
-  for (int d = 0; d < D; ++d) {
-    if (cfg.prior_kind[d] == 4) { prop[d] = cur[d]; continue; }
-    double diff = a.donors[(size_t)ia * D + d] - a.donors[(size_t)ib * D + d];
-    double x = fma(gamma, diff, cur[d]);
-    if (cfg.periodic[d]) x = x - floor(x);
-    else if (!(x > 0.0 && x < 1.0)) inb = false;
-    prop[d] = x;
-  }
-  return inb;
-}
-
-__device__ __forceinline__ double simple_loglike(const DevCfg& cfg, const double* u) {
-  const int D = cfg.ndim;
-  if (cfg.like_kind == 3) {
-    double r = 0.0;
-    for (int d = 0; d < D; ++d) r = fmax(r, fabs(u[d] - 0.5));
-    return -r;
-  }
-  double th[kMaxDim];
-  for (int d = 0; d < D; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], u[d]) - cfg.toy_mean[d];
-  double qf = 0.0;
-  for (int i = 0; i < D; ++i)
-    for (int j = 0; j < D; ++j) qf += th[i] * cfg.toy_prec[i * D + j] * th[j];
-  return cfg.toy_lognorm - 0.5 * qf;
-}
-
-__global__ void k_loglike_simple(const DevCfg* __restrict__ cfgp, const double* __restrict__ u, long long B, double* logl) {
-  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (i >= B) return;
-  double uu[kMaxDim];
-  for (int d = 0; d < cfgp->ndim; ++d) uu[d] = u[i * cfgp->ndim + d];
-  logl[i] = simple_loglike(*cfgp, uu);
-}
-
-__global__ void k_walk_simple(const DevCfg* __restrict__ cfgp, WalkArgs a) {
-  long long row = blockIdx.x * (long long)blockDim.x + threadIdx.x;
-  if (row >= a.B) return;
-  const DevCfg& cfg = *cfgp;
-  const int D = cfg.ndim;
-  const int W = a.W_dev ? *a.W_dev : a.W;
-  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
-  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
-  const uint32_t slot = (uint32_t)(a.slot0 + row);
-  double cur[kMaxDim], prop[kMaxDim];
-  for (int d = 0; d < D; ++d) cur[d] = a.u[row * D + d];
-  double curl = a.logl[row];
-  int na = 0, ne = 0, no = 0;
-  for (int t = 0; t < W; ++t) {
-    bool inb = de_propose(cfg, a, sid, (uint32_t)t, slot, cur, prop);
-    uint8_t fl = 0;
-    double pl = nan("");
-    if (!inb) { ++no; fl = 1; }
-    else {
-      pl = simple_loglike(cfg, prop);
-      ++ne; fl = 4;
-      if (pl > lstar) {
-        for (int d = 0; d < D; ++d) cur[d] = prop[d];
-        curl = pl; ++na; fl |= 2;
-      }
-    }
-    if (a.tflags) a.tflags[row * a.trace_stride + t] = fl;
-    if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
-  }
-  for (int d = 0; d < D; ++d) a.u[row * D + d] = cur[d];
-  a.logl[row] = curl;
-  if (a.n_accept) a.n_accept[row] = na;
-  if (a.n_eval) a.n_eval[row] = ne;
-  if (a.n_oob) a.n_oob[row] = no;
-}
-
-// GW walk: one CTA per walker, all W steps in one launch, speculative chunks of up to DMAX steps.
-//
-// A walker's chain is serial (proposal t+1 starts from the point accepted at t), and one step is: propose + transform + ~3 kflop
-// of serial waveform set-up by ONE thread, then a bin sweep.  With acceptance rates of 0.1-10 % per step the outcome "rejected" is
-// almost certain, so the kernel works on a CHUNK of future steps at once, all proposed from the current point: warp 0 draws the
-// proposals of steps t0, t0+1, ... 32 at a time (Philox counters are per step) until E of them are in bounds, builds the E
-// coefficient blocks side by side (SIMT: E set-ups for the latency of one), the physical ones are swept PG at a time (shared
-// table loads, ILP), and thread 0 then walks through the chunk's steps in order: out-of-bounds -> counted; logL' > L* -> accepted,
-// and the steps after it are DISCARDED (they started from a stale point) and redone in the next chunk from t0 + j + 1.  The
-// decisions, counters and trace are exactly those of the sequential algorithm (oracle_walk); only work is wasted, never semantics
-// changed.  Each walker adapts its own E (start 2; halved after a chunk with an acceptance, doubled up to the slot cap after one
-// without), or E is fixed by option.
-constexpr int kWalkDMax = 32;   // evaluations per chunk (cap): one warp sets them up side by side
-constexpr int kWalkPG = 2;     // particles per bin sweep
-constexpr int kWalkSteps = 128;   // steps per chunk (cap): proposals are drawn 32 at a time until enough are in bounds
-
-template <int MODEL, int NDET, int PG, int NT>
-__device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
-                                            const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
-                                            const int* slot, double* red, double* out /*smem [PG][N]*/) {
-  using AL = AccLayout<MODEL, NDET>;
-  constexpr int NV = PG * AL::N;
-  double acc[PG][AL::N];
-  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, mt, active, slot, acc);
-  double v[NV];
-#pragma unroll
-  for (int p = 0; p < PG; ++p)
-#pragma unroll
-    for (int i = 0; i < AL::N; ++i) v[p * AL::N + i] = acc[p][i];
-  block_reduce<NV, NT>(v, red, out);
-}
-
-// dynamic shared memory of k_walk_gw for a chunk cap of dm steps
-template <int NDET, int NT>
-constexpr size_t walk_smem_bytes(int dm) {
-  return sizeof(double2) * dm * (NDET > 1 ? NDET - 1 : 1) * (32 + NT / 32 + 1) + sizeof(double) * dm * (CB_SIZE + kMaxDim);
-}
-
-// NT threads per walker: 128 when all walkers of the batch are resident at 4 CTAs per SM, 96 (5 per SM) or 64 (8 per SM) when
-// that keeps a larger batch in one wave (config 4: k = 700 on 148 SMs).
-// RB: the likelihood of a proposal is the relative-binning one (edges instead of a full bin sweep).
-template <int MODEL, int NDET, int NT, bool RB>
-__global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restrict__ cfgp, Tables tb, WalkArgs a, RbDev rb) {
-  using AL = AccLayout<MODEL, NDET>;
-  constexpr int NW = NT / 32, PG = kWalkPG, ND1 = NDET > 1 ? NDET - 1 : 1;
-  constexpr int DMX = kWalkDMax;
-  const int DM = max(1, min(DMX, a.spec_cap));   // buffers are carved for this many steps per chunk
-  // per-chunk buffers in dynamic shared memory (WalkSmem<NDET>::kBytes): coefficient blocks, phasor tables, proposals
-  extern __shared__ __align__(16) unsigned char walk_smem[];
-  double2* tabL = reinterpret_cast<double2*>(walk_smem);          // [DM][ND1][32]
-  double2* tabW = tabL + DM * ND1 * 32;                            // [DM][ND1][NW]
-  double2* step = tabW + DM * ND1 * NW;                            // [DM][ND1]
-  double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
-  double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
-  double2* rbuf = reinterpret_cast<double2*>(cbs + DM * (CB_SIZE + kMaxDim));              // RB: partial sums [32][NT/32][2 NDET]
-  __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DMX];
-  __shared__ MathTables mtab;
-  __shared__ bool active[PG];
-  __shared__ int slot[PG];
-  __shared__ double s_cur[kMaxDim], s_curl;
-  __shared__ double s_stage[32][kMaxDim];       // phase A1: one proposal per lane of warp 0
-  __shared__ int s_flag[DMX];                   // per slot: 1 in bounds but unphysical theta (logL = -inf), 2 to be swept
-  __shared__ unsigned char s_step[kWalkSteps];  // per step of the chunk: 0 out of bounds, else slot + 1
-  __shared__ int s_t0, s_d, s_nsteps, s_nslots;
-  const DevCfg& cfg = *cfgp;
-  const int D = cfg.ndim;
-  const int W = a.W_dev ? *a.W_dev : a.W;
-  const int spec = max(1, min(DM, a.spec));   // cap of the evaluations per chunk
-  const bool spec_fixed = a.spec_fixed != 0;
-  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
-  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
-  const int tid = threadIdx.x, lane = tid & 31;
-  const long long row = blockIdx.x;
-  int na = 0, ne = 0, no = 0;   // thread 0's counters
-  load_math_tables(&mtab, tb.mt, tid, NT);
-  if (tid == 0) {
-    for (int d = 0; d < D; ++d) s_cur[d] = a.u[row * D + d];
-    s_curl = a.logl[row];
-    s_t0 = 0;
-    s_d = spec_fixed ? spec : min(spec, 2);
-  }
-  __syncthreads();
-  while (true) {
-    const int t0 = s_t0;
-    if (t0 >= W) break;
-    // ---- phase A (warp 0).  A1: propose steps t0, t0+1, ... 32 at a time from the current point until s_d of them are in
-    // bounds (out-of-bounds steps cost a Philox block and 11 FMAs, nothing else) or the step cap is reached; the chunk ends with
-    // the step of the last collected in-bounds proposal.  A2: the expensive part -- prior transform and waveform set-up -- for the
-    // collected proposals, one per lane, all lanes busy.
-    if (tid < 32) {
-      const int emax = s_d;
-      int nslots = 0, nsteps = 0;
-      while (nslots < emax && nsteps < kWalkSteps && t0 + nsteps < W) {
-        const int j = nsteps + lane;
-        const bool live = j < kWalkSteps && t0 + j < W;
-        const bool inb = live && de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur, s_stage[lane]);
-        const unsigned bal = __ballot_sync(0xffffffffu, inb);
-        const int rank = __popc(bal & ((1u << lane) - 1u));
-        const int room = emax - nslots, cnt = __popc(bal);
-        int consumed = min(32, min(kWalkSteps - nsteps, W - t0 - nsteps));
-        if (cnt > room) {   // more in-bounds proposals than slots left: stop right after the room-th one
-          const unsigned m2 = __ballot_sync(0xffffffffu, inb && rank == room - 1);
-          consumed = __ffs(m2);
-        }
-        if (lane < consumed) {
-          s_step[j] = inb ? (unsigned char)(nslots + rank + 1) : 0;
-          if (inb)
-            for (int d = 0; d < D; ++d) s_prop[nslots + rank][d] = s_stage[lane][d];
-        }
-        nslots += min(cnt, room);
-        nsteps += consumed;
-        __syncwarp();
-      }
-      if (lane == 0) { s_nsteps = nsteps; s_nslots = nslots; }
-      if (lane < nslots) {
-        double th[11];
-#pragma unroll
-        for (int d = 0; d < 11; ++d) th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], s_prop[lane][d]);
-        s_flag[lane] = setup_particle<MODEL>(cfg, th, cbs + lane * CB_SIZE) ? 2 : 1;
-      }
-    }
-    __syncthreads();
-    const int nd = s_nslots, nsteps = s_nsteps;
-    // the proposals that need a sweep, in order (every thread counts them the same way)
-    int n_in = 0;
-#pragma unroll
-    for (int j = 0; j < DMX; ++j) n_in += (j < nd && s_flag[j] == 2) ? 1 : 0;
-    if (RB && n_in > 0) {
-      // ---- phase B, relative binning: NT/32 threads per proposal, each walks a contiguous run of bins edge by edge (ratio r = g/g0
-      // at the edge, then the bin between the previous edge and this one; the first edge of a run is recomputed by its owner), no
-      // barrier until the partial sums meet in shared memory
-      constexpr int T = NT / 32;
-      const int nbn = rb.nb;
-      const int sl = tid / T, part = tid % T;
-      double v[2 * NDET];
-#pragma unroll
-      for (int i = 0; i < 2 * NDET; ++i) v[i] = 0.0;
-      if (sl < nd && s_flag[sl] == 2) {
-        const CbPtr cb{cbs + sl * CB_SIZE};
-        const int per = (nbn + T - 1) / T, b0 = part * per, b1 = min(nbn, b0 + per);
-        double2 prev[NDET];
-        for (int i = b0; i <= b1 && b0 < b1; ++i) {
-          double2 g[NDET];
-          gw_g_at<MODEL, NDET>(cb, tb, __ldg(rb.edge + i), &mtab, g);
-#pragma unroll
-          for (int d = 0; d < NDET; ++d) {
-            const double2 ig = __ldg(rb.ig0 + (size_t)d * (nbn + 1) + i);
-            const double2 r = make_double2(fma(g[d].x, ig.x, -(g[d].y * ig.y)), fma(g[d].x, ig.y, g[d].y * ig.x));
-            if (i > b0) {
-              const size_t ib = (size_t)d * nbn + (i - 1);
-              const double iw = __ldg(rb.inv_w + (i - 1));
-              const double r0r = 0.5 * (prev[d].x + r.x), r0i = 0.5 * (prev[d].y + r.y);
-              const double r1r = (r.x - prev[d].x) * iw, r1i = (r.y - prev[d].y) * iw;
-              const double2 a0 = __ldg(rb.A0 + ib), a1 = __ldg(rb.A1 + ib);
-              v[2 * d] += fma(a0.x, r0r, a0.y * r0i) + fma(a1.x, r1r, a1.y * r1i);
-              v[2 * d + 1] += fma(__ldg(rb.B0 + ib), fma(r0r, r0r, r0i * r0i), 2.0 * __ldg(rb.B1 + ib) * fma(r0r, r1r, r0i * r1i));
-            }
-            prev[d] = r;
-          }
-        }
-      }
-      double* rpart = reinterpret_cast<double*>(rbuf);      // [32 slots][T][2 NDET]
-#pragma unroll
-      for (int i = 0; i < 2 * NDET; ++i) rpart[(sl * T + part) * 2 * NDET + i] = v[i];
-      __syncthreads();
-      if (part == 0 && sl < nd && s_flag[sl] == 2) {
-        double l = 0.0;
-#pragma unroll
-        for (int d = 0; d < NDET; ++d) {
-          double dh = 0.0, hh = 0.0;
-#pragma unroll
-          for (int t = 0; t < T; ++t) { dh += rpart[(sl * T + t) * 2 * NDET + 2 * d]; hh += rpart[(sl * T + t) * 2 * NDET + 2 * d + 1]; }
-          l += dh - 0.5 * hh;
-        }
-        s_logl[sl] = l;
-      }
-      __syncthreads();
-    }
-    if (!RB && n_in > 0) {
-      build_phasor_tables<NDET, NT>(cfg, cbs, nd, tabL, tabW, step);
-      __syncthreads();
-      // ---- phase B: sweeps, PG particles at a time (a single left-over goes through the one-particle loop)
-      for (int g = 0; g < n_in; g += PG) {
-        const int ng = min(PG, n_in - g);
-        if (tid < PG) {
-          int cnt = 0, mine = -1, first = 0;
-#pragma unroll
-          for (int j = 0; j < DMX; ++j) {
-            if (j < nd && s_flag[j] == 2) {
-              if (cnt == g) first = j;
-              if (cnt == g + tid) mine = j;
-              ++cnt;
-            }
-          }
-          slot[tid] = (mine >= 0) ? mine : first;
-          active[tid] = mine >= 0;
-        }
-        __syncthreads();
-        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
-        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
-        if (tid < ng) s_logl[slot[tid]] = finish_logl<MODEL, NDET>(cfg, cbs + slot[tid] * CB_SIZE, out + tid * AL::N, nullptr);
-        __syncthreads();
-      }
-    }
-    // ---- phase C: the chunk's steps in order; the first acceptance invalidates the rest of the chunk
-    if (tid == 0) {
-      int used = nsteps;
-      bool hit = false;
-      for (int j = 0; j < nsteps; ++j) {
-        const int t = t0 + j;
-        const int sl = (int)s_step[j] - 1;
-        if (sl < 0) {
-          ++no;
-          if (a.tflags) a.tflags[row * a.trace_stride + t] = 1;
-          if (a.tlogl) a.tlogl[row * a.trace_stride + t] = nan("");
-          continue;
-        }
-        ++ne;
-        const double pl = (s_flag[sl] == 2) ? s_logl[sl] : -INFINITY;
-        uint8_t tf = 4;
-        const bool acc_ = pl > lstar;
-        if (acc_) {
-          for (int d = 0; d < D; ++d) s_cur[d] = s_prop[sl][d];
-          s_curl = pl; ++na; tf |= 2;
-        }
-        if (a.tflags) a.tflags[row * a.trace_stride + t] = tf;
-        if (a.tlogl) a.tlogl[row * a.trace_stride + t] = pl;
-        if (acc_) { used = j + 1; hit = true; break; }
-      }
-      s_t0 = t0 + used;
-      // per-walker chunk size (evaluations): halve after a chunk that ended in an acceptance (the rest of it was wasted), double
-      // after one that did not; a function of the walker's own chain only, so still deterministic
-      if (!spec_fixed) s_d = hit ? max(1, s_d >> 1) : min(spec, s_d << 1);
-    }
-    __syncthreads();
-  }
-  if (tid == 0) {
-    for (int d = 0; d < D; ++d) a.u[row * D + d] = s_cur[d];
-    a.logl[row] = s_curl;
-    if (a.n_accept) a.n_accept[row] = na;
-    if (a.n_eval) a.n_eval[row] = ne;
-    if (a.n_oob) a.n_oob[row] = no;
-  }
-}
-
-// ======================================================================================================
-// K3: selection, evidence, replacement, adaptation
-// ======================================================================================================
-// Stable rank by counting: order[rank(i)] = i with rank(i) = #{j : l_j < l_i or (l_j == l_i and j < i)}  (R:L6).
-__global__ void k_rank(const double* __restrict__ logl, int n, int* order) {
-  __shared__ double tile[256];
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  double li = (i < n) ? logl[i] : 0.0;
-  int rank = 0;
-  for (int base = 0; base < n; base += 256) {
-    int j = base + threadIdx.x;
-    tile[threadIdx.x] = (j < n) ? logl[j] : INFINITY;
-    __syncthreads();
-    int lim = min(256, n - base);
-    for (int jj = 0; jj < lim; ++jj) {
-      double lj = tile[jj];
-      rank += (lj < li) || (lj == li && (base + jj) < i);
-    }
-    __syncthreads();
-  }
-  if (i < n) order[rank] = i;
-}
-
-__device__ __forceinline__ double logaddexp_d(double a, double b) {
-  if (a == -INFINITY) return b;
-  if (b == -INFINITY) return a;
-  double m = fmax(a, b);
-  return m + log1p(exp(-fabs(a - b)));
-}
-
-__device__ __forceinline__ void evidence_update(double li, double ni, double& logx, double& logz, double& h, double& logw) {
-  logw = logx + log(-expm1(-1.0 / ni));
-  double lw = li + logw;
-  double zn = logaddexp_d(logz, lw);
-  double hn = exp(lw - zn) * li;
-  if (logz != -INFINITY) hn += exp(logz - zn) * (h + logz);
-  hn -= zn;
-  h = hn; logz = zn; logx -= 1.0 / ni;
-}
-
-// Sequential evidence scan over the k dead points in ascending logL (eq. 3-5 with the saw-tooth live count; R:L16, L17).
-__global__ void k_evidence(DevState* st, const double* __restrict__ logl, const double* __restrict__ u, const int* __restrict__ order,
-                           int n, int k, int D, double* dead) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  double logx = st->logx, logz = st->logz, h = st->h;
-  for (int i = 0; i < k; ++i) {
-    int id = order[i];
-    double logw;
-    evidence_update(logl[id], (double)(n - i), logx, logz, h, logw);
-    if (dead) {
-      double* row = dead + (size_t)i * (D + 3);
-      for (int d = 0; d < D; ++d) row[d] = u[(size_t)id * D + d];
-      row[D] = logl[id]; row[D + 1] = logw; row[D + 2] = (double)(n - i);
-    }
-  }
-  st->logx = logx; st->logz = logz; st->h = h;
-  st->lstar = logl[order[k - 1]];
-  int W = (int)floor(st->walks);
-  st->W = max(1, min(W, st->maxmcmc));
-}
-
-// Survivor array in ascending-logL order + start points (uniform survivor, Philox tag 1; R:L7).
-__global__ void k_gather_start(const DevState* __restrict__ st, const double* __restrict__ u, const double* __restrict__ logl,
-                               const int* __restrict__ order, int n, int k, int D, uint32_t k0, uint32_t k1, double* surv, double* cur_u,
-                               double* cur_l) {
-  const int m = n - k;
-  int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < m) {
-    int id = order[k + i];
-    for (int d = 0; d < D; ++d) surv[(size_t)i * D + d] = u[(size_t)id * D + d];
-  }
-  if (i < k) {
-    uint32_t w[4];
-    philox4x32_10(0u, 0u, (uint32_t)i, (1u << 24) | (uint32_t)(st->iter & 0xFFFFFF), k0, k1, w);
-    int id = order[k + __umulhi(w[0], (uint32_t)m)];
-    for (int d = 0; d < D; ++d) cur_u[(size_t)i * D + d] = u[(size_t)id * D + d];
-    cur_l[i] = logl[id];
-  }
-}
-
-__global__ void k_writeback(const int* __restrict__ order, int k, int D, const double* __restrict__ cur_u, const double* __restrict__ cur_l,
-                            double* u, double* logl) {
-  int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= k) return;
-  int id = order[j];
-  for (int d = 0; d < D; ++d) u[(size_t)id * D + d] = cur_u[(size_t)j * D + d];
-  logl[id] = cur_l[j];
-}
-
-// Batch-level adaptation (R:L13-L15) and termination quantities (R:L18).  Single CTA, fixed-order reductions.
-__global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __restrict__ ne, const int* __restrict__ no, int k,
-                        const double* __restrict__ logl, int n) {
-  __shared__ long long s_a[256], s_e[256], s_o[256], s_s[256];
-  __shared__ int s_min[256], s_max[256];
-  __shared__ double s_d[256];
-  const int t = threadIdx.x;
-  long long a = 0, e = 0, o = 0, s = 0;
-  int mn = INT_MAX, mx = INT_MIN;
-  for (int j = t; j < k; j += 256) {
-    a += na[j]; e += ne[j]; o += no[j]; s += (na[j] == 0);
-    mn = min(mn, na[j]); mx = max(mx, na[j]);
-  }
-  s_a[t] = a; s_e[t] = e; s_o[t] = o; s_s[t] = s; s_min[t] = mn; s_max[t] = mx;
-  double lm = -INFINITY;
-  for (int i = t; i < n; i += 256) lm = fmax(lm, logl[i]);
-  s_d[t] = lm;
-  __syncthreads();
-  for (int w = 128; w > 0; w >>= 1) {
-    if (t < w) {
-      s_a[t] += s_a[t + w]; s_e[t] += s_e[t + w]; s_o[t] += s_o[t + w]; s_s[t] += s_s[t + w];
-      s_min[t] = min(s_min[t], s_min[t + w]); s_max[t] = max(s_max[t], s_max[t + w]);
-      s_d[t] = fmax(s_d[t], s_d[t + w]);
-    }
-    __syncthreads();
-  }
-  const double lmax = s_d[0];
-  __syncthreads();
-  double acc = 0.0;
-  for (int i = t; i < n; i += 256) acc += exp(logl[i] - lmax);
-  s_d[t] = acc;
-  __syncthreads();
-  for (int w = 128; w > 0; w >>= 1) {
-    if (t < w) s_d[t] += s_d[t + w];
-    __syncthreads();
-  }
-  if (t == 0) {
-    const int W = st->W;
-    double amean = (double)s_a[0] / k;
-    double r = fmax(0.5, amean) / W;
-    double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
-    st->walks = walks;
-    st->n_eval_total += s_e[0];
-    double lse = lmax + log(s_d[0]);
-    ns_stats& o_ = st->stats;
-    o_.iteration = st->iter;
-    o_.logl_star = st->lstar; o_.logx = st->logx; o_.logz = st->logz; o_.h = st->h;
-    o_.dlogz = logaddexp_d(st->logz, lmax + st->logx) - st->logz;
-    o_.live_frac_log = lse - log((double)n) + st->logx - st->logz;
-    o_.walk_len = W; o_.pad0 = 0; o_.walks_next = walks;
-    o_.accept_mean = amean; o_.accept_min = s_min[0]; o_.accept_max = s_max[0];
-    o_.n_eval = s_e[0]; o_.n_oob = s_o[0]; o_.n_stuck = s_s[0]; o_.n_eval_total = st->n_eval_total;
-    st->iter += 1;
-  }
-}
-
-// Final evidence: adds the live points with n_i = n..1 to a copy of the accumulators (R:L17).  out: logz, h.
-__global__ void k_finalize(const DevState* __restrict__ st, const double* __restrict__ logl, const int* __restrict__ order, int n,
-                           double* out) {
-  if (threadIdx.x != 0 || blockIdx.x != 0) return;
-  double logx = st->logx, logz = st->logz, h = st->h, lw;
-  for (int i = 0; i < n; ++i) evidence_update(logl[order[i]], (double)(n - i), logx, logz, h, lw);
-  out[0] = logz; out[1] = h;
-}
-
-// FP64 FMA throughput probe: 8 independent chains per thread.
-__global__ void k_dfma_probe(long long iters, double* sink) {
-  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
-  const double m = 0.999999, c = 1e-7;
-  for (long long i = 0; i < iters; ++i) {
-    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
-  }
-  double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
-  if (s == 123.456) sink[0] = s;
-}
 
 }  // namespace
 
