@@ -245,7 +245,7 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
         q = fma(pm[p][3], f34, q);
         q = fma(pm[p][4], atan_tab((f - pm[p][5]) * pm[p][6], mt), q);
         const double fx = f - am[p][0];
-        const double amp = am[p][1] * rcp_nr(fma(fx, fx, am[p][2])) * ex[p];
+        const double amp = am[p][1] * rcp_nr1(fma(fx, fx, am[p][2])) * ex[p];
         ex[p] *= exr[p];
         tail(p, q, amp, w, wsv);
       }

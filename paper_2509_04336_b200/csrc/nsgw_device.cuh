@@ -188,6 +188,15 @@ __device__ __forceinline__ double rcp_nr(double d) {
   return y;
 }
 
+// One Newton step only: relative error <= (seed error)^2 ~ 2^-40 -- for quantities that enter logL through a smooth factor
+// (a 1e-12 relative error of the amplitude or of the small remainder t of atan_tab is 1e-12 of that bin's term).
+__device__ __forceinline__ double rcp_nr1(double d) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(d));
+  const double e = fma(-d, y, 1.0);
+  return fma(y, e, y);
+}
+
 // exp(x) for |x| <= 700: n = rint(64 x / ln 2), r = x - n ln2/64 (two-term Cody-Waite, |r| <= 0.0055), degree-5 Taylor
 // (truncation 3.4e-17 relative), 2^(n/64) from the table and an exponent-field add.
 __device__ __forceinline__ double exp_tab(double x, const MathTables* mt) {
@@ -224,7 +233,7 @@ __device__ __forceinline__ double atan_tab(double y, const MathTables* mt) {
   jq -= magic;
   const double c = jq * (1.0 / 32.0);
   const double num = fma(-c, d, n), den = fma(c, n, d);
-  const double t = num * rcp_nr(den);
+  const double t = num * rcp_nr1(den);
   const double z = t * t;
   double p = fma(z, kAtanC[0], kAtanC[1]);
   p = fma(p, z, kAtanC[2]);
@@ -625,7 +634,7 @@ __device__ __forceinline__ void phenom_bin_t(const CB& cb, const BinBasis& b, co
     amp = p;
   } else {
     double fx = f - cb(CB_AM + 0);
-    amp = cb(CB_AM + 1) * rcp_nr(fma(fx, fx, cb(CB_AM + 2))) * ex;
+    amp = cb(CB_AM + 1) * rcp_nr1(fma(fx, fx, cb(CB_AM + 2))) * ex;
   }
 }
 
