@@ -30,11 +30,11 @@ UNIT = "evals/s"
 
 def alg_flops_per_bin(n_det, model="taylorf2"):
     """Algorithmic fp64 flops per (particle, bin) of the minimal formulation the kernel implements,
-    FMA = 2: 9-FMA phase (18); table-driven sincos: exact reduction (3 add), r^2 (1), sin 2 FMA + 1 mul (5), cos 3 FMA (6),
-    complex product with the table entry (6) = 21; detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex
+    FMA = 2: 9-FMA phase (18); table-driven sincos: exact reduction (F2I, I2F on the conversion pipe + 1 subtraction), r^2 (1),
+    sin 2 FMA + 1 mul (5), cos 3 FMA (6), complex product with the table entry (6) = 19; detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex
     Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
     assert model == "taylorf2"
-    return 18 + 21 + 8 + 14 * (n_det - 1)
+    return 18 + 19 + 8 + 14 * (n_det - 1)
 
 
 class ClockSampler:

@@ -424,7 +424,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       for (int j = 0; j < PP; ++j) {
         const double q = phase_pn_qt(a[j], b);
         double sn, cs;
-        sincos_lut(q, &mtab, sn, cs);
+        sincos_lut<true>(q, &mtab, sn, cs);
         acc[j][0] = fma(w[0].x, cs, acc[j][0]);
         acc[j][1] = fma(-w[0].x, sn, acc[j][1]);
         acc[j][0] = fma(-w[0].y, sn, acc[j][0]);

@@ -157,12 +157,22 @@ __device__ __forceinline__ void load_math_tables(MathTables* dst, const MathTabl
   for (int i = tid; i < (int)(sizeof(MathTables) / sizeof(double)); i += nthreads) d[i] = __ldg(g + i);
 }
 
+// CVT = true reduces with F2I / I2F (conversion pipe, off the FP64 pipe: measured +3 % in k_bins_lp, whose loop has no other
+// conversion-pipe work) instead of the three-add magic-number form (better where MUFU reciprocals already load that pipe).
+template <bool CVT = false>
 __device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, double& s, double& c) {
-  const double magic = 6755399441055744.0;  // 1.5 * 2^52
-  double kk = u + magic;
-  const int ki = __double2loint(kk);
-  kk -= magic;
-  const double r = u - kk;
+  int ki;
+  double r;
+  if (CVT) {
+    ki = __double2int_rn(u);
+    r = u - (double)ki;                        // exact: |u - k| <= 1/2 and |u| < 2^31
+  } else {
+    const double magic = 6755399441055744.0;  // 1.5 * 2^52
+    double kk = u + magic;
+    ki = __double2loint(kk);
+    kk -= magic;
+    r = u - kk;
+  }
   const double z = r * r;
   const double2 T = mt->sc[ki & 255];
   double ps = fma(z, kLutC[2], kLutC[1]);
