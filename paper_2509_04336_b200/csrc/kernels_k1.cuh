@@ -464,9 +464,22 @@ __global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restri
   double sums[AL::N];
 #pragma unroll
   for (int i = 0; i < AL::N; ++i) sums[i] = 0.0;
-  for (int c = 0; c < nchunks; ++c)
+  // range order is the summation order (fixed); loads of eight ranges are issued together (the sums themselves are short chains)
+  int c = 0;
+  for (; c + 8 <= nchunks; c += 8) {
+    double v[8][AL::N];
 #pragma unroll
-    for (int i = 0; i < AL::N; ++i) sums[i] += partial[((long long)c * AL::N + i) * B + p];
+    for (int j = 0; j < 8; ++j)
+#pragma unroll
+      for (int i = 0; i < AL::N; ++i) v[j][i] = __ldg(partial + ((long long)(c + j) * AL::N + i) * B + p);
+#pragma unroll
+    for (int j = 0; j < 8; ++j)
+#pragma unroll
+      for (int i = 0; i < AL::N; ++i) sums[i] += v[j][i];
+  }
+  for (; c < nchunks; ++c)
+#pragma unroll
+    for (int i = 0; i < AL::N; ++i) sums[i] += __ldg(partial + ((long long)c * AL::N + i) * B + p);
   logl[p] = finish_logl<MODEL, NDET>(*cfgp, cbs_g + p * CB_SIZE, sums, parts ? parts + p * 2 * NDET : nullptr);
 }
 
