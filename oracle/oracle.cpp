@@ -638,6 +638,102 @@ void orc_walk(const orc_problem* p, const double* surv_u, int32_t m, double* u, 
   }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Hit-and-run slice sampling inner kernel (the blackjax-ns default the paper builds on, and names as future
+// comparison; no formula in the paper: DESIGN.md reading R:L25).  One slice step from x under the constraint
+// "inside the unit cube (periodic dims wrap) and logL > L*":
+//   direction: z ~ N(0, I) over the free dims (Box-Muller on Philox blocks 0..7: z_2i = sqrt(-2 ln U1) cos(2 pi U2), z_2i+1 = .. sin),
+//              dir = Lc z / |z| with Lc a lower-triangular factor given by the caller (Cholesky of the live points' covariance);
+//   bracket:   l = -U0, r = l + 1 (U0 from block 8); stepping out: while inside(l) l -= 1 (at most 32 times), same for r;
+//   shrinkage: t = l + U_k (r - l) (U_k from block 9 + k/2, first or second pair of words); inside(t) -> move there; else the
+//              bracket end on t's side becomes t; at most 64 candidates, then the point stays.
+// Every inside() test of an in-cube point is one likelihood evaluation.  trace (optional): per step the number of evaluations
+// and the logL after the step.
+// ---------------------------------------------------------------------------------------------
+void orc_slice_walk(const orc_problem* p, const double* Lc /*[D][D] lower, row-major, free dims only used*/, double* u, double* logl,
+                    int64_t B, double logl_star, int32_t S, uint64_t seed, uint32_t stream_id, int64_t slot0, int32_t* n_eval,
+                    int32_t* n_oob, int32_t* n_expand, int32_t* n_shrink, int32_t* n_stuck, int32_t* t_evals, double* t_logl,
+                    int threads) {
+  const int D = p->ndim;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(threads > 0 ? threads : omp_get_max_threads_safe())
+  for (int64_t row = 0; row < B; ++row) {
+    const uint32_t j = (uint32_t)(slot0 + row);
+    double x[16], y[16], dir[16], z[16];
+    for (int d = 0; d < D; ++d) x[d] = u[row * D + d];
+    double xl = logl[row];
+    int ne = 0, no = 0, nx = 0, ns = 0, nk = 0;
+    int fr[16], nfree = 0;
+    for (int d = 0; d < D; ++d)
+      if (p->prior_kind[d] != PRIOR_FIXED) fr[nfree++] = d;
+    for (int s = 0; s < S; ++s) {
+      const int ne0 = ne;
+      // direction
+      double z2 = 0.0;
+      for (int i = 0; 2 * i < nfree; ++i) {
+        uint32_t w[4];
+        philox_block(seed, (uint32_t)i, (uint32_t)s, j, stream_id, w);
+        const double U1 = orc_u53(w[0], w[1]), U2 = orc_u53(w[2], w[3]);
+        const double rad = std::sqrt(-2.0 * std::log(U1));
+        z[2 * i] = rad * std::cos(2.0 * PI * U2);
+        if (2 * i + 1 < nfree) z[2 * i + 1] = rad * std::sin(2.0 * PI * U2);
+      }
+      for (int a = 0; a < nfree; ++a) z2 += z[a] * z[a];
+      const double inv = 1.0 / std::sqrt(z2);
+      for (int d = 0; d < D; ++d) dir[d] = 0.0;
+      for (int a = 0; a < nfree; ++a) {
+        double acc = 0.0;
+        for (int b = 0; b <= a; ++b) acc += Lc[(size_t)fr[a] * D + fr[b]] * z[b];
+        dir[fr[a]] = acc * inv;
+      }
+      auto inside = [&](double t, double* lout) -> bool {
+        bool oob = false;
+        for (int d = 0; d < D; ++d) {
+          if (p->prior_kind[d] == PRIOR_FIXED) { y[d] = x[d]; continue; }
+          double v = std::fma(t, dir[d], x[d]);
+          if (p->periodic[d]) v = v - std::floor(v);
+          else if (!(v > 0.0 && v < 1.0)) oob = true;
+          y[d] = v;
+        }
+        if (oob) { ++no; return false; }
+        const double l = loglike_from_u(p, y);
+        ++ne;
+        *lout = l;
+        return l > logl_star;
+      };
+      uint32_t w8[4];
+      philox_block(seed, 8u, (uint32_t)s, j, stream_id, w8);
+      double l = -orc_u53(w8[0], w8[1]), r = l + 1.0, tmp;
+      for (int k = 0; k < 32 && inside(l, &tmp); ++k) { l -= 1.0; ++nx; }
+      for (int k = 0; k < 32 && inside(r, &tmp); ++k) { r += 1.0; ++nx; }
+      bool moved = false;
+      for (int k = 0; k < 64; ++k) {
+        uint32_t w[4];
+        philox_block(seed, 9u + (uint32_t)(k / 2), (uint32_t)s, j, stream_id, w);
+        const double U = (k % 2 == 0) ? orc_u53(w[0], w[1]) : orc_u53(w[2], w[3]);
+        const double t = l + U * (r - l);
+        double lt;
+        if (inside(t, &lt)) {
+          for (int d = 0; d < D; ++d) x[d] = y[d];
+          xl = lt; moved = true;
+          break;
+        }
+        ++ns;
+        if (t < 0.0) l = t; else r = t;
+      }
+      if (!moved) ++nk;
+      if (t_evals) t_evals[row * S + s] = ne - ne0;
+      if (t_logl) t_logl[row * S + s] = xl;
+    }
+    for (int d = 0; d < D; ++d) u[row * D + d] = x[d];
+    logl[row] = xl;
+    if (n_eval) n_eval[row] = ne;
+    if (n_oob) n_oob[row] = no;
+    if (n_expand) n_expand[row] = nx;
+    if (n_shrink) n_shrink[row] = ns;
+    if (n_stuck) n_stuck[row] = nk;
+  }
+}
+
 // Proposal scale draw exposed for distribution pins: gamma for (seed, t, j, stream_id); returns coin via *is_one.
 double orc_gamma_draw(int n_free, uint64_t seed, uint32_t t, uint32_t j, uint32_t stream_id, int32_t m, int32_t* a_out, int32_t* b_out, int32_t* is_one) {
   uint32_t b0[4], b1[4], b2[4];

@@ -145,6 +145,25 @@ class OracleProblem:
         _lib.orc_gw_loglike(C.byref(self.p), _dp(theta), C.c_int64(B), _dp(logl), _dp(pr), C.c_int(threads))
         return (logl, pr) if parts else logl
 
+    # ---- hit-and-run slice sampling inner kernel (DESIGN.md R:L25) --------------------------------------
+    def slice_walk(self, Lc, u, logl, logl_star, S, seed, stream_id, slot0=0, trace=False, threads=0):
+        """Copies of u / logl are evolved by S slice steps each; Lc [ndim, ndim] lower-triangular direction factor."""
+        u = _f64(u).reshape(-1, self.ndim).copy()
+        logl = _f64(logl).copy()
+        Lc = _f64(Lc).reshape(self.ndim, self.ndim)
+        B = u.shape[0]
+        cnt = {k: np.zeros(B, dtype=np.int32) for k in ("n_eval", "n_oob", "n_expand", "n_shrink", "n_stuck")}
+        te = np.zeros((B, S), dtype=np.int32) if trace else None
+        tl = np.zeros((B, S)) if trace else None
+        ip = lambda a: a.ctypes.data_as(C.POINTER(C.c_int32)) if a is not None else None
+        _lib.orc_slice_walk(C.byref(self.p), _dp(Lc), _dp(u), _dp(logl), C.c_int64(B), C.c_double(logl_star), C.c_int32(S),
+                            C.c_uint64(seed), C.c_uint32(stream_id), C.c_int64(slot0), ip(cnt["n_eval"]), ip(cnt["n_oob"]),
+                            ip(cnt["n_expand"]), ip(cnt["n_shrink"]), ip(cnt["n_stuck"]), ip(te), _dp(tl), C.c_int(threads))
+        out = dict(u=u, logl=logl, **cnt)
+        if trace:
+            out["trace_evals"], out["trace_logl"] = te, tl
+        return out
+
     # ---- relative binning (DESIGN.md R:L24) ----------------------------------------------------------
     def relbin(self, theta0, chi=1.0, eps=0.5):
         return OracleRelBin(self, theta0, chi, eps)
