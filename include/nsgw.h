@@ -136,6 +136,21 @@ int64_t ns_run(ns_handle* h, int32_t term_kind, double term_tol, int64_t max_ite
 int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double term_tol, int64_t max_iter, ns_stats* last_host,
                     int64_t* iters_host, double** dead_dev);
 
+/* Hit-and-run slice-sampling inner kernel (the blackjax-ns default the paper builds on, and names as a future
+ * comparison; reading R:L25), as a batch call with the same shape as ns_walk_batch: every row of u_dev [B, ndim]
+ * (in: start, out: end; logl_dev [B] likewise) does n_steps slice steps under "inside the unit cube (periodic dims wrap) and
+ * logL > logl_star".  One step: direction Lc z / |z| with z ~ N(0, I) over the non-FIXED dims and lc_dev [ndim, ndim] a
+ * lower-triangular factor (row-major; e.g. the Cholesky factor of the live points' covariance in unit-cube coordinates); bracket of
+ * width 1 placed uniformly about the point, stepped out while its ends are inside (at most 32 times per end); shrinkage with
+ * uniform candidates (at most 64).  Philox counter (block, step, slot0 + row, stream_id) as in ns_walk_batch.  Counters (each
+ * may be NULL): likelihood evaluations, out-of-cube candidates, bracket expansions, rejected shrink candidates, steps that gave up.
+ * trace_evals_dev / trace_logl_dev (optional, [B, n_steps]): evaluations of each step and logL after it.  The number of
+ * evaluations per step varies from walker to walker (this is the divergence the acceptance walk avoids).  Exact likelihood only
+ * (-5 when NSGW_OPT_LIKELIHOOD selects relative binning). */
+int ns_slice_batch(ns_handle* h, const double* lc_dev, double* u_dev, double* logl_dev, int64_t B, double logl_star, int32_t n_steps,
+                   uint64_t seed, uint32_t stream_id, int64_t slot0, int32_t* n_eval_dev, int32_t* n_oob_dev, int32_t* n_expand_dev,
+                   int32_t* n_shrink_dev, int32_t* n_stuck_dev, int32_t* trace_evals_dev, double* trace_logl_dev, void* stream);
+
 /* ---- Relative binning ("heterodyned likelihood"; the paper names it as the remedy for the bins x samples cost,
  * P:172, and gives no formula: DESIGN.md reading R:L24 restates the published scheme). ----
  * ns_relbin_setup builds, on the device, the summary data about the fiducial parameters theta0_host[11] (physical, Table-1 order):

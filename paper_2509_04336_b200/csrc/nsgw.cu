@@ -7,6 +7,7 @@
 //                        particle pair), k_bins_lp + k_finish (lane per particle), k_waveform
 //   kernels_relbin.cuh   k_rb_delta / k_rb_select / k_rb_summary / k_relbin (relative binning, R:L24)
 //   kernels_walk.cuh     de_propose, k_walk_simple, k_walk_gw (speculative chunks; exact or relative-binning likelihood)
+//   kernels_slice.cuh    k_slice_simple, k_slice_gw (hit-and-run slice sampling, R:L25)
 //   kernels_k3.cuh       k_rank / k_evidence / k_gather_start / k_writeback / k_adapt / k_finalize, k_dfma_probe
 // This file: ns_handle, launch geometry, argument checks and the extern "C" entry points.
 #include <cstdio>
@@ -45,6 +46,7 @@ struct DevState {
 #include "kernels_k1.cuh"
 #include "kernels_relbin.cuh"
 #include "kernels_walk.cuh"
+#include "kernels_slice.cuh"
 #include "kernels_k3.cuh"
 
 
@@ -628,6 +630,35 @@ int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
 }  // namespace
 
 extern "C" {
+
+int ns_slice_batch(ns_handle* h, const double* lc_dev, double* u_dev, double* logl_dev, int64_t B, double logl_star, int32_t n_steps,
+                   uint64_t seed, uint32_t stream_id, int64_t slot0, int32_t* n_eval_dev, int32_t* n_oob_dev, int32_t* n_expand_dev,
+                   int32_t* n_shrink_dev, int32_t* n_stuck_dev, int32_t* trace_evals_dev, double* trace_logl_dev, void* stream) {
+  if (!h) return -3;
+  if (B < 0 || n_steps < 0 || !lc_dev || (B > 0 && (!u_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  if (h->opt_like == 1) return fail(h, -5, "the slice kernel evaluates the exact likelihood only");
+  if (B == 0) return 0;
+  cudaStream_t s = (cudaStream_t)stream;
+  SliceArgs a;
+  memset(&a, 0, sizeof(a));
+  a.Lc = lc_dev; a.u = u_dev; a.logl = logl_dev; a.B = B; a.lstar = logl_star; a.S = n_steps;
+  a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32); a.stream_id = stream_id; a.slot0 = slot0;
+  a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.n_expand = n_expand_dev; a.n_shrink = n_shrink_dev; a.n_stuck = n_stuck_dev;
+  a.t_evals = trace_evals_dev; a.t_logl = trace_logl_dev;
+  if (!is_gw(h->cfg.like_kind)) {
+    k_slice_simple<<<(unsigned)((B + 63) / 64), 64, 0, s>>>(h->d_cfg, a);
+    LAUNCH_CHECK(h);
+    return 0;
+  }
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  const int nd = h->cfg.n_det;
+#define SLICE_GW(M, N) k_slice_gw<M, N, 128><<<(unsigned)B, 128, 0, s>>>(h->d_cfg, h->tb, a)
+  if (tf2) { if (nd == 1) SLICE_GW(1, 1); else if (nd == 2) SLICE_GW(1, 2); else SLICE_GW(1, 3); }
+  else { if (nd == 1) SLICE_GW(2, 1); else if (nd == 2) SLICE_GW(2, 2); else SLICE_GW(2, 3); }
+#undef SLICE_GW
+  LAUNCH_CHECK(h);
+  return 0;
+}
 
 int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) {
   if (!h) return -3;

@@ -43,7 +43,7 @@ class NsStats(C.Structure):
 
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
-           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 _lib = None
@@ -210,6 +210,21 @@ class Handle:
         out = dict(n_accept=na, n_eval=ne, n_oob=no)
         if trace:
             out["flags"], out["trace_logl"] = fl, tl
+        return out
+
+    def slice_batch(self, lc, u, logl, logl_star, n_steps, seed, stream_id, slot0=0, trace=False):
+        """In place on u / logl (hit-and-run slice sampling, R:L25).  Returns dict of counters (+ trace)."""
+        B = u.shape[0]
+        cnt = {k: torch.zeros(B, dtype=torch.int32, device="cuda") for k in ("n_eval", "n_oob", "n_expand", "n_shrink", "n_stuck")}
+        te = torch.zeros(B, n_steps, dtype=torch.int32, device="cuda") if trace else None
+        tl = torch.zeros(B, n_steps, dtype=torch.float64, device="cuda") if trace else None
+        self._check(lib().ns_slice_batch(self._h, _ptr(lc), _ptr(u), _ptr(logl), C.c_int64(B), C.c_double(logl_star), C.c_int32(n_steps),
+                                         C.c_uint64(seed), C.c_uint32(stream_id), C.c_int64(slot0), _ptr(cnt["n_eval"]),
+                                         _ptr(cnt["n_oob"]), _ptr(cnt["n_expand"]), _ptr(cnt["n_shrink"]), _ptr(cnt["n_stuck"]),
+                                         _ptr(te), _ptr(tl), _stream()), "ns_slice_batch")
+        out = dict(cnt)
+        if trace:
+            out["trace_evals"], out["trace_logl"] = te, tl
         return out
 
     # ---- sampler -----------------------------------------------------------------------------------

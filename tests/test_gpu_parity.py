@@ -711,6 +711,73 @@ def test_relbin_given_edges_and_errors(nsgw, c2):
         nsgw.Handle(spec1, smp1).relbin_setup(W.INJ_C3)                   # not a GW handle
 
 
+# ------------------------------------------------------------------------------------------------------
+# Hit-and-run slice sampling (R:L25): the same chains as the oracle on shared Philox streams
+# ------------------------------------------------------------------------------------------------------
+def _slice_compare(res_g, ug, lg, res_o, lstar):
+    """Walkers whose per-step evaluation counts all agree made the same decisions: identical counters, end points to rounding.
+    A walker may differ only where a candidate's logL sits within 1e-8 of L* (or a coordinate within 1e-12 of a bound)."""
+    te_g, te_o = res_g["trace_evals"].cpu().numpy(), res_o["trace_evals"]
+    clean = np.all(te_g == te_o, axis=1)
+    assert clean.mean() > 0.98, clean.mean()
+    for key in ("n_eval", "n_oob", "n_expand", "n_shrink", "n_stuck"):
+        assert np.array_equal(res_g[key].cpu().numpy()[clean], res_o[key][clean]), key
+    np.testing.assert_allclose(ug.cpu().numpy()[clean], res_o["u"][clean], rtol=0, atol=1e-11)
+    np.testing.assert_allclose(lg.cpu().numpy()[clean], res_o["logl"][clean], rtol=0, atol=1e-9 * max(1.0, abs(lstar)))
+    np.testing.assert_allclose(res_g["trace_logl"].cpu().numpy()[clean], res_o["trace_logl"][clean], rtol=0,
+                               atol=1e-9 * max(1.0, abs(lstar)))
+    return clean
+
+
+def test_slice_toy_and_shell_parity(nsgw):
+    for spec, lc_scale in ((W.config1()[0], 0.05), (W.shell_spec(6, [0, 1, 0, 0, 1, 0]), 0.2)):
+        P = O.OracleProblem(spec)
+        D = spec["ndim"]
+        h = nsgw.Handle(spec)
+        pts = O.draw_live(D, 300, 5)
+        ld = P.loglike_u(pts)
+        lstar = float(np.quantile(ld, 0.5))
+        keep = np.where(ld > lstar)[0][:97]
+        u0, l0 = pts[keep].copy(), ld[keep].copy()
+        rng = np.random.default_rng(3)
+        A = rng.normal(size=(D, D)) * lc_scale
+        Lc = np.linalg.cholesky(A @ A.T + 1e-4 * np.eye(D))
+        res_o = P.slice_walk(Lc, u0, l0, lstar, 12, 31337, (6 << 24) | 4, slot0=2, trace=True)
+        ug, lg = dev(u0), dev(l0)
+        res_g = h.slice_batch(dev(Lc), ug, lg, lstar, 12, 31337, (6 << 24) | 4, slot0=2, trace=True)
+        clean = _slice_compare(res_g, ug, lg, res_o, lstar)
+        assert clean.all()                                    # no transcendental in these likelihoods near a threshold
+        assert res_o["n_expand"].sum() > 0 and res_o["n_shrink"].sum() > 0
+
+
+@pytest.mark.parametrize("kind,dets", [(W.LIKE_TAYLORF2, ["H1", "L1"]), (W.LIKE_PHENOMD, ["H1", "L1", "V1"]), (W.LIKE_PHENOMD, ["L1"])])
+def test_slice_gw_parity(nsgw, kind, dets):
+    spec = W.gw_spec(kind, dets, 4.0, 256.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    P = O.OracleProblem(spec)
+    h = nsgw.Handle(spec)
+    rng = np.random.default_rng(17)
+    m, B, S = 250, 120, 6
+    u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+    pts = u_inj[None, :] + rng.normal(0, 1, (m, 11)) * np.array(W.C5_SIGMA) * 0.5
+    per = np.array(spec["periodic"], bool)
+    pts[:, per] -= np.floor(pts[:, per])
+    pts[:, ~per] = np.clip(pts[:, ~per], 1e-6, 1 - 1e-6)
+    ld = P.loglike_u(pts)
+    lstar = float(np.median(ld))
+    surv = pts[ld > lstar]
+    Lc = np.linalg.cholesky(np.cov(surv.T) + 1e-12 * np.eye(11))      # the live points' covariance, as a sampler would use it
+    start = rng.integers(0, len(surv), B)
+    u0, l0 = surv[start].copy(), ld[ld > lstar][start].copy()
+    res_o = P.slice_walk(Lc, u0, l0, lstar, S, 2024, (6 << 24) | 9, slot0=0, trace=True)
+    ug, lg = dev(u0), dev(l0)
+    res_g = h.slice_batch(dev(Lc), ug, lg, lstar, S, 2024, (6 << 24) | 9, slot0=0, trace=True)
+    _slice_compare(res_g, ug, lg, res_o, lstar)
+    te = res_o["trace_evals"]
+    assert te.min() >= 1 and te.max() > te.min() + 2           # the per-step cost really varies from walker to walker
+    assert np.all(res_o["logl"] > lstar)
+
+
 def test_error_codes(nsgw, c2):
     import ctypes as C
     h = nsgw.Handle(c2)
