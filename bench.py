@@ -314,6 +314,45 @@ def run_ours(args):
                                                 "wall_s_per_run": wall / len(hs)}
             for hh in hs:
                 hh.close()
+            # slice-sampling inner kernel against the acceptance walk from the same mid-run state of config 3:
+            # survivors as donors / covariance source, k = 500 replacements
+            hs3 = nsgw.Handle(spec3, smp3, seed=1)
+            for _ in range(40):
+                hs3.step(want_stats=False)
+            u_l, l_l = hs3.get_live()
+            order = torch.argsort(l_l)
+            kk = smp3["n_delete"]
+            donors = u_l[order[kk:]].contiguous()
+            ld = l_l[order[kk:]].contiguous()
+            lstar = float(l_l[order[kk - 1]])
+            lc = torch.linalg.cholesky(torch.cov(donors.T) + 1e-12 * torch.eye(11, dtype=torch.float64, device="cuda")).contiguous()
+            idx = torch.arange(kk, device="cuda") % donors.shape[0]
+            res = {}
+            for S_ in (11, 55):
+                uw, lw = donors[idx].clone(), ld[idx].clone()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                cnt = hs3.slice_batch(lc, uw, lw, lstar, S_, 777, (6 << 24) | 1, trace=True)
+                b.record(stream)
+                torch.cuda.synchronize()
+                ne = cnt["n_eval"].double()
+                te = cnt["trace_evals"].double()
+                res[f"S={S_}"] = {"ms": a.elapsed_time(b), "evals": int(ne.sum()), "evals_per_s": float(ne.sum()) / (a.elapsed_time(b) * 1e-3),
+                                  "evals_per_step_mean": float(te.mean()), "evals_per_step_std": float(te.std()),
+                                  "evals_per_step_max": int(te.max()), "evals_per_walker_min": int(ne.min()),
+                                  "evals_per_walker_max": int(ne.max()), "expand_per_step": float(cnt["n_expand"].double().mean()) / S_,
+                                  "shrink_per_step": float(cnt["n_shrink"].double().mean()) / S_, "stuck": int(cnt["n_stuck"].sum())}
+            uw, lw = donors[idx].clone(), ld[idx].clone()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            cw = hs3.walk_batch(donors, uw, lw, lstar, 5000, 777, 3)
+            b.record(stream)
+            torch.cuda.synchronize()
+            res["acceptance_walk_W=5000"] = {"ms": a.elapsed_time(b), "evals": int(cw["n_eval"].sum()),
+                                             "evals_per_s": float(cw["n_eval"].sum()) / (a.elapsed_time(b) * 1e-3),
+                                             "accept_mean": float(cw["n_accept"].double().mean())}
+            extras["slice_vs_walk_config3_midrun"] = res
+            hs3.close()
             # sequential limit: config 1 with k = 1 against the batched k = 50 (same n_live, same rule)
             spec1, smp1, logz_true = W.config1()
             seq = {}
