@@ -774,7 +774,40 @@ struct orc_state {
   double logx, logz, h, walks, delay;
   int64_t iter, n_eval_total;
   int threads;
+  int inner_kind = 0;   // 0 acceptance walk, 1 hit-and-run slice sampling (R:L25)
+  int n_slice = 0;      // slice steps per replacement
 };
+
+// Lower-triangular factor of the covariance of m points (unit-cube coordinates, free dims; FIXED dims get zero rows), the
+// direction factor of the slice kernel inside the sampler (R:L25): mean and covariance by sequential sums over the points in the
+// order given, 1/(m-1) normalisation, diagonal times (1 + 1e-12), textbook row-by-row Cholesky.  Lc [D][D] row-major.
+void orc_live_cholesky(const orc_problem* p, const double* pts, int32_t m, double* Lc) {
+  const int D = p->ndim;
+  double mean[16], C[16][16];
+  for (int a = 0; a < D; ++a) {
+    double acc = 0.0;
+    for (int i = 0; i < m; ++i) acc += pts[(size_t)i * D + a];
+    mean[a] = acc / m;
+  }
+  for (int a = 0; a < D; ++a)
+    for (int b = 0; b <= a; ++b) {
+      double acc = 0.0;
+      for (int i = 0; i < m; ++i) acc += (pts[(size_t)i * D + a] - mean[a]) * (pts[(size_t)i * D + b] - mean[b]);
+      C[a][b] = acc / (m - 1);
+    }
+  for (int a = 0; a < D * D; ++a) Lc[a] = 0.0;
+  for (int a = 0; a < D; ++a) {
+    if (p->prior_kind[a] == PRIOR_FIXED) continue;
+    for (int b = 0; b <= a; ++b) {
+      if (p->prior_kind[b] == PRIOR_FIXED) continue;
+      double sum = (a == b) ? C[a][a] * (1.0 + 1e-12) : C[a][b];
+      for (int c = 0; c < b; ++c) sum -= Lc[a * D + c] * Lc[b * D + c];
+      Lc[a * D + b] = (a == b) ? std::sqrt(sum) : sum / Lc[b * D + b];
+    }
+  }
+}
+
+void orc_state_set_inner(struct orc_state* s, int32_t kind, int32_t n_slice);
 
 orc_state* orc_state_create(const orc_problem* p, const orc_sampler_cfg* c, const double* live_u, uint64_t seed, int threads) {
   orc_state* s = new orc_state();
@@ -792,6 +825,7 @@ orc_state* orc_state_create(const orc_problem* p, const orc_sampler_cfg* c, cons
 }
 
 void orc_state_free(orc_state* s) { delete s; }
+void orc_state_set_inner(orc_state* s, int32_t kind, int32_t n_slice) { s->inner_kind = kind; s->n_slice = n_slice; }
 
 void orc_state_get_live(const orc_state* s, double* u, double* logl) {
   std::memcpy(u, s->u.data(), sizeof(double) * s->u.size());
@@ -858,6 +892,17 @@ void orc_step(orc_state* s, orc_stats* st, double* dead) {
     cl[j] = survl[sj];
   }
   std::vector<int32_t> na(k), ne(k), no(k);
+  const bool slice = s->inner_kind == 1;
+  if (slice) {
+    // R:L25 inside the sampler: directions from the survivors' covariance, n_slice steps per replacement, no walk-length adaptation
+    std::vector<double> Lc((size_t)D * D);
+    orc_live_cholesky(&s->prob, surv.data(), m, Lc.data());
+    std::vector<int32_t> nk(k);
+    W = s->n_slice;
+    orc_slice_walk(&s->prob, Lc.data(), cu.data(), cl.data(), k, lstar, W, s->seed, (0u << 24) | it24, 0, ne.data(), no.data(), nullptr,
+                   nullptr, nk.data(), nullptr, nullptr, s->threads);
+    for (int j = 0; j < k; ++j) na[j] = W - nk[j];      // steps that moved the point
+  } else
   orc_walk(&s->prob, surv.data(), m, cu.data(), cl.data(), k, lstar, W, s->seed, (0u << 24) | it24, 0, na.data(), ne.data(), no.data(),
            nullptr, nullptr, s->threads);
   // (5) write back into the dead slots
@@ -875,7 +920,7 @@ void orc_step(orc_state* s, orc_stats* st, double* dead) {
   }
   double amean = (double)sa / k;
   double r = std::max(0.5, amean) / W;
-  s->walks = std::min((s->walks * s->delay + s->cfg.naccept / r) / (s->delay + 1.0), (double)s->cfg.maxmcmc);
+  if (!slice) s->walks = std::min((s->walks * s->delay + s->cfg.naccept / r) / (s->delay + 1.0), (double)s->cfg.maxmcmc);
   s->n_eval_total += se;
   // (7) termination quantities (R:L18)
   double lmax = NEG_INF, lse = NEG_INF;

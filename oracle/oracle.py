@@ -168,6 +168,12 @@ class OracleProblem:
     def relbin(self, theta0, chi=1.0, eps=0.5):
         return OracleRelBin(self, theta0, chi, eps)
 
+    def live_cholesky(self, pts):
+        pts = _f64(pts).reshape(-1, self.ndim)
+        Lc = np.zeros((self.ndim, self.ndim))
+        _lib.orc_live_cholesky(C.byref(self.p), _dp(pts), C.c_int32(pts.shape[0]), _dp(Lc))
+        return Lc
+
     def use_relbin(self, rb):
         """Routes loglike_u, walk and the sampler through the relative-binning likelihood `rb` (None: back to the exact one)."""
         self._rb_in_use = rb                      # keep it alive
@@ -215,6 +221,10 @@ class OracleSampler:
         if getattr(self, "h", None) and _lib is not None:
             _lib.orc_state_free(self.h)
             self.h = None
+
+    def use_slice_kernel(self, n_slice):
+        """Replacements by n_slice hit-and-run slice steps (R:L25) instead of the acceptance walk (n_slice = 0: back to the walk)."""
+        _lib.orc_state_set_inner(self.h, C.c_int32(1 if n_slice > 0 else 0), C.c_int32(n_slice))
 
     def live(self):
         u = np.empty((self.n_live, self.ndim))

@@ -94,3 +94,52 @@ def test_slice_same_seed_same_chain_and_slot_keys_the_stream():
     assert len({tuple(r) for r in a["u"]}) == 8           # same start, different slots: different chains
     c = P.slice_walk(np.eye(4) * 0.2, u0[3:5], l0[3:5], -0.3, 10, 9, 3, slot0=3)
     assert np.array_equal(c["u"], a["u"][3:5])            # the chain depends on the slot, not on the batch it is in
+
+
+def test_live_cholesky_is_the_factor_of_the_sample_covariance():
+    spec = W.shell_spec(5)
+    spec["prior_kind"] = [W.UNIFORM, W.UNIFORM, W.FIXED, W.UNIFORM, W.UNIFORM]
+    P = O.OracleProblem(spec)
+    rng = np.random.default_rng(1)
+    A = rng.normal(size=(5, 5))
+    pts = 0.5 + 0.05 * rng.normal(size=(400, 5)) @ A.T
+    Lc = P.live_cholesky(pts)
+    free = [0, 1, 3, 4]
+    C = np.cov(pts.T)[np.ix_(free, free)]
+    np.testing.assert_allclose((Lc @ Lc.T)[np.ix_(free, free)], C, rtol=1e-9, atol=1e-15)
+    assert np.all(Lc[2] == 0) and np.all(Lc[:, 2] == 0) and np.allclose(Lc, np.tril(Lc))
+    np.testing.assert_allclose(Lc[np.ix_(free, free)], np.linalg.cholesky(C), rtol=1e-8, atol=1e-14)
+
+
+def test_slice_sampler_gaussian_logz_closed_form_and_shrinkage():
+    """The whole sampler with the slice kernel inside (directions from the survivors' covariance): config-1 evidence against the
+    closed form, and the cube-shell volume law E[log X] (BJ pins of the acceptance-walk sampler, repeated for this kernel)."""
+    spec, smp, ref = W.config1()
+    P = O.OracleProblem(spec)
+    pulls = []
+    for seed in range(1, 7):
+        S = O.OracleSampler(P, smp["n_live"], smp["n_delete"], smp["naccept"], smp["maxmcmc"], smp["walks0"], smp["delay"], seed=seed)
+        S.use_slice_kernel(20)
+        n, st = S.run(0, 0.01, 500)
+        logz, err, _ = S.finalize()
+        assert st["walk_len"] == 20 and st["accept_min"] >= 19      # every slice step moves the point
+        pulls.append((logz - ref["logz_exact"]) / err)
+    pulls = np.array(pulls)
+    assert np.all(np.abs(pulls) < 3.5) and abs(pulls.mean()) < 1.5, pulls
+    # cube shells: the true volume of each dead point is (2r)^D
+    D = 6
+    sspec = W.shell_spec(D)
+    Ps = O.OracleProblem(sspec)
+    bias = []
+    for seed in range(1, 5):
+        S = O.OracleSampler(Ps, 400, 200, 10, 500, 20.0, -1.0, seed=seed)
+        S.use_slice_kernel(12)
+        tot = []
+        for it in range(12):
+            st, dead = S.step(want_dead=True)
+            r = -dead[:, D]
+            logx_true = D * np.log(2 * r)
+            logx_est = dead[:, D + 1] - np.log(-np.expm1(-1.0 / dead[:, D + 2]))     # logw = logX_prev + log(1 - e^{-1/n})
+            tot.append(np.mean(logx_est - logx_true))
+        bias.append(np.mean(tot[4:]))
+    assert abs(np.mean(bias)) < 0.12, bias
