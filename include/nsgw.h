@@ -201,6 +201,13 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * / ns_walk_batch / ns_loglike_u_batch.  Setting it re-evaluates the live points' logL with the chosen likelihood (default
  * stream, synchronises); do so again after a new ns_relbin_setup. */
 #define NSGW_OPT_LIKELIHOOD 2
+/* key NSGW_OPT_INNER_KERNEL: what ns_step / ns_run replace the deleted points with: 0 = the acceptance walk (default; the paper's
+ * kernel), 1 = hit-and-run slice sampling (R:L25): direction factor = Cholesky factor of the covariance of the surviving live
+ * points (recomputed on the device every iteration), NSGW_OPT_SLICE_STEPS steps per replacement (key 4; 0 = 5 per non-FIXED
+ * dimension), no walk-length adaptation; ns_stats then reports walk_len = the number of slice steps and accept_* = the steps that
+ * moved the point.  Exact likelihood only. */
+#define NSGW_OPT_INNER_KERNEL 3
+#define NSGW_OPT_SLICE_STEPS 4
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */

@@ -93,8 +93,9 @@ __global__ void k_writeback(const int* __restrict__ order, int k, int D, const d
 }
 
 // Batch-level adaptation (R:L13-L15) and termination quantities (R:L18).  Single CTA, fixed-order reductions.
+// fixed_w > 0 (slice kernel): report that many steps per replacement and leave the walk length alone.
 __global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __restrict__ ne, const int* __restrict__ no, int k,
-                        const double* __restrict__ logl, int n) {
+                        const double* __restrict__ logl, int n, int fixed_w) {
   __shared__ long long s_a[256], s_e[256], s_o[256], s_s[256];
   __shared__ int s_min[256], s_max[256];
   __shared__ double s_d[256];
@@ -129,10 +130,10 @@ __global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __r
     __syncthreads();
   }
   if (t == 0) {
-    const int W = st->W;
+    const int W = fixed_w > 0 ? fixed_w : st->W;
     double amean = (double)s_a[0] / k;
     double r = fmax(0.5, amean) / W;
-    double walks = fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
+    double walks = fixed_w > 0 ? st->walks : fmin((st->walks * st->delay + st->naccept / r) / (st->delay + 1.0), (double)st->maxmcmc);
     st->walks = walks;
     st->n_eval_total += s_e[0];
     double lse = lmax + log(s_d[0]);

@@ -9,17 +9,20 @@ struct SliceArgs {
   double* logl;          // [B] in/out
   long long B;
   double lstar;
+  const double* lstar_dev;     // if non-null overrides lstar (ns_step)
+  const long long* iter_dev;   // if non-null: stream_id |= (*iter & 0xFFFFFF)
   int S;                 // slice steps per walker
   uint32_t k0, k1, stream_id;
   long long slot0;
   int* n_eval; int* n_oob; int* n_expand; int* n_shrink; int* n_stuck;
+  int* n_moved;                   // optional: S - n_stuck (what the sampler's statistics call accepted steps)
   int* t_evals; double* t_logl;   // optional trace [B, S]
 };
 
 constexpr int kSliceMaxExpand = 32, kSliceMaxShrink = 64;
 
 // Direction of step s of walker `slot`: z ~ N(0, I) over the free dims (Box-Muller, Philox blocks 0..7), dir = Lc z / |z|.
-__device__ __forceinline__ void slice_direction(const DevCfg& cfg, const SliceArgs& a, uint32_t s, uint32_t slot, double* dir) {
+__device__ __forceinline__ void slice_direction(const DevCfg& cfg, const SliceArgs& a, uint32_t sid, uint32_t s, uint32_t slot, double* dir) {
   const int D = cfg.ndim;
   int fr[kMaxDim], nfree = 0;
   for (int d = 0; d < D; ++d)
@@ -27,7 +30,7 @@ __device__ __forceinline__ void slice_direction(const DevCfg& cfg, const SliceAr
   double z[kMaxDim];
   for (int i = 0; 2 * i < nfree; ++i) {
     uint32_t w[4];
-    philox4x32_10((uint32_t)i, s, slot, a.stream_id, a.k0, a.k1, w);
+    philox4x32_10((uint32_t)i, s, slot, sid, a.k0, a.k1, w);
     const double U1 = u01(w[0], w[1]), U2 = u01(w[2], w[3]);
     const double rad = sqrt(-2.0 * log(U1));
     z[2 * i] = rad * cos(2.0 * kPi * U2);
@@ -57,9 +60,9 @@ __device__ __forceinline__ bool slice_point(const DevCfg& cfg, const double* x, 
   return inb;
 }
 
-__device__ __forceinline__ double slice_shrink_uniform(const SliceArgs& a, uint32_t s, uint32_t slot, int k) {
+__device__ __forceinline__ double slice_shrink_uniform(const SliceArgs& a, uint32_t sid, uint32_t s, uint32_t slot, int k) {
   uint32_t w[4];
-  philox4x32_10(9u + (uint32_t)(k / 2), s, slot, a.stream_id, a.k0, a.k1, w);
+  philox4x32_10(9u + (uint32_t)(k / 2), s, slot, sid, a.k0, a.k1, w);
   return (k % 2 == 0) ? u01(w[0], w[1]) : u01(w[2], w[3]);
 }
 
@@ -70,27 +73,29 @@ __global__ void k_slice_simple(const DevCfg* __restrict__ cfgp, SliceArgs a) {
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const uint32_t slot = (uint32_t)(a.slot0 + row);
+  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
+  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
   double x[kMaxDim], y[kMaxDim], dir[kMaxDim];
   for (int d = 0; d < D; ++d) x[d] = a.u[row * D + d];
   double xl = a.logl[row];
   int ne = 0, no = 0, nx = 0, ns = 0, nk = 0;
   for (int s = 0; s < a.S; ++s) {
     const int ne0 = ne;
-    slice_direction(cfg, a, (uint32_t)s, slot, dir);
+    slice_direction(cfg, a, sid, (uint32_t)s, slot, dir);
     auto inside = [&](double t, double& lt) -> bool {
       if (!slice_point(cfg, x, dir, t, y)) { ++no; return false; }
       lt = simple_loglike(cfg, y);
       ++ne;
-      return lt > a.lstar;
+      return lt > lstar;
     };
     uint32_t w8[4];
-    philox4x32_10(8u, (uint32_t)s, slot, a.stream_id, a.k0, a.k1, w8);
+    philox4x32_10(8u, (uint32_t)s, slot, sid, a.k0, a.k1, w8);
     double l = -u01(w8[0], w8[1]), r = l + 1.0, tmp;
     for (int k = 0; k < kSliceMaxExpand && inside(l, tmp); ++k) { l -= 1.0; ++nx; }
     for (int k = 0; k < kSliceMaxExpand && inside(r, tmp); ++k) { r += 1.0; ++nx; }
     bool moved = false;
     for (int k = 0; k < kSliceMaxShrink; ++k) {
-      const double t = l + slice_shrink_uniform(a, (uint32_t)s, slot, k) * (r - l);
+      const double t = l + slice_shrink_uniform(a, sid, (uint32_t)s, slot, k) * (r - l);
       double lt;
       if (inside(t, lt)) {
         for (int d = 0; d < D; ++d) x[d] = y[d];
@@ -111,6 +116,7 @@ __global__ void k_slice_simple(const DevCfg* __restrict__ cfgp, SliceArgs a) {
   if (a.n_expand) a.n_expand[row] = nx;
   if (a.n_shrink) a.n_shrink[row] = ns;
   if (a.n_stuck) a.n_stuck[row] = nk;
+  if (a.n_moved) a.n_moved[row] = a.S - nk;
 }
 
 // GW likelihoods: one CTA per walker.  Thread 0 runs the slice step's control flow; the likelihood of its candidate points is
@@ -135,6 +141,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
   const int tid = threadIdx.x;
   const long long row = blockIdx.x;
   const uint32_t wslot = (uint32_t)(a.slot0 + row);
+  const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
+  const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
   load_math_tables(&mtab, tb.mt, tid, NT);
   // thread 0's state
   double xl = 0.0, l = 0.0, r = 0.0, cand_t[PG] = {0.0, 0.0};
@@ -151,9 +159,9 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
     // ---- thread 0: next candidates
     if (tid == 0) {
       if (fresh) {          // new slice step: direction and bracket
-        slice_direction(cfg, a, (uint32_t)s, wslot, s_dir);
+        slice_direction(cfg, a, sid, (uint32_t)s, wslot, s_dir);
         uint32_t w8[4];
-        philox4x32_10(8u, (uint32_t)s, wslot, a.stream_id, a.k0, a.k1, w8);
+        philox4x32_10(8u, (uint32_t)s, wslot, sid, a.k0, a.k1, w8);
         l = -u01(w8[0], w8[1]); r = l + 1.0;
         mode = 0; kl = kr = ksh = 0; l_act = r_act = true; ne0 = ne; fresh = false;
       }
@@ -163,7 +171,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
         if (l_act) { cand_t[0] = l; s_flag[0] = slice_point(cfg, s_x, s_dir, l, s_y[0]) ? 2 : 0; }
         if (r_act) { cand_t[1] = r; s_flag[1] = slice_point(cfg, s_x, s_dir, r, s_y[1]) ? 2 : 0; }
       } else {
-        cand_t[0] = l + slice_shrink_uniform(a, (uint32_t)s, wslot, ksh) * (r - l);
+        cand_t[0] = l + slice_shrink_uniform(a, sid, (uint32_t)s, wslot, ksh) * (r - l);
         s_flag[0] = slice_point(cfg, s_x, s_dir, cand_t[0], s_y[0]) ? 2 : 0;
       }
     }
@@ -196,7 +204,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
         if (s_flag[c] == 0) { ++no; return false; }
         ++ne;
         lt = (s_flag[c] == 2) ? s_logl[c] : -INFINITY;
-        return lt > a.lstar;
+        return lt > lstar;
       };
       double lt = 0.0;
       bool done = false;
@@ -230,5 +238,42 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
     if (a.n_expand) a.n_expand[row] = nx;
     if (a.n_shrink) a.n_shrink[row] = ns;
     if (a.n_stuck) a.n_stuck[row] = nk;
+    if (a.n_moved) a.n_moved[row] = a.S - nk;
+  }
+}
+
+// Direction factor inside the sampler: lower-triangular Cholesky factor of the covariance of the m survivors (unit-cube
+// coordinates, free dims; FIXED dims get zero rows): sequential sums in the survivors' order, 1/(m-1), diagonal (1 + 1e-12).
+// One CTA: thread per dimension (means), thread per (a, b) pair (covariances), thread 0 (factorisation).
+__global__ void k_cov_chol(const DevCfg* __restrict__ cfgp, const double* __restrict__ pts, int m, double* Lc) {
+  __shared__ double mean[kMaxDim], C[kMaxDim][kMaxDim];
+  const DevCfg& cfg = *cfgp;
+  const int D = cfg.ndim, t = threadIdx.x;
+  if (t < D) {
+    double acc = 0.0;
+    for (int i = 0; i < m; ++i) acc += pts[(size_t)i * D + t];
+    mean[t] = acc / m;
+  }
+  __syncthreads();
+  if (t < D * D) {
+    const int a_ = t / D, b_ = t % D;
+    if (b_ <= a_) {
+      double acc = 0.0;
+      for (int i = 0; i < m; ++i) acc += (pts[(size_t)i * D + a_] - mean[a_]) * (pts[(size_t)i * D + b_] - mean[b_]);
+      C[a_][b_] = acc / (m - 1);
+    }
+  }
+  __syncthreads();
+  if (t == 0) {
+    for (int i = 0; i < D * D; ++i) Lc[i] = 0.0;
+    for (int a_ = 0; a_ < D; ++a_) {
+      if (cfg.prior_kind[a_] == 4) continue;
+      for (int b_ = 0; b_ <= a_; ++b_) {
+        if (cfg.prior_kind[b_] == 4) continue;
+        double sum = (a_ == b_) ? C[a_][a_] * (1.0 + 1e-12) : C[a_][b_];
+        for (int c = 0; c < b_; ++c) sum -= Lc[a_ * D + c] * Lc[b_ * D + c];
+        Lc[a_ * D + b_] = (a_ == b_) ? sqrt(sum) : sum / Lc[b_ * D + b_];
+      }
+    }
   }
 }

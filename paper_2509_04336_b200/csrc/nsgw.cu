@@ -81,6 +81,9 @@ struct ns_handle {
   double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [n_ranges][N][B]
   size_t partial_cap = 0;
   int n_sm = 148;
+  int opt_inner = 0;            // 0 acceptance walk, 1 hit-and-run slice sampling inside ns_step
+  int opt_slice_steps = 0;      // slice steps per replacement (0: 5 per free dimension)
+  double* d_lc = nullptr;       // slice kernel: direction factor [ndim][ndim]
   int opt_like = 0;             // 0 exact likelihood, 1 relative binning (sampler and ns_loglike_u_batch)
   int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
@@ -377,7 +380,7 @@ void ns_free(ns_handle* h) {
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
   cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
   if (h->s_own) cudaStreamDestroy(h->s_own);
-  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
+  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf); cudaFree(h->d_lc);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -508,6 +511,7 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
     INIT_CHECK(cudaMalloc(&h->d_cur_u, sizeof(double) * (size_t)k * D), -2);
     INIT_CHECK(cudaMalloc(&h->d_cur_l, sizeof(double) * (size_t)k), -2);
     INIT_CHECK(cudaMalloc(&h->d_cnt, sizeof(int) * 3 * (size_t)k), -2);
+    INIT_CHECK(cudaMalloc(&h->d_lc, sizeof(double) * (size_t)D * D), -2);
     if (live_u_dev) {
       INIT_CHECK(cudaMemcpyAsync(h->d_live_u, live_u_dev, sizeof(double) * (size_t)n * D, cudaMemcpyDeviceToDevice, s), -2);
     } else {
@@ -600,6 +604,24 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
 }  // extern "C"
 
 namespace {
+// Slice kernel launch (bin-less likelihoods: thread per walker; GW: CTA per walker).
+int launch_slice(ns_handle* h, const SliceArgs& a, cudaStream_t s) {
+  if (a.B == 0) return 0;
+  if (!is_gw(h->cfg.like_kind)) {
+    k_slice_simple<<<(unsigned)((a.B + 63) / 64), 64, 0, s>>>(h->d_cfg, a);
+    LAUNCH_CHECK(h);
+    return 0;
+  }
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  const int nd = h->cfg.n_det;
+#define SLICE_GW(M, N) k_slice_gw<M, N, 128><<<(unsigned)a.B, 128, 0, s>>>(h->d_cfg, h->tb, a)
+  if (tf2) { if (nd == 1) SLICE_GW(1, 1); else if (nd == 2) SLICE_GW(1, 2); else SLICE_GW(1, 3); }
+  else { if (nd == 1) SLICE_GW(2, 1); else if (nd == 2) SLICE_GW(2, 2); else SLICE_GW(2, 3); }
+#undef SLICE_GW
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
 // One nested-sampling iteration enqueued on stream s (no synchronisation, no host read-back).
 int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
   const int n = h->cfg.n_live, k = h->cfg.n_delete, D = h->cfg.ndim, m = n - k;
@@ -619,11 +641,27 @@ int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
   a.spec_fixed = h->opt_walk_spec > 0;
   a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
   a.n_accept = h->d_cnt; a.n_eval = h->d_cnt + k; a.n_oob = h->d_cnt + 2 * k;
-  int rc = launch_walk(h, a, s);
+  int rc = 0;
+  if (h->opt_inner == 1) {
+    // hit-and-run slice sampling (R:L25): directions from the survivors' covariance, a fixed number of steps, no adaptation
+    k_cov_chol<<<1, 256, 0, s>>>(h->d_cfg, h->d_surv, m, h->d_lc);
+    LAUNCH_CHECK(h);
+    SliceArgs sa;
+    memset(&sa, 0, sizeof(sa));
+    sa.Lc = h->d_lc; sa.u = h->d_cur_u; sa.logl = h->d_cur_l; sa.B = k;
+    sa.lstar_dev = &h->d_state->lstar; sa.iter_dev = &h->d_state->iter;
+    sa.S = h->opt_slice_steps > 0 ? h->opt_slice_steps : 5 * h->n_free;
+    sa.k0 = k0; sa.k1 = k1; sa.stream_id = 0u; sa.slot0 = 0;
+    sa.n_moved = h->d_cnt; sa.n_eval = h->d_cnt + k; sa.n_oob = h->d_cnt + 2 * k;
+    rc = launch_slice(h, sa, s);
+  } else {
+    rc = launch_walk(h, a, s);
+  }
   if (rc) return rc;
   k_writeback<<<(k + 127) / 128, 128, 0, s>>>(h->d_order, k, D, h->d_cur_u, h->d_cur_l, h->d_live_u, h->d_live_l);
   LAUNCH_CHECK(h);
-  k_adapt<<<1, 256, 0, s>>>(h->d_state, h->d_cnt, h->d_cnt + k, h->d_cnt + 2 * k, k, h->d_live_l, n);
+  k_adapt<<<1, 256, 0, s>>>(h->d_state, h->d_cnt, h->d_cnt + k, h->d_cnt + 2 * k, k, h->d_live_l, n,
+                            h->opt_inner == 1 ? (h->opt_slice_steps > 0 ? h->opt_slice_steps : 5 * h->n_free) : 0);
   LAUNCH_CHECK(h);
   return 0;
 }
@@ -645,19 +683,7 @@ int ns_slice_batch(ns_handle* h, const double* lc_dev, double* u_dev, double* lo
   a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32); a.stream_id = stream_id; a.slot0 = slot0;
   a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.n_expand = n_expand_dev; a.n_shrink = n_shrink_dev; a.n_stuck = n_stuck_dev;
   a.t_evals = trace_evals_dev; a.t_logl = trace_logl_dev;
-  if (!is_gw(h->cfg.like_kind)) {
-    k_slice_simple<<<(unsigned)((B + 63) / 64), 64, 0, s>>>(h->d_cfg, a);
-    LAUNCH_CHECK(h);
-    return 0;
-  }
-  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
-  const int nd = h->cfg.n_det;
-#define SLICE_GW(M, N) k_slice_gw<M, N, 128><<<(unsigned)B, 128, 0, s>>>(h->d_cfg, h->tb, a)
-  if (tf2) { if (nd == 1) SLICE_GW(1, 1); else if (nd == 2) SLICE_GW(1, 2); else SLICE_GW(1, 3); }
-  else { if (nd == 1) SLICE_GW(2, 1); else if (nd == 2) SLICE_GW(2, 2); else SLICE_GW(2, 3); }
-#undef SLICE_GW
-  LAUNCH_CHECK(h);
-  return 0;
+  return launch_slice(h, a, s);
 }
 
 int ns_step(ns_handle* h, ns_stats* stats_host, double* dead_dev, void* stream) {
@@ -860,6 +886,13 @@ int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (!h) return -3;
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
   if (key == NSGW_OPT_WALK_SPEC && value >= 0 && value <= kWalkDMax) { h->opt_walk_spec = value; return 0; }
+  if (key == NSGW_OPT_INNER_KERNEL && (value == 0 || value == 1)) {
+    if (value == 1 && h->opt_like == 1) return fail(h, -5, "the slice kernel evaluates the exact likelihood only");
+    h->opt_inner = value;
+    return 0;
+  }
+  if (key == NSGW_OPT_SLICE_STEPS && value >= 0) { h->opt_slice_steps = value; return 0; }
+  if (key == NSGW_OPT_LIKELIHOOD && value == 1 && h->opt_inner == 1) return fail(h, -5, "the slice kernel evaluates the exact likelihood only");
   if (key == NSGW_OPT_LIKELIHOOD && (value == 0 || value == 1)) {
     if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
     if (value == 1 && h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");

@@ -331,7 +331,7 @@ def _sorted_live(u, l):
     return u[o], l[o]
 
 
-def _step_parity(nsgw, spec, smp, nsteps, seed, tol_l, relbin_theta0=None):
+def _step_parity(nsgw, spec, smp, nsteps, seed, tol_l, relbin_theta0=None, slice_steps=0):
     """Step-for-step comparison on the same seed and live points.  Integer work (walk length, counters) must be identical;
     floating-point state agrees to rounding drift.  Near-tied logL (a gamma = 1 proposal from a donor lands on another donor
     to 1 ulp) may be ranked in either order, so live sets are compared as sets (sorted by logL), not slot by slot."""
@@ -344,6 +344,10 @@ def _step_parity(nsgw, spec, smp, nsteps, seed, tol_l, relbin_theta0=None):
     if relbin_theta0 is not None:
         h.relbin_setup(relbin_theta0)
         h.set_option(2, 1)
+    if slice_steps:
+        S.use_slice_kernel(slice_steps)                # both sides replace points by hit-and-run slice steps (R:L25)
+        h.set_option(4, slice_steps)
+        h.set_option(3, 1)
     D, k = spec["ndim"], smp["n_delete"]
     for it in range(nsteps):
         dead_g = torch.empty(k, D + 3, dtype=torch.float64, device="cuda")
@@ -709,6 +713,32 @@ def test_relbin_given_edges_and_errors(nsgw, c2):
     spec1, smp1, _ = W.config1()
     with pytest.raises(nsgw.NsgwError):
         nsgw.Handle(spec1, smp1).relbin_setup(W.INJ_C3)                   # not a GW handle
+
+
+def test_ns_step_parity_slice_kernel(nsgw):
+    # the sampler with the slice kernel inside (covariance factor computed on the device every iteration), step for step
+    spec, smp, _ = W.config1()
+    _step_parity(nsgw, spec, smp, 8, 13, 1e-10, slice_steps=9)
+    _step_parity(nsgw, W.shell_spec(5, [0, 1, 0, 0, 0]), dict(n_live=150, n_delete=50, naccept=10, maxmcmc=200, walks0=20.0, delay=-1.0),
+                 6, 14, 1e-12, slice_steps=7)
+    gspec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 128.0, (20.0, 40.0))
+    gspec = W.make_data(gspec, W.INJ_C3, 10.0, wf)
+    _step_parity(nsgw, gspec, dict(n_live=100, n_delete=50, naccept=8, maxmcmc=60, walks0=12.0, delay=-1.0), 3, 15, 1e-8, slice_steps=5)
+
+
+def test_slice_sampler_config1_closed_form_logz(nsgw):
+    spec, smp, ref = W.config1()
+    pulls = []
+    for seed in range(1, 9):
+        h = nsgw.Handle(spec, smp, seed=seed)
+        h.set_option(4, 20)
+        h.set_option(3, 1)
+        nit, st = h.run(smp["term_kind"], smp["term_tol"], 500)
+        assert st["walk_len"] == 20 and st["accept_min"] >= 19 and st["dlogz"] < smp["term_tol"]
+        logz, err, _ = h.finalize_evidence()
+        pulls.append((logz - ref["logz_exact"]) / err)
+    pulls = np.array(pulls)
+    assert np.all(np.abs(pulls) < 3.5) and abs(pulls.mean()) < 1.3, pulls
 
 
 # ------------------------------------------------------------------------------------------------------
