@@ -353,6 +353,19 @@ def run_ours(args):
                                              "accept_mean": float(cw["n_accept"].double().mean())}
             extras["slice_vs_walk_config3_midrun"] = res
             hs3.close()
+            # full config-3 run with the slice kernel inside the sampler (55 = 5 x 11 steps per replacement)
+            hsl = nsgw.Handle(spec3, smp3, seed=1)
+            hsl.set_option(4, 55)
+            hsl.set_option(3, 1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            nit, st = hsl.run(smp3["term_kind"], smp3["term_tol"], 4000)
+            logz, err, H = hsl.finalize_evidence()
+            wall = time.perf_counter() - t0
+            extras["ns_run_config3_slice"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
+                                              "logz_err": err, "H": H, "slice_steps": st["walk_len"], "moved_mean_last": st["accept_mean"],
+                                              "evals_per_s": st["n_eval_total"] / wall}
+            hsl.close()
             # sequential limit: config 1 with k = 1 against the batched k = 50 (same n_live, same rule)
             spec1, smp1, logz_true = W.config1()
             seq = {}

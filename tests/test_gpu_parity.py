@@ -726,6 +726,36 @@ def test_ns_step_parity_slice_kernel(nsgw):
     _step_parity(nsgw, gspec, dict(n_live=100, n_delete=50, naccept=8, maxmcmc=60, walks0=12.0, delay=-1.0), 3, 15, 1e-8, slice_steps=5)
 
 
+def test_slice_and_walk_kernels_agree_on_gw_evidence(nsgw):
+    """Two different inner kernels, one evidence: PhenomD-form, H1+L1, 20-512 Hz, SNR 12, free Mc, q, dL, tc (a problem on which
+    both chains mix: the walk reaches its naccept, the slice kernel moves at every step); three seeds each."""
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 512.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    free = (0, 1, 4, 8)
+    kinds, lo_, hi_ = list(spec["prior_kind"]), list(spec["prior_lo"]), list(spec["prior_hi"])
+    for d in range(11):
+        if d not in free:
+            kinds[d] = W.FIXED
+            lo_[d] = hi_[d] = W.INJ_C3[d]
+    spec["prior_kind"], spec["prior_lo"], spec["prior_hi"] = kinds, lo_, hi_
+    spec["periodic"] = [0] * 11
+    smp = dict(n_live=600, n_delete=300, naccept=30, maxmcmc=3000, walks0=60.0, delay=-1.0)
+    out = {}
+    for name, opts in (("walk", []), ("slice", [(4, 24), (3, 1)])):
+        zs, es = [], []
+        for seed in (1, 2, 3):
+            h = nsgw.Handle(spec, smp, seed=seed)
+            for k_, v_ in opts:
+                h.set_option(k_, v_)
+            h.run(0, 0.1, 2000)
+            z, e, _ = h.finalize_evidence()
+            zs.append(z)
+            es.append(e)
+        out[name] = (np.mean(zs), np.mean(es) / math.sqrt(3))
+    (zw, ew), (zs_, es_) = out["walk"], out["slice"]
+    assert abs(zw - zs_) < 3.5 * math.hypot(ew, es_), out
+
+
 def test_slice_sampler_config1_closed_form_logz(nsgw):
     spec, smp, ref = W.config1()
     pulls = []
