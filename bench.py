@@ -222,8 +222,8 @@ def run_ours(args):
         flops_launch = float(B) * n_freq * alg_flops_per_bin(n_det)
         ach = flops_launch / (kern_ms / kern_n * 1e-3) / 1e12
         # DRAM bytes per launch of the dominant kernel: dram__bytes_read.sum + dram__bytes_write.sum of the committed
-        # `ncu --set full` capture of this same command (profiles/r01x_k_bins_lp_ncu_full.txt); only valid for the default batch
-        traffic = (19319552 + 65280) if (B == 65536 and n_freq == 4017) else None
+        # `ncu --set full` capture of this same command (profiles/r01ad_k_bins_lp_ncu_full.txt); only valid for the default batch
+        traffic = (19319552 + 84992) if (B == 65536 and n_freq == 4017) else None
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
                 "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic 96 B x B = %d" % (96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
