@@ -122,7 +122,8 @@ __global__ void k_slice_simple(const DevCfg* __restrict__ cfgp, SliceArgs a) {
 // GW likelihoods: one CTA per walker.  Thread 0 runs the slice step's control flow; the likelihood of its candidate points is
 // evaluated by the whole CTA with the same machinery as k_walk_gw (per-candidate set-up by one lane each, then a bin sweep).
 // The two ends of the bracket are tested together while stepping out (their tests are independent given x and the direction, so
-// the evaluations, counters and results are those of the sequential statement); shrinkage candidates go one at a time.
+// the evaluations, counters and results are those of the sequential statement); shrinkage candidates go two at a time, the second
+// being the sequential statement's next draw under the assumption that the first is rejected (discarded, uncounted, otherwise).
 template <int MODEL, int NDET, int NT>
 __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restrict__ cfgp, Tables tb, SliceArgs a) {
   using AL = AccLayout<MODEL, NDET>;
@@ -171,8 +172,15 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
         if (l_act) { cand_t[0] = l; s_flag[0] = slice_point(cfg, s_x, s_dir, l, s_y[0]) ? 2 : 0; }
         if (r_act) { cand_t[1] = r; s_flag[1] = slice_point(cfg, s_x, s_dir, r, s_y[1]) ? 2 : 0; }
       } else {
+        // shrinkage, two candidates per round: the second is the one the sequential statement draws IF the first is rejected
+        // (the bracket end on the first one's side moves to it; the draw itself does not depend on any likelihood value)
         cand_t[0] = l + slice_shrink_uniform(a, sid, (uint32_t)s, wslot, ksh) * (r - l);
         s_flag[0] = slice_point(cfg, s_x, s_dir, cand_t[0], s_y[0]) ? 2 : 0;
+        if (ksh + 1 < kSliceMaxShrink) {
+          const double l2 = (cand_t[0] < 0.0) ? cand_t[0] : l, r2 = (cand_t[0] < 0.0) ? r : cand_t[0];
+          cand_t[1] = l2 + slice_shrink_uniform(a, sid, (uint32_t)s, wslot, ksh + 1) * (r2 - l2);
+          s_flag[1] = slice_point(cfg, s_x, s_dir, cand_t[1], s_y[1]) ? 2 : 0;
+        }
       }
     }
     __syncthreads();
@@ -212,13 +220,15 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_slice_gw(const DevCfg* __restr
         if (l_act) { if (outcome(0, lt)) { l -= 1.0; ++nx; if (++kl == kSliceMaxExpand) l_act = false; } else l_act = false; }
         if (r_act) { if (outcome(1, lt)) { r += 1.0; ++nx; if (++kr == kSliceMaxExpand) r_act = false; } else r_act = false; }
       } else {
-        if (outcome(0, lt)) {
-          for (int d = 0; d < D; ++d) s_x[d] = s_y[0][d];
-          xl = lt; done = true;
-        } else {
-          ++ns;
-          if (cand_t[0] < 0.0) l = cand_t[0]; else r = cand_t[0];
-          if (++ksh == kSliceMaxShrink) { ++nk; done = true; }
+        for (int c = 0; c < PG && !done && s_flag[c] >= 0; ++c) {      // in order; the second only if the first was rejected
+          if (outcome(c, lt)) {
+            for (int d = 0; d < D; ++d) s_x[d] = s_y[c][d];
+            xl = lt; done = true;
+          } else {
+            ++ns;
+            if (cand_t[c] < 0.0) l = cand_t[c]; else r = cand_t[c];
+            if (++ksh == kSliceMaxShrink) { ++nk; done = true; }
+          }
         }
       }
       if (done) {
