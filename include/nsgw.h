@@ -50,7 +50,7 @@ typedef struct {
   int32_t prior_kind[NSGW_MAX_DIM];    /* NSGW_PRIOR_* per dimension; FIXED dims take the value prior_lo */
   double prior_lo[NSGW_MAX_DIM], prior_hi[NSGW_MAX_DIM];
   int32_t periodic[NSGW_MAX_DIM];      /* 1 = wrap the unit-cube coordinate instead of rejecting */
-  int32_t n_det, n_freq;               /* GW: detectors (<= 4) and bins per detector */
+  int32_t n_det, n_freq;               /* GW: detectors (kernels are built for 1..3; 4 returns -5) and bins per detector */
   double f_min, df;                    /* f_k = f_min + k df, k = 0..n_freq-1 (both ends inclusive, R:L1) */
   double det_vertex[NSGW_MAX_DET][3];  /* Earth-fixed vertex position [m] */
   double det_xarm[NSGW_MAX_DET][3], det_yarm[NSGW_MAX_DET][3]; /* arm unit vectors */
