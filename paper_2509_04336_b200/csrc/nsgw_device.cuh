@@ -336,7 +336,8 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   cb[CB_VALID] = 1.0;
 
   const double eta = q / ((1.0 + q) * (1.0 + q));
-  const double M = Mc * kGMsunS * pow(eta, -0.6);
+  // (powers as exp(c log x): half the dependent instructions of pow(), a few ulp -- this set-up is the serial latency of a walk chunk)
+  const double M = Mc * kGMsunS * exp(-0.6 * log(eta));
   const double m1 = M / (1.0 + q), m2 = M * q / (1.0 + q);
   const double delta = (m1 - m2) / M;
   const double chis = 0.5 * (chi1 + chi2), chia = 0.5 * (chi1 - chi2);
@@ -347,7 +348,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   sincos(dec, &sd, &cd);
   sincos(psi, &sp, &cp);
   const double ci = cos(iota);
-  const double A0 = sqrt(5.0 / 24.0) * pow(kPi, -2.0 / 3.0) * pow(Mc * kGMsunS, 5.0 / 6.0) / (dL * kMpcS);
+  const double A0 = 0.2127875101396634 /* sqrt(5/24) pi^-2/3 */ * exp((5.0 / 6.0) * log(Mc * kGMsunS)) / (dL * kMpcS);
   double tc0 = tc, dt0 = 0.0;   // tc0 = tc + dt of detector 0: the common phase carries detector 0's arrival time
   for (int d = 0; d < cfg.n_det; ++d) {
     DetResp r = detector_response(cfg, d, sg, cg, sd, cd, sp, cp);
@@ -406,8 +407,9 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   double af = 2.0 * sqrt(3.0) * eta - 3.871 * eta2 + 4.028 * eta3 + S;
   af = fmin(0.99, fmax(-0.99, af));
   const double Erad = 0.05597 * eta + 0.5810 * eta2 - 0.9607 * eta3 + 3.352 * eta2 * eta2;
-  const double Frd = (1.5251 - 1.1568 * pow(1.0 - af, 0.1292)) / (2.0 * kPi * (1.0 - Erad));
-  const double Qf = 0.7 + 1.4187 * pow(1.0 - af, -0.4990);
+  const double lg1af = log(1.0 - af);
+  const double Frd = (1.5251 - 1.1568 * exp(0.1292 * lg1af)) / (2.0 * kPi * (1.0 - Erad));
+  const double Qf = 0.7 + 1.4187 * exp(-0.4990 * lg1af);
   const double Fdamp = Frd / (2.0 * Qf);
   const double wF = gam3 * Fdamp;
   double Fpeak;
@@ -416,8 +418,8 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
 
   // -- phase pieces in F = M f and their connection (C0/C1 at 0.018 and Frd/2, analytic derivatives) --
   const double ieta = 1.0 / eta;
-  auto pn_phase = [&](double F, double& val, double& der) {
-    double v = cbrt(kPi * F), lv = log(v);
+  auto pn_phase = [&](double F, double& val, double& der) {   // only ever called at F = 0.018
+    const double v = 0.3838316585355026 /* cbrt(pi 0.018) */, lv = -0.957551211745524 /* ln of it */;
     double vk[8];
     vk[0] = 1.0;
 #pragma unroll
@@ -436,7 +438,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   };
   auto ins_phase = [&](double F, double& val, double& der) {
     pn_phase(F, val, der);
-    double F13 = cbrt(F), F23 = F13 * F13;
+    const double F13 = 0.26207413942088964 /* cbrt(0.018) */, F23 = F13 * F13;
     val += ieta * (sig1 * F + 0.75 * sig2 * F * F13 + 0.6 * sig3 * F * F23 + 0.5 * sig4 * F * F);
     der += ieta * (sig1 + sig2 * F13 + sig3 * F23 + sig4 * F);
   };
@@ -462,7 +464,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   mr_phase(Fpeak, vm, dm);
   const double t0 = dm + C2m;
 
-  const double M13 = cbrt(M), M23 = M13 * M13;
+  const double M13 = cv * 0.6827840632552957 /* pi^-1/3 */, M23 = M13 * M13;
   a[4] = -0.25 * kPi - 2.0 * phic + e5 * (c5 + 3.0 * c5 * lncv);
   a[9] = 2.0 * kPi * tc0 + (sig1 * ieta - t0) * M;
   a[10] = 0.75 * sig2 * ieta * M * M13;
@@ -470,7 +472,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   a[12] = 0.5 * sig4 * ieta * M * M;
 #pragma unroll
   for (int i = 0; i < 13; ++i) cb[CB_PH + i] = a[i] * kQT;
-  cb[CB_PB + 0] = (bet2 * ieta * log(M) + C1i - 2.0 * phic) * kQT;
+  cb[CB_PB + 0] = (bet2 * ieta * (3.0 * lncv - 1.1447298858494002 /* ln pi */) + C1i - 2.0 * phic) * kQT;
   cb[CB_PB + 1] = bet2 * ieta * kQT;
   cb[CB_PB + 2] = ((bet1 * ieta + C2i - t0) * M + 2.0 * kPi * tc0) * kQT;
   cb[CB_PB + 3] = -bet3 * ieta / (3.0 * M * M * M) * kQT;
@@ -518,7 +520,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   const double F1 = 0.014;
   double v1, d1;
   {
-    double x1 = cbrt(F1 / M);  // x at the junction: f^1/3
+    double x1 = 0.241014226417523 /* cbrt(0.014) */ / M13;  // x at the junction: f^1/3
     double p = 0.0, dp = 0.0;
 #pragma unroll
     for (int i = 9; i >= 0; --i) { dp = dp * x1 + p; p = p * x1 + ai[i]; }
