@@ -162,7 +162,7 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 #define NSGW_LP_OCC 3
 #endif
 constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
-constexpr long long kLpMinBatch = 2048;   // below this the CTA-per-particle kernel fills the machine better
+constexpr long long kLpMinBatch = 1024;   // below this the CTA-per-particle kernel fills the machine better
 
 int ensure_partial(ns_handle* h, size_t n) {
   if (n > h->partial_cap) {
@@ -180,14 +180,18 @@ int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaS
   constexpr int NT = kLpNT, PP = kLpPP;
   const long long ngroups = (B + NT * PP - 1) / (NT * PP);
   const long long grid_max = (long long)h->n_sm * kLpOCC;
-  // bins per task (multiple of the unroll, 32..256): the value that minimises rounds x (bins per task + per-task overhead),
-  // rounds = ceil(tasks / resident CTAs) -- large tiles amortise the per-task set-up, small ones balance the last round
+  // bins per task (multiple of the unroll, 32..256): the value that minimises rounds x (bins per task + per-task overhead) x
+  // slow-down from sharing the SM, rounds = ceil(tasks / resident CTAs) -- large tiles amortise the per-task set-up, small ones
+  // balance the last round; one CTA alone on an SM already runs at ~85 % of the FP64 pipe, so co-resident CTAs divide it
+  // (this is what makes few, long tasks the better choice for small batches), plus k_finish's cost per range
   int kr = kLpKR;
   {
     double best = 1e300;
     for (int c = 32; c <= kLpKR; c += kLpUNR) {
-      const long long nt = ngroups * ((h->cfg.n_freq + c - 1) / c);
-      const double cost = (double)((nt + grid_max - 1) / grid_max) * (c + 8);
+      const int nr = (h->cfg.n_freq + c - 1) / c;
+      const long long nt = ngroups * nr;
+      const long long per_sm = std::min<long long>(kLpOCC, (nt + h->n_sm - 1) / h->n_sm);
+      const double cost = (double)((nt + grid_max - 1) / grid_max) * (c + 8) * std::max(1.0, 0.85 * per_sm) + 0.25 * nr;
       if (cost < best - 1e-9) { best = cost; kr = c; }
     }
   }
