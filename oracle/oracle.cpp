@@ -26,6 +26,11 @@
 //   evidence ................. eq. 3-5 shrinkage sum, Gaussian closed-form logZ, 2-D quadrature
 //   top-k .................... numpy stable argsort
 //   full 11-D runs ........... statistical only (exact parity unpinned by nature)
+//   relative binning (R:L24) . exact along constant-ratio directions, partition of <d,h0>/<h0,h0>, second-order time-shift bound,
+//                              error / 4 per halving of eps (tests/test_oracle_relbin.py)
+//   slice kernel (R:L25) ..... uniformity in cube shells and Gaussian ellipsoids from a single start (closed-form laws), sample
+//                              covariance factor against numpy, config-1 evidence and shell volumes with it inside the sampler
+//                              (tests/test_oracle_slice.py)
 
 #include <cmath>
 #include <cstdint>
