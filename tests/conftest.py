@@ -16,3 +16,10 @@ def pytest_configure(config):
 def oracle_mod():
     from oracle import oracle as O
     return O
+
+
+def pytest_sessionstart(session):
+    # a fresh checkout has no libnsgw.so (built files are git-ignored): build it once, in-tree, before any test loads it
+    from paper_2509_04336_b200 import build
+    if os.path.exists(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")):
+        build.build()
