@@ -2,8 +2,11 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
 It imports nothing from paper_2509_04336_b200 (the CUDA path) and the CUDA path imports nothing from here.
-Every function is a thin call into oracle.cpp, whose header lists what pins each part.
+Every function is a thin call into oracle.cpp, whose header lists what pins each part, except the posterior weights at the
+end of this file (reading R:L26), written out here in NumPy/math.fsum and pinned by tests/test_oracle_posterior.py.
 """
+import math
+
 import ctypes as C
 import numpy as np
 
@@ -342,3 +345,49 @@ def evidence_update(logl_i, n_i, logx, logz, h):
 
 def neff(n, k):
     return _lib.orc_neff(C.c_int32(n), C.c_int32(k))
+
+
+# ---- posterior weights ("posterior samples as a natural by-product", "weights ... calculated using the prior volumes
+#      enclosed between successive dead points and the likelihoods"; DESIGN reading R:L26) ---------------------------------------
+def posterior_rows(dead, live_u, live_logl, logx):
+    """The sample set of a run: the recorded dead points ([n_dead, D+3] rows u.., logL, log w, n_i as orc_step writes them)
+    followed by the live points in ascending logL, whose widths continue the shrinkage from logx with n_i = n, n-1, .., 1
+    (R:L17: log w_i = logX_{i-1} + log(1 - exp(-1/n_i)), logX_i = logX_{i-1} - 1/n_i).  Returns u [N, D], logL [N], log w [N]."""
+    live_u = _f64(live_u)
+    live_logl = _f64(live_logl)
+    n, D = live_u.shape
+    dead = np.zeros((0, D + 3)) if dead is None else _f64(dead).reshape(-1, D + 3)
+    order = argsort(live_logl)
+    lw = np.empty(n)
+    lx = float(logx)
+    for j in range(n):
+        nj = float(n - j)
+        lw[j] = lx + math.log(-math.expm1(-1.0 / nj))
+        lx -= 1.0 / nj
+    u = np.concatenate([dead[:, :D], live_u[order]])
+    logl = np.concatenate([dead[:, D], live_logl[order]])
+    logw = np.concatenate([dead[:, D + 1], lw])
+    return u, logl, logw
+
+
+def posterior_weights(logl, logw):
+    """log p_i = logL_i + log w_i - logZ with logZ = log sum_i L_i w_i over the rows (R:L26).  Returns (log p, logZ)."""
+    t = _f64(logl) + _f64(logw)
+    m = float(np.max(t))
+    logz = m + math.log(math.fsum(np.exp(t - m).tolist()))
+    return t - logz, logz
+
+
+def posterior(prob, dead, live_u, live_logl, logx, theta_ref=None):
+    """Weighted posterior sample of a run (R:L26): theta = prior transform of every row, log p, logZ over the rows, Kish's
+    effective sample size 1 / sum p_i^2 and, for a reference point, the credible level of each parameter
+    CL_d = sum_i p_i [theta_i,d < theta_ref,d] (the statistic a PP test histograms)."""
+    u, logl, logw = posterior_rows(dead, live_u, live_logl, logx)
+    logp, logz = posterior_weights(logl, logw)
+    theta = prob.prior_transform(u)
+    pw = np.exp(logp)
+    out = {"theta": theta, "logp": logp, "logz": logz, "ess": 1.0 / math.fsum((pw * pw).tolist())}
+    if theta_ref is not None:
+        ref = _f64(theta_ref)
+        out["cl"] = np.array([math.fsum(pw[theta[:, d] < ref[d]].tolist()) for d in range(theta.shape[1])])
+    return out
