@@ -175,6 +175,19 @@ int ns_get_live(ns_handle* h, double* u_dev, double* logl_dev, void* stream);
 /* Adds the remaining live points (n_i = n, n-1, .., 1; R:L17) to a copy of the accumulators.  Synchronises. */
 int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host, double* h_host, void* stream);
 
+/* Weighted posterior sample of a run ("posterior samples as a natural by-product"; "weights ... calculated using the
+ * prior volumes enclosed between successive dead points and the likelihoods"; DESIGN reading R:L26).  Rows: the n_dead rows of
+ * dead_dev ([n_dead, ndim+3] device, as ns_step / ns_run wrote them; may be NULL when n_dead = 0) followed by the handle's
+ * n_live live points in ascending logL, whose widths continue the shrinkage with n_i = n, n-1, .., 1 (R:L17).  N = n_dead + n_live.
+ * theta_dev [N, ndim] (device, optional) receives the prior transform of every row; logp_dev [N] (device, required) the
+ * normalised log posterior weight logL_i + log w_i - logZ, logZ = log sum_i L_i w_i over the rows.  summary_host (optional,
+ * [2 + ndim] host doubles; the call synchronises iff it is given): logZ, Kish's effective sample size 1 / sum p_i^2, and per
+ * parameter the credible level sum_i p_i [theta_i,d < theta_ref_host[d]] of a reference point (host, [ndim], physical
+ * parameters; optional, needs theta_dev; NaN when absent) -- the statistic a PP test histograms.  The handle's sampler
+ * state is not changed.  Errors: -1 bad arguments, -3 no live set. */
+int ns_posterior(ns_handle* h, const double* dead_dev, int64_t n_dead, double* theta_dev, double* logp_dev,
+                 const double* theta_ref_host, double* summary_host, void* stream);
+
 /* Device FP64 FMA throughput probe used for the roofline denominator: runs `iters` dependent-chain DFMAs x 8 chains per
  * thread on a full grid and returns achieved TFLOP/s in *tflops_host (synchronises; timed with CUDA events). */
 int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream);

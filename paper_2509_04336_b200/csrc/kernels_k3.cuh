@@ -150,12 +150,85 @@ __global__ void k_adapt(DevState* st, const int* __restrict__ na, const int* __r
 }
 
 // Final evidence: adds the live points with n_i = n..1 to a copy of the accumulators (R:L17).  out: logz, h.
+// lw_out (optional) [n]: the width log w of each live point in ascending-logL order (the rows R:L26 appends to the dead points).
 __global__ void k_finalize(const DevState* __restrict__ st, const double* __restrict__ logl, const int* __restrict__ order, int n,
-                           double* out) {
+                           double* out, double* lw_out) {
   if (threadIdx.x != 0 || blockIdx.x != 0) return;
   double logx = st->logx, logz = st->logz, h = st->h, lw;
-  for (int i = 0; i < n; ++i) evidence_update(logl[order[i]], (double)(n - i), logx, logz, h, lw);
+  for (int i = 0; i < n; ++i) {
+    evidence_update(logl[order[i]], (double)(n - i), logx, logz, h, lw);
+    if (lw_out) lw_out[i] = lw;
+  }
   out[0] = logz; out[1] = h;
+}
+
+// Posterior rows (R:L26): the recorded dead points followed by the live points in ascending logL.  theta
+// (optional) [N, D] = prior transform of each row; t [N] = logL + log w.
+__global__ void k_post_rows(const DevCfg* __restrict__ cfg, const double* __restrict__ dead, long long n_dead,
+                            const double* __restrict__ live_u, const double* __restrict__ live_l, const int* __restrict__ order,
+                            const double* __restrict__ lw_live, int n, double* theta, double* t) {
+  const long long r = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (r >= n_dead + n) return;
+  const int D = cfg->ndim;
+  const double* u;
+  double l, w;
+  if (r < n_dead) {
+    const double* row = dead + (size_t)r * (D + 3);
+    u = row; l = row[D]; w = row[D + 1];
+  } else {
+    const int j = (int)(r - n_dead), id = order[j];
+    u = live_u + (size_t)id * D; l = live_l[id]; w = lw_live[j];
+  }
+  if (theta)
+    for (int d = 0; d < D; ++d)
+      theta[(size_t)r * D + d] = prior_transform_dim(cfg->prior_kind[d], cfg->prior_lo[d], cfg->prior_hi[d], u[d]);
+  t[r] = l + w;
+}
+
+constexpr int kPostThreads = 1024;
+
+// Fixed-order sum (or maximum) over the CTA: strided partials, then a binary tree in shared memory.
+template <bool MAX>
+__device__ __forceinline__ double post_reduce(double v, double* red) {
+  __syncthreads();
+  red[threadIdx.x] = v;
+  __syncthreads();
+  for (int s = kPostThreads / 2; s > 0; s >>= 1) {
+    if ((int)threadIdx.x < s) red[threadIdx.x] = MAX ? fmax(red[threadIdx.x], red[threadIdx.x + s]) : red[threadIdx.x] + red[threadIdx.x + s];
+    __syncthreads();
+  }
+  return red[0];
+}
+
+// Normalises t in place to log p = t - logZ, logZ = log sum exp t (R:L26), and reduces the summaries: out[0] = logZ,
+// out[1] = 1 / sum p^2, out[2 + d] = sum p [theta_d < ref_d] (NaN without a reference point).  One CTA, fixed order.
+__global__ void __launch_bounds__(kPostThreads) k_post_norm(double* t, long long N, const double* __restrict__ theta, int D,
+                                                            const double* __restrict__ ref, double* out) {
+  __shared__ double red[kPostThreads];
+  const int tid = threadIdx.x;
+  double m = -INFINITY;
+  for (long long i = tid; i < N; i += kPostThreads) m = fmax(m, t[i]);
+  m = post_reduce<true>(m, red);
+  double s = 0.0;
+  for (long long i = tid; i < N; i += kPostThreads) s += exp(t[i] - m);
+  s = post_reduce<false>(s, red);
+  const double logz = m + log(s);
+  double s2 = 0.0;
+  for (long long i = tid; i < N; i += kPostThreads) {
+    const double lp = t[i] - logz, p = exp(lp);
+    t[i] = lp;
+    s2 += p * p;
+  }
+  s2 = post_reduce<false>(s2, red);
+  if (tid == 0) { out[0] = logz; out[1] = 1.0 / s2; }
+  for (int d = 0; d < D; ++d) {
+    double c = 0.0;
+    if (ref && theta)
+      for (long long i = tid; i < N; i += kPostThreads)
+        if (theta[(size_t)i * D + d] < ref[d]) c += exp(t[i]);
+    c = post_reduce<false>(c, red);
+    if (tid == 0) out[2 + d] = (ref && theta) ? c : NAN;
+  }
 }
 
 // FP64 FMA throughput probe: 8 independent chains per thread.

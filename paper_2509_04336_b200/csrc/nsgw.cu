@@ -32,6 +32,8 @@ thread_local std::string g_init_error;
 
 // CTA width of the CTA-per-particle sweep kernel (k_bins); the walk kernel chooses 128 / 96 / 64 by batch size.
 constexpr int kBinsThreads = 256;
+constexpr int kPostOut = 2 + kMaxDim;                 // ns_posterior summaries: logZ, ESS, CL per parameter
+constexpr int kFinDoubles = 2 + kPostOut + kMaxDim;   // d_fin / h_fin: final evidence, posterior summaries, reference point
 
 // ======================================================================================================
 // Device state of the sampler
@@ -92,7 +94,8 @@ struct ns_handle {
   long long theta_cap = 0;
   double* d_hio = nullptr;      // host-entry scratch: theta [B,11] + logl [B]
   long long hio_cap = 0;
-  double* d_fin = nullptr;      // 2 doubles
+  double* d_fin = nullptr;      // 2 doubles (final evidence) + kPostOut (posterior summaries) + kMaxDim (reference point)
+  double* d_post_lw = nullptr;  // [n_live] widths of the live points' rows (R:L26)
   ns_stats* h_stats = nullptr;  // pinned
   double* h_fin = nullptr;      // pinned
   uint64_t seed = 0;
@@ -382,7 +385,7 @@ void ns_free(ns_handle* h) {
   if (!h) return;
   cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_mtab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
-  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_hio);
+  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_post_lw); cudaFree(h->d_hio);
   if (h->s_own) cudaStreamDestroy(h->s_own);
   cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf); cudaFree(h->d_lc);
   if (h->h_stats) cudaFreeHost(h->h_stats);
@@ -497,9 +500,9 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
 
   // ---- sampler state
   INIT_CHECK(cudaMalloc(&h->d_state, sizeof(DevState)), -2);
-  INIT_CHECK(cudaMalloc(&h->d_fin, sizeof(double) * 2), -2);
+  INIT_CHECK(cudaMalloc(&h->d_fin, sizeof(double) * kFinDoubles), -2);
   INIT_CHECK(cudaMallocHost(&h->h_stats, sizeof(ns_stats)), -2);
-  INIT_CHECK(cudaMallocHost(&h->h_fin, sizeof(double) * 2), -2);
+  INIT_CHECK(cudaMallocHost(&h->h_fin, sizeof(double) * kFinDoubles), -2);
   const int n = cfg->n_live, k = cfg->n_delete, D = cfg->ndim;
   DevState hs;
   memset(&hs, 0, sizeof(hs));
@@ -511,6 +514,7 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
     INIT_CHECK(cudaMalloc(&h->d_live_u, sizeof(double) * (size_t)n * D), -2);
     INIT_CHECK(cudaMalloc(&h->d_live_l, sizeof(double) * (size_t)n), -2);
     INIT_CHECK(cudaMalloc(&h->d_order, sizeof(int) * (size_t)n), -2);
+    INIT_CHECK(cudaMalloc(&h->d_post_lw, sizeof(double) * (size_t)n), -2);
     INIT_CHECK(cudaMalloc(&h->d_surv, sizeof(double) * (size_t)(n - k) * D), -2);
     INIT_CHECK(cudaMalloc(&h->d_cur_u, sizeof(double) * (size_t)k * D), -2);
     INIT_CHECK(cudaMalloc(&h->d_cur_l, sizeof(double) * (size_t)k), -2);
@@ -875,7 +879,7 @@ int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host,
   const int n = h->cfg.n_live, k = h->cfg.n_delete;
   k_rank<<<(n + 255) / 256, 256, 0, s>>>(h->d_live_l, n, h->d_order);
   LAUNCH_CHECK(h);
-  k_finalize<<<1, 32, 0, s>>>(h->d_state, h->d_live_l, h->d_order, n, h->d_fin);
+  k_finalize<<<1, 32, 0, s>>>(h->d_state, h->d_live_l, h->d_order, n, h->d_fin, nullptr);
   LAUNCH_CHECK(h);
   CU_CHECK(h, cudaMemcpyAsync(h->h_fin, h->d_fin, sizeof(double) * 2, cudaMemcpyDeviceToHost, s));
   CU_CHECK(h, cudaStreamSynchronize(s));
@@ -883,6 +887,35 @@ int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host,
   if (logz_host) *logz_host = h->h_fin[0];
   if (h_host) *h_host = h->h_fin[1];
   if (logz_err_host) *logz_err_host = std::sqrt(std::max(h->h_fin[1], 0.0) / neff);
+  return 0;
+}
+
+int ns_posterior(ns_handle* h, const double* dead_dev, int64_t n_dead, double* theta_dev, double* logp_dev, const double* theta_ref_host,
+                 double* summary_host, void* stream) {
+  if (!h) return -3;
+  if (h->cfg.n_live <= 0) return fail(h, -3, "handle has no live set");
+  if (n_dead < 0 || (n_dead > 0 && !dead_dev) || !logp_dev) return fail(h, -1, "bad arguments");
+  if (theta_ref_host && !theta_dev) return fail(h, -1, "credible levels need theta_dev");
+  cudaStream_t s = (cudaStream_t)stream;
+  const int n = h->cfg.n_live, D = h->cfg.ndim;
+  const long long N = n_dead + n;
+  double* d_out = h->d_fin + 2;
+  double* d_ref = h->d_fin + 2 + kPostOut;
+  if (theta_ref_host) CU_CHECK(h, cudaMemcpyAsync(d_ref, theta_ref_host, sizeof(double) * D, cudaMemcpyHostToDevice, s));
+  k_rank<<<(n + 255) / 256, 256, 0, s>>>(h->d_live_l, n, h->d_order);
+  LAUNCH_CHECK(h);
+  k_finalize<<<1, 32, 0, s>>>(h->d_state, h->d_live_l, h->d_order, n, h->d_fin, h->d_post_lw);
+  LAUNCH_CHECK(h);
+  k_post_rows<<<(unsigned)((N + 255) / 256), 256, 0, s>>>(h->d_cfg, dead_dev, n_dead, h->d_live_u, h->d_live_l, h->d_order, h->d_post_lw, n,
+                                                         theta_dev, logp_dev);
+  LAUNCH_CHECK(h);
+  k_post_norm<<<1, kPostThreads, 0, s>>>(logp_dev, N, theta_dev, D, theta_ref_host ? d_ref : nullptr, d_out);
+  LAUNCH_CHECK(h);
+  if (summary_host) {
+    CU_CHECK(h, cudaMemcpyAsync(h->h_fin + 2, d_out, sizeof(double) * (2 + D), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(h, cudaStreamSynchronize(s));
+    for (int i = 0; i < 2 + D; ++i) summary_host[i] = h->h_fin[2 + i];
+  }
   return 0;
 }
 

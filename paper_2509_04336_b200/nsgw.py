@@ -43,7 +43,7 @@ class NsStats(C.Structure):
 
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
-           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence", "ns_posterior",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 _lib = None
@@ -294,6 +294,21 @@ class Handle:
         a, b, c = C.c_double(), C.c_double(), C.c_double()
         self._check(lib().ns_finalize_evidence(self._h, C.byref(a), C.byref(b), C.byref(c), _stream()), "ns_finalize_evidence")
         return a.value, b.value, c.value
+
+    def posterior(self, dead=None, theta_ref=None, want_theta=True):
+        """ns_posterior: rows = dead (device [n_dead, ndim+3], optional) + the live points.  Returns a dict with theta [N, ndim]
+        (device), logp [N] (device), logz, ess and cl [ndim] (NumPy; NaN without theta_ref)."""
+        import numpy as np
+        n_dead = 0 if dead is None else int(dead.shape[0])
+        N = n_dead + self.n_live
+        theta = torch.empty((N, self.ndim), dtype=torch.float64, device="cuda") if (want_theta or theta_ref is not None) else None
+        logp = torch.empty(N, dtype=torch.float64, device="cuda")
+        summ = (C.c_double * (2 + self.ndim))()
+        ref = None
+        if theta_ref is not None:
+            ref = (C.c_double * self.ndim)(*[float(x) for x in theta_ref])
+        self._check(lib().ns_posterior(self._h, _ptr(dead), C.c_int64(n_dead), _ptr(theta), _ptr(logp), ref, summ, _stream()), "ns_posterior")
+        return {"theta": theta, "logp": logp, "logz": summ[0], "ess": summ[1], "cl": np.array(summ[2:2 + self.ndim])}
 
 
 def run_many(handles, term_kind, term_tol, max_iter, dead=None):

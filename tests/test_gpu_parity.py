@@ -857,3 +857,96 @@ def test_error_codes(nsgw, c2):
 def test_fp64_peak_probe(nsgw):
     tf = nsgw.measure_fp64_peak(1 << 16)
     assert 10.0 < tf < 60.0, tf
+
+
+# ---- posterior weights (ns_posterior; reading R:L26) --------------------------------------------------------------------------
+def _posterior_parity(nsgw, spec, smp, seed, max_iter, ref, term=(0, 0.01)):
+    h = nsgw.Handle(spec, smp, seed=seed)
+    k, D = smp["n_delete"], spec["ndim"]
+    dead, nit, logx = None, 0, 0.0
+    if max_iter:
+        buf = torch.full((max_iter * k, D + 3), float("nan"), dtype=torch.float64, device="cuda")
+        nit, st = h.run(term[0], term[1], max_iter, dead=buf)
+        dead, logx = buf[: nit * k].contiguous(), st["logx"]
+    out = h.posterior(dead, theta_ref=ref)
+    lu, ll = h.get_live()
+    want = O.posterior(O.OracleProblem(spec), None if dead is None else dead.cpu().numpy(), lu.cpu().numpy(), ll.cpu().numpy(), logx,
+                       theta_ref=ref)
+    N = nit * k + smp["n_live"]
+    assert out["theta"].shape == (N, D) and out["logp"].shape == (N,)
+    np.testing.assert_allclose(out["theta"].cpu().numpy(), want["theta"], rtol=4e-15, atol=4e-15)
+    np.testing.assert_allclose(out["logp"].cpu().numpy(), want["logp"], rtol=0, atol=1e-10)
+    assert abs(out["logz"] - want["logz"]) < 1e-10
+    assert abs(out["ess"] / want["ess"] - 1.0) < 1e-10
+    np.testing.assert_allclose(out["cl"], want["cl"], rtol=0, atol=1e-12)
+    assert abs(out["logz"] - h.finalize_evidence()[0]) < 1e-9          # same terms as the sequential scan, other summation order
+    assert abs(float(torch.exp(out["logp"]).sum()) - 1.0) < 1e-12
+    # the sampler's state is untouched and the call is bit-reproducible (fixed-order reductions)
+    again = h.posterior(dead, theta_ref=ref)
+    assert torch.equal(again["logp"], out["logp"]) and again["ess"] == out["ess"] and np.array_equal(again["cl"], out["cl"])
+    lu2, ll2 = h.get_live()
+    assert torch.equal(lu2, lu) and torch.equal(ll2, ll)
+    return out, want
+
+
+def test_posterior_parity_config1(nsgw):
+    spec, smp, _ = W.config1()
+    ref = [0.1, -0.3, 0.4, 0.2]
+    out, _ = _posterior_parity(nsgw, spec, smp, 5, 500, ref)        # to termination: 50+ iterations, several thousand rows
+    assert 300 < out["ess"] < 3000
+    _posterior_parity(nsgw, spec, smp, 6, 28, ref)                  # stopped early: the live points' rows carry the mass
+    out0, _ = _posterior_parity(nsgw, spec, smp, 7, 0, ref)         # no dead points at all: live rows only, logX = 0
+    assert out0["theta"].shape[0] == smp["n_live"]
+    # without a reference point: NaN levels, same weights
+    h = nsgw.Handle(spec, smp, seed=7)
+    o2 = h.posterior(None)
+    assert np.all(np.isnan(o2["cl"])) and torch.equal(o2["logp"], out0["logp"])
+    o3 = h.posterior(None, want_theta=False)
+    assert o3["theta"] is None and torch.equal(o3["logp"], out0["logp"])
+
+
+def test_posterior_parity_gw_priors(nsgw):
+    # PhenomD-form problem with the full 11-parameter prior box (power-law distance, sine / cosine angles, periodic dims)
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 200.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 10.0, wf)
+    smp = dict(n_live=90, n_delete=45, naccept=8, maxmcmc=40, walks0=10.0, delay=-1.0)
+    _posterior_parity(nsgw, spec, smp, 8, 7, list(W.INJ_C3), term=(0, 1e-9))
+
+
+def test_posterior_argument_errors(nsgw):
+    import ctypes as C
+    spec, smp, _ = W.config1()
+    h = nsgw.Handle(spec, smp, seed=1)
+    L = nsgw.lib()
+    logp = torch.empty(smp["n_live"] + 5, dtype=torch.float64, device="cuda")
+    ref = (C.c_double * 4)(0.0, 0.0, 0.0, 0.0)
+    null = C.c_void_p(0)
+    assert L.ns_posterior(h._h, null, C.c_int64(5), null, C.c_void_p(logp.data_ptr()), None, None, null) == -1     # rows without a buffer
+    assert L.ns_posterior(h._h, null, C.c_int64(0), null, null, None, None, null) == -1                          # no output
+    assert L.ns_posterior(h._h, null, C.c_int64(0), null, C.c_void_p(logp.data_ptr()), ref, None, null) == -1      # levels need theta
+    assert L.ns_posterior(h._h, null, C.c_int64(-1), null, C.c_void_p(logp.data_ptr()), None, None, null) == -1
+    assert L.ns_posterior(None, null, C.c_int64(0), null, C.c_void_p(logp.data_ptr()), None, None, null) == -3
+    hb = nsgw.Handle(W.config2(wf))                                                                              # no live set
+    assert L.ns_posterior(hb._h, null, C.c_int64(0), null, C.c_void_p(logp.data_ptr()), None, None, null) == -3
+
+
+def test_posterior_config1_moments_from_device_runs(nsgw):
+    # end to end on the device: weighted second moments and marginal CDFs of the analytic Gaussian over 24 runs
+    spec, smp, _ = W.config1()
+    cov, _ = W.givens_cov()
+    ref = np.array([0.1, -0.3, 0.4, 0.2])
+    k, D = smp["n_delete"], 4
+    second, cls, esss = [], [], []
+    for seed in range(101, 125):
+        h = nsgw.Handle(spec, smp, seed=seed)
+        buf = torch.empty((500 * k, D + 3), dtype=torch.float64, device="cuda")
+        nit, st = h.run(smp["term_kind"], smp["term_tol"], 500, dead=buf)
+        out = h.posterior(buf[: nit * k].contiguous(), theta_ref=ref)
+        pw = torch.exp(out["logp"])
+        second.append(((out["theta"] * pw[:, None]).T @ out["theta"]).cpu().numpy())
+        cls.append(out["cl"])
+        esss.append(out["ess"])
+    sig = np.sqrt(np.diag(cov))
+    assert np.allclose(np.mean(second, axis=0), cov, atol=0.06 * float(np.max(sig)) ** 2, rtol=0.08)
+    cdf = np.array([0.5 * (1 + math.erf(r / s / math.sqrt(2))) for r, s in zip(ref, sig)])
+    assert np.all(np.abs(np.mean(cls, axis=0) - cdf) < 4.5 * 0.5 / np.sqrt(np.mean(esss) * len(cls)))
