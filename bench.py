@@ -418,6 +418,32 @@ def run_ours(args):
                                   "accept_max": int(na.max()), "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl)})
             extras["config5_sweep"] = sweep
             h5.close()
+            # PP test (stand-in for the paper's 100-injection study): config-3 shape, priors, PSD and sampler
+            # settings; injections drawn from the prior, each in its own noise; credible levels of the injected values from the
+            # weighted posterior (ns_posterior); KS test of uniformity per parameter
+            from paper_2509_04336_b200 import pp
+
+            def pt_cuda(s, uu):
+                tmp = dict(s)
+                tmp["strain"] = np.zeros((s["n_det"], s["n_freq"], 2))
+                hh = nsgw.Handle(tmp)
+                out = hh.prior_transform_batch(torch.as_tensor(uu).cuda()).cpu().numpy()
+                hh.close()
+                return out
+
+            specs_pp, th_pp = W.pp_problem_set(spec3, args.pp_injections, 9001, wf_cuda_for(nsgw, torch), pt_cuda)
+            for label, kw in (("exact", {}), ("relbin", {"relbin_eps": 0.5})):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                res = pp.credible_levels(specs_pp, th_pp, smp3, smp3["term_kind"], smp3["term_tol"], 400, seed0=500, group=4, **kw)
+                wall = time.perf_counter() - t0
+                ks = [pp.ks_uniform(res["cl"][:, d]) for d in range(11)]
+                extras["pp_config3_" + label] = {
+                    "injections": args.pp_injections, "wall_s": wall, "n_eval_total": int(res["evals"].sum()),
+                    "iterations_mean": float(res["iters"].mean()), "ess_median": float(np.median(res["ess"])),
+                    "ks_D": [round(k_[0], 4) for k_ in ks], "ks_p": [round(k_[1], 4) for k_ in ks],
+                    "cl_mean": [round(float(x), 4) for x in res["cl"].mean(axis=0)],
+                    "cl_var": [round(float(x), 4) for x in res["cl"].var(axis=0)]}
         line["extras"] = extras
 
     # ---- CPU baseline: the oracle as it stands on the host cores, bounded sample of the same rows (rank 0, N=1)
@@ -465,6 +491,7 @@ def main():
     ap.add_argument("--quick", action="store_true", help="skip the walk / full-run extras")
     ap.add_argument("--full-extras", action="store_true", help="also run the config-4 nested-sampling run and the config-5 sweep")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--pp-injections", type=int, default=100, help="injections of the PP leg of --full-extras")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

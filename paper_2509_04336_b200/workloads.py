@@ -216,3 +216,32 @@ def shell_spec(ndim, periodic=None):
     """Cube-shell test likelihood L(u) = -max_d |u_d - 1/2| (walk-uniformity / volume pins)."""
     return dict(like_kind=LIKE_SHELL, ndim=ndim, prior_kind=[UNIFORM] * ndim, prior_lo=[0.0] * ndim, prior_hi=[1.0] * ndim,
                 periodic=list(periodic) if periodic is not None else [0] * ndim, n_det=0, n_freq=0)
+
+
+def fix_dims(spec, free, theta_fixed):
+    """Copy of a GW spec with every parameter outside `free` FIXED at theta_fixed (periodic flags cleared on fixed dims)."""
+    spec = dict(spec)
+    kinds, lo, hi, per = list(spec["prior_kind"]), list(spec["prior_lo"]), list(spec["prior_hi"]), list(spec["periodic"])
+    for d in range(spec["ndim"]):
+        if d not in free:
+            kinds[d] = FIXED
+            lo[d] = hi[d] = float(theta_fixed[d])
+            per[d] = 0
+    spec["prior_kind"], spec["prior_lo"], spec["prior_hi"], spec["periodic"] = kinds, lo, hi, per
+    return spec
+
+
+def pp_problem_set(spec, n_inj, seed, waveform_fn, prior_transform_fn):
+    """Stand-in for the paper's 100-injection study: n_inj signals drawn from the prior of `spec` (which carries its PSD),
+    each in its own noise realisation.  Row i of the Philox(seed) uniforms goes through the caller's prior transform
+    (prior_transform_fn(spec, u[n, ndim]) -> theta[n, ndim]) and waveform (waveform_fn(spec, theta) -> h[n_det, n_freq, 2]); the
+    strain is h + noise(seed + 1 + i).  Returns (list of specs, theta[n_inj, ndim])."""
+    u = uniforms(n_inj, spec["ndim"], seed)
+    theta = np.asarray(prior_transform_fn(spec, u), dtype=np.float64)
+    out = []
+    for i in range(n_inj):
+        s = dict(spec)
+        s["theta_inj"] = theta[i].copy()
+        s["strain"] = np.asarray(waveform_fn(spec, theta[i])) + noise(spec, spec["psd"], seed + 1 + i)
+        out.append(s)
+    return out, theta

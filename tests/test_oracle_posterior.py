@@ -120,3 +120,36 @@ def test_config1_posterior_when_stopped_early():
     cdf = np.array([0.5 * (1 + math.erf(r / s / math.sqrt(2))) for r, s in zip(ref, sig)])
     assert np.all(np.abs(cls.mean(axis=0) - cdf) < 5.0 * 0.5 / np.sqrt(np.mean(esss) * len(cls))), (cls.mean(axis=0), cdf)
     assert np.allclose(second, cov, atol=0.25 * float(np.max(sig)) ** 2), second - cov
+
+
+def _toy_pp_specs(n_inj, seed):
+    """PP law on the Gaussian toy: theta_inj ~ U(box), observed d = theta_inj + eps, eps ~ N(0, Sigma); the likelihood of theta
+    is N(d; theta, Sigma), so the credible levels of theta_inj under the posterior are uniform."""
+    spec, smp, _ = W.config1()
+    cov, _ = W.givens_cov()
+    rng = np.random.Generator(np.random.Philox(key=seed))
+    th = rng.uniform(-10.0, 10.0, size=(n_inj, 4))
+    d = th + rng.multivariate_normal(np.zeros(4), cov, size=n_inj)
+    specs = []
+    for i in range(n_inj):
+        s = dict(spec)
+        s["toy_mean"] = list(d[i])
+        specs.append(s)
+    return specs, th, smp
+
+
+def test_pp_law_on_the_gaussian_toy():
+    from scipy import stats
+    specs, th, smp = _toy_pp_specs(120, 41)
+    cl = np.empty((len(specs), 4))
+    for i, s in enumerate(specs):
+        P = O.OracleProblem(s)
+        S = O.OracleSampler(P, smp["n_live"], smp["n_delete"], smp["naccept"], smp["maxmcmc"], smp["walks0"], smp["delay"], seed=1000 + i)
+        nit, st, dead = S.run(smp["term_kind"], smp["term_tol"], 500, want_dead=True)
+        lu, ll = S.live()
+        cl[i] = O.posterior(P, dead, lu, ll, st["logx"], theta_ref=th[i])["cl"]
+    pv = [stats.kstest(cl[:, d], "uniform").pvalue for d in range(4)]
+    assert min(pv) > 0.01 / 4, pv
+    assert np.all(np.abs(cl.mean(axis=0) - 0.5) < 4.0 / math.sqrt(12 * len(specs)))
+    # posteriors too narrow / too wide pile the levels up at the ends / in the middle: the variance of uniform levels is 1/12
+    assert np.all(np.abs(cl.var(axis=0) - 1 / 12) < 0.035)
