@@ -432,7 +432,15 @@ def run_ours(args):
                 return out
 
             specs_pp, th_pp = W.pp_problem_set(spec3, args.pp_injections, 9001, wf_cuda_for(nsgw, torch), pt_cuda)
-            for label, kw in (("exact", {}), ("relbin", {"relbin_eps": 0.5})):
+            # the same with the distance prior cut to [200, 800] Mpc (SNR 20-80 for the config-3 masses): the regime relative
+            # binning is made for (eps 0.1: the tolerance has to shrink as the SNR grows)
+            spec3n = dict(spec3)
+            spec3n["prior_lo"], spec3n["prior_hi"] = list(spec3["prior_lo"]), list(spec3["prior_hi"])
+            spec3n["prior_lo"][4], spec3n["prior_hi"][4] = 200.0, 800.0
+            specs_pn, th_pn = W.pp_problem_set(spec3n, args.pp_injections, 9002, wf_cuda_for(nsgw, torch), pt_cuda)
+            for label, kw in (("exact", {}), ("relbin", {"relbin_eps": 0.5}), ("near_exact", {}), ("near_relbin", {"relbin_eps": 0.1})):
+                if label.startswith("near"):
+                    specs_pp, th_pp = specs_pn, th_pn
                 torch.cuda.synchronize()
                 t0 = time.perf_counter()
                 res = pp.credible_levels(specs_pp, th_pp, smp3, smp3["term_kind"], smp3["term_tol"], 400, seed0=500, group=4, **kw)
