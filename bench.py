@@ -381,6 +381,34 @@ def run_ours(args):
                 hk.close()
             seq["logz_closed_form"] = logz_true["logz_exact"]
             extras["config1_sequential_limit"] = seq
+            # the same on a GW problem that both settings finish (PhenomD-form, H1+L1, 20-128 Hz = 433 bins, SNR 10; Mc, q, dL, tc
+            # free, n_live 400): k = 200 against k = 1 (one CTA walks at a time: the sequential bilby-like limit on this machine);
+            # and config 3 itself with k = 1, first 2000 iterations only
+            wfc = wf_cuda_for(nsgw, torch)
+            spec_s = W.fix_dims(W.make_data(W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 128.0, (20.0, 40.0)), W.INJ_C3, 10.0, wfc),
+                                (0, 1, 4, 8), W.INJ_C3)
+            gseq = {}
+            for kdel in (200, 1):
+                smp_k = dict(n_live=400, n_delete=kdel, naccept=20, maxmcmc=2000, walks0=50.0, delay=-1.0)
+                hk = nsgw.Handle(spec_s, smp_k, seed=1)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                nit, st = hk.run(0, 0.1, 200000)
+                lz, le, _ = hk.finalize_evidence()
+                wall = time.perf_counter() - t0
+                gseq[f"k={kdel}"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": lz, "logz_err": le,
+                                     "walk_len_last": st["walk_len"], "evals_per_s": st["n_eval_total"] / wall}
+                hk.close()
+            hk = nsgw.Handle(spec3, dict(smp3, n_delete=1), seed=1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            nit, st = hk.run(smp3["term_kind"], smp3["term_tol"], 2000)
+            wall = time.perf_counter() - t0
+            gseq["config3_k=1_first_2000_iterations"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"],
+                                                         "walk_len_last": st["walk_len"], "evals_per_s": st["n_eval_total"] / wall,
+                                                         "logx": st["logx"]}
+            hk.close()
+            extras["gw_sequential_limit"] = gseq
             # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
             spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
             h4 = nsgw.Handle(spec4, smp4, seed=1)

@@ -990,3 +990,11 @@ def test_pp_levels_uniform_gw_four_parameters(nsgw):
     pv = [stats.kstest(cl[:, j], "uniform").pvalue for j in range(len(free))]
     assert min(pv) > 0.01 / len(free), (pv, cl.mean(axis=0))
     assert np.all(res["ess"] > 100)
+
+
+def test_ns_step_parity_gw_single_deletion(nsgw):
+    # k = 1 (the sequential limit): one walker per iteration, adaptation after every replacement
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 200.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 10.0, wf)
+    smp = dict(n_live=40, n_delete=1, naccept=6, maxmcmc=60, walks0=12.0, delay=-1.0)
+    _step_parity(nsgw, spec, smp, 12, 3, 1e-8)
