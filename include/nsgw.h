@@ -188,6 +188,15 @@ int ns_finalize_evidence(ns_handle* h, double* logz_host, double* logz_err_host,
 int ns_posterior(ns_handle* h, const double* dead_dev, int64_t n_dead, double* theta_dev, double* logp_dev,
                  const double* theta_ref_host, double* summary_host, void* stream);
 
+/* Equal-weight posterior sample by systematic resampling of the rows ns_posterior produced (DESIGN reading R:L27): one uniform
+ * U from the Philox block with counter (0, 0, 0, 4 << 24) under key = seed; draw j = 0..n_out-1 sits at (j + U) / n_out of the
+ * cumulative weights C_i = p_0 + .. + p_i (row order) and takes the first row with C_i > (j + U) / n_out * C_{N-1}; row i is
+ * drawn floor(n_out p_i) or ceil(n_out p_i) times.  logp_dev [N] (device); cum_dev [N] (device scratch, receives C);
+ * idx_dev [n_out] int64 (device, optional) the drawn rows, ascending; theta_out_dev [n_out, ndim] (device, optional) the rows of
+ * theta_dev [N, ndim] gathered.  At least one output.  Asynchronous on `stream`.  Errors: -1 bad arguments. */
+int ns_posterior_resample(ns_handle* h, const double* logp_dev, const double* theta_dev, int64_t N, int64_t n_out, uint64_t seed,
+                          double* cum_dev, int64_t* idx_dev, double* theta_out_dev, void* stream);
+
 /* Device FP64 FMA throughput probe used for the roofline denominator: runs `iters` dependent-chain DFMAs x 8 chains per
  * thread on a full grid and returns achieved TFLOP/s in *tflops_host (synchronises; timed with CUDA events). */
 int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream);

@@ -391,3 +391,16 @@ def posterior(prob, dead, live_u, live_logl, logx, theta_ref=None):
         ref = _f64(theta_ref)
         out["cl"] = np.array([math.fsum(pw[theta[:, d] < ref[d]].tolist()) for d in range(theta.shape[1])])
     return out
+
+
+def posterior_resample(logp, n_out, seed):
+    """Equal-weight posterior sample by systematic resampling (reading R:L27): one uniform U = u53(w0, w1) from the Philox block
+    with counter (0, 0, 0, 4 << 24) and key = seed; positions t_j = (j + U) / n_out, j = 0..n_out-1; C_i = p_0 + .. + p_i in row
+    order; row of draw j = the first i with C_i > t_j C_{N-1}.  Row i is drawn floor(n_out p_i) or ceil(n_out p_i) times.
+    Returns (idx [n_out] int64, U)."""
+    w = philox([0, 0, 0, 4 << 24], [seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF])
+    U = u53(w[0], w[1])
+    cum = np.cumsum(np.exp(_f64(logp)))
+    t = (np.arange(n_out) + U) / n_out
+    idx = np.searchsorted(cum, t * cum[-1], side="right")
+    return np.minimum(idx, cum.size - 1).astype(np.int64), U

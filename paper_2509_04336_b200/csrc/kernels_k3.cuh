@@ -231,6 +231,47 @@ __global__ void __launch_bounds__(kPostThreads) k_post_norm(double* t, long long
   }
 }
 
+// Inclusive cumulative sum of p = exp(log p) in row order (R:L27).  One CTA: thread t owns the contiguous rows
+// [t L, (t + 1) L), L = ceil(N / kPostThreads); thread 0 scans the partials; fixed order, bit-reproducible.
+__global__ void __launch_bounds__(kPostThreads) k_post_cumsum(const double* __restrict__ logp, long long N, double* cum) {
+  __shared__ double part[kPostThreads];
+  const int tid = threadIdx.x;
+  const long long L = (N + kPostThreads - 1) / kPostThreads;
+  const long long lo = min(N, tid * L), hi = min(N, lo + L);
+  double s = 0.0;
+  for (long long i = lo; i < hi; ++i) s += exp(logp[i]);
+  part[tid] = s;
+  __syncthreads();
+  if (tid == 0) {
+    double run = 0.0;
+    for (int t = 0; t < kPostThreads; ++t) { const double v = part[t]; part[t] = run; run += v; }
+  }
+  __syncthreads();
+  s = part[tid];
+  for (long long i = lo; i < hi; ++i) { s += exp(logp[i]); cum[i] = s; }
+}
+
+// Systematic resampling (R:L27): draw j sits at t_j = (j + U) / n_out, U = u01 of Philox block (0, 0, 0, 4 << 24) under
+// key = seed; its row is the first i with C_i > t_j C_{N-1} (binary search).  idx and / or the gathered theta rows are written.
+__global__ void k_post_pick(const double* __restrict__ cum, long long N, long long n_out, uint32_t k0, uint32_t k1, int D,
+                            const double* __restrict__ theta, long long* idx, double* theta_out) {
+  const long long j = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (j >= n_out) return;
+  uint32_t w[4];
+  philox4x32_10(0u, 0u, 0u, 4u << 24, k0, k1, w);
+  const double U = u01(w[0], w[1]);
+  const double v = (((double)j + U) / (double)n_out) * cum[N - 1];
+  long long lo = 0, hi = N;            // first i in [0, N) with cum[i] > v; N if none
+  while (lo < hi) {
+    const long long mid = (lo + hi) >> 1;
+    if (cum[mid] > v) hi = mid; else lo = mid + 1;
+  }
+  const long long i = min(lo, N - 1);
+  if (idx) idx[j] = i;
+  if (theta_out)
+    for (int d = 0; d < D; ++d) theta_out[(size_t)j * D + d] = theta[(size_t)i * D + d];
+}
+
 // FP64 FMA throughput probe: 8 independent chains per thread.
 __global__ void k_dfma_probe(long long iters, double* sink) {
   double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;

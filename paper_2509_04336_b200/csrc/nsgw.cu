@@ -919,6 +919,21 @@ int ns_posterior(ns_handle* h, const double* dead_dev, int64_t n_dead, double* t
   return 0;
 }
 
+int ns_posterior_resample(ns_handle* h, const double* logp_dev, const double* theta_dev, int64_t N, int64_t n_out, uint64_t seed,
+                          double* cum_dev, int64_t* idx_dev, double* theta_out_dev, void* stream) {
+  if (!h) return -3;
+  if (N <= 0 || n_out < 0 || !logp_dev || !cum_dev || (!idx_dev && !theta_out_dev) || (theta_out_dev && !theta_dev))
+    return fail(h, -1, "bad arguments");
+  cudaStream_t s = (cudaStream_t)stream;
+  k_post_cumsum<<<1, kPostThreads, 0, s>>>(logp_dev, N, cum_dev);
+  LAUNCH_CHECK(h);
+  if (n_out == 0) return 0;
+  k_post_pick<<<(unsigned)((n_out + 255) / 256), 256, 0, s>>>(cum_dev, N, n_out, (uint32_t)(seed & 0xFFFFFFFFull), (uint32_t)(seed >> 32),
+                                                             h->cfg.ndim, theta_dev, reinterpret_cast<long long*>(idx_dev), theta_out_dev);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (!h) return -3;
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }

@@ -43,7 +43,7 @@ class NsStats(C.Structure):
 
 
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
-           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence", "ns_posterior",
+           "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence", "ns_posterior", "ns_posterior_resample",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 # nsgw_set_option keys (include/nsgw.h)
@@ -312,6 +312,16 @@ class Handle:
             ref = (C.c_double * self.ndim)(*[float(x) for x in theta_ref])
         self._check(lib().ns_posterior(self._h, _ptr(dead), C.c_int64(n_dead), _ptr(theta), _ptr(logp), ref, summ, _stream()), "ns_posterior")
         return {"theta": theta, "logp": logp, "logz": summ[0], "ess": summ[1], "cl": np.array(summ[2:2 + self.ndim])}
+
+    def posterior_resample(self, logp, n_out, seed, theta=None):
+        """ns_posterior_resample: systematic resampling of the weighted rows.  Returns (idx [n_out] int64 device, theta rows or None)."""
+        N = int(logp.shape[0])
+        cum = torch.empty(N, dtype=torch.float64, device="cuda")
+        idx = torch.empty(n_out, dtype=torch.int64, device="cuda")
+        out = torch.empty((n_out, self.ndim), dtype=torch.float64, device="cuda") if theta is not None else None
+        self._check(lib().ns_posterior_resample(self._h, _ptr(logp), _ptr(theta), C.c_int64(N), C.c_int64(n_out), C.c_uint64(seed),
+                                                _ptr(cum), _ptr(idx), _ptr(out), _stream()), "ns_posterior_resample")
+        return idx, out
 
 
 def run_many(handles, term_kind, term_tol, max_iter, dead=None):

@@ -998,3 +998,44 @@ def test_ns_step_parity_gw_single_deletion(nsgw):
     spec = W.make_data(spec, W.INJ_C3, 10.0, wf)
     smp = dict(n_live=40, n_delete=1, naccept=6, maxmcmc=60, walks0=12.0, delay=-1.0)
     _step_parity(nsgw, spec, smp, 12, 3, 1e-8)
+
+
+def test_posterior_resample_parity(nsgw):
+    # systematic resampling of a run's weighted rows (R:L27): same rows as the oracle except where a comb position falls within
+    # rounding of a cumulative weight (the two sides sum p in different orders), and there by one row at most
+    spec, smp, _ = W.config1()
+    h = nsgw.Handle(spec, smp, seed=9)
+    k, D = smp["n_delete"], 4
+    buf = torch.empty((500 * k, D + 3), dtype=torch.float64, device="cuda")
+    nit, st = h.run(smp["term_kind"], smp["term_tol"], 500, dead=buf)
+    out = h.posterior(buf[: nit * k].contiguous())
+    logp = out["logp"].cpu().numpy()
+    cum = np.cumsum(np.exp(logp))
+    for n_out, seed in ((4000, 1), (333, 2 ** 33 + 7), (1, 3), (20000, 4)):
+        idx_g, th_g = h.posterior_resample(out["logp"], n_out, seed, theta=out["theta"])
+        idx_o, U = O.posterior_resample(logp, n_out, seed)
+        ig = idx_g.cpu().numpy()
+        bad = np.nonzero(ig != idx_o)[0]
+        t = (bad + U) / n_out * cum[-1]
+        assert np.all(np.abs(ig[bad] - idx_o[bad]) <= 1)
+        assert np.all(np.minimum(np.abs(cum[ig[bad]] - t), np.abs(cum[idx_o[bad]] - t)) < 1e-12 * cum[-1])
+        assert bad.size <= max(1, n_out // 1000)
+        assert torch.equal(th_g, out["theta"][idx_g])
+        cnt = np.bincount(ig, minlength=logp.size)
+        p = np.exp(logp)
+        assert np.all(cnt >= np.floor(n_out * p - 1e-6)) and np.all(cnt <= np.ceil(n_out * p + 1e-6))
+        again, _ = h.posterior_resample(out["logp"], n_out, seed, theta=out["theta"])
+        assert torch.equal(again, idx_g)
+    # equal-weight sample reproduces the weighted second moments (n_out >> ESS: resampling noise 1/n_out per weight)
+    cov, _ = W.givens_cov()
+    pw = torch.exp(out["logp"])
+    m2w = ((out["theta"] * pw[:, None]).T @ out["theta"]).cpu().numpy()
+    m2s = (th_g.T @ th_g / th_g.shape[0]).cpu().numpy()
+    assert np.allclose(m2s, m2w, atol=8e-3)
+    # argument errors
+    import ctypes as C
+    L, null = nsgw.lib(), C.c_void_p(0)
+    lp, cm = C.c_void_p(out["logp"].data_ptr()), C.c_void_p(torch.empty(logp.size, dtype=torch.float64, device="cuda").data_ptr())
+    assert L.ns_posterior_resample(h._h, lp, null, C.c_int64(logp.size), C.c_int64(10), C.c_uint64(1), cm, null, null, null) == -1   # no output
+    assert L.ns_posterior_resample(h._h, lp, null, C.c_int64(0), C.c_int64(10), C.c_uint64(1), cm, cm, null, null) == -1             # no rows
+    assert L.ns_posterior_resample(h._h, lp, null, C.c_int64(logp.size), C.c_int64(10), C.c_uint64(1), cm, null, cm, null) == -1     # gather needs theta

@@ -153,3 +153,31 @@ def test_pp_law_on_the_gaussian_toy():
     assert np.all(np.abs(cl.mean(axis=0) - 0.5) < 4.0 / math.sqrt(12 * len(specs)))
     # posteriors too narrow / too wide pile the levels up at the ends / in the middle: the variance of uniform levels is 1/12
     assert np.all(np.abs(cl.var(axis=0) - 1 / 12) < 0.035)
+
+
+def test_systematic_resampling_invariants():
+    rng = np.random.default_rng(11)
+    logp, _ = O.posterior_weights(rng.normal(0, 3, 500), rng.normal(-5, 2, 500))
+    p = np.exp(logp)
+    for n_out, seed in ((1000, 1), (137, 2), (5000, 2 ** 40 + 3)):
+        idx, U = O.posterior_resample(logp, n_out, seed)
+        assert 0.0 < U < 1.0 and idx.shape == (n_out,) and np.all(np.diff(idx) >= 0)
+        cnt = np.bincount(idx, minlength=p.size)
+        # systematic resampling: every row is drawn floor(n p) or ceil(n p) times
+        assert np.all(cnt >= np.floor(n_out * p - 1e-9)) and np.all(cnt <= np.ceil(n_out * p + 1e-9))
+        assert cnt.sum() == n_out
+    # different seeds move the comb; the same seed repeats it
+    a, Ua = O.posterior_resample(logp, 1000, 5)
+    b, Ub = O.posterior_resample(logp, 1000, 6)
+    c, Uc = O.posterior_resample(logp, 1000, 5)
+    assert Ua != Ub and Ua == Uc and np.array_equal(a, c) and not np.array_equal(a, b)
+    # equal weights, as many draws as rows: every row exactly once, whatever U
+    lp = np.full(64, -math.log(64.0))
+    assert np.array_equal(O.posterior_resample(lp, 64, 9)[0], np.arange(64))
+    # a single draw is the U-quantile of the cumulative weights
+    i1, U1 = O.posterior_resample(logp, 1, 3)
+    cum = np.cumsum(p)
+    assert cum[i1[0]] > U1 * cum[-1] and (i1[0] == 0 or cum[i1[0] - 1] <= U1 * cum[-1])
+    # the uniform is the RNG contract's: block (0, 0, 0, 4 << 24) under key = seed
+    w = O.philox([0, 0, 0, 4 << 24], [3, 0])
+    assert U1 == O.u53(w[0], w[1])
