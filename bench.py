@@ -288,6 +288,30 @@ def run_ours(args):
             extras["ns_run_config3_relbin"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
                                                "logz_err": err, "H": H, "n_bins": nbins, "walk_len_last": st["walk_len"],
                                                "accept_mean_last": st["accept_mean"], "evals_per_s": st["n_eval_total"] / wall}
+            # posterior post-processing of such a run (ns_posterior + ns_posterior_resample; R:L26-27), timed with CUDA events
+            k3, D3 = smp3["n_delete"], 11
+            h3p = nsgw.Handle(spec3, smp3, seed=1)
+            h3p.relbin_setup(W.INJ_C3)
+            h3p.set_option(2, 1)
+            dead3 = torch.empty((200 * k3, D3 + 3), dtype=torch.float64, device="cuda")
+            nit, st = h3p.run(smp3["term_kind"], smp3["term_tol"], 200, dead=dead3)
+            rows3 = dead3[: nit * k3].contiguous()
+            for _ in range(3):
+                post = h3p.posterior(rows3, theta_ref=W.INJ_C3)
+                h3p.posterior_resample(post["logp"], 10000, 1, theta=post["theta"])
+            a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            a.record(stream)
+            for _ in range(10):
+                post = h3p.posterior(rows3, theta_ref=W.INJ_C3)
+            b.record(stream)
+            for _ in range(10):
+                h3p.posterior_resample(post["logp"], 10000, 1, theta=post["theta"])
+            c.record(stream)
+            torch.cuda.synchronize()
+            extras["posterior_config3_relbin"] = {"rows": int(rows3.shape[0]) + smp3["n_live"], "ns_posterior_ms": a.elapsed_time(b) / 10,
+                                                  "resample_10000_ms": b.elapsed_time(c) / 10, "ess": post["ess"], "logz_rows": post["logz"],
+                                                  "cl_injection": [round(float(x), 4) for x in post["cl"]]}
+            h3p.close()
             h3r.close()
             nb2 = h.relbin_setup(W.INJ_C3)
             rb_out = torch.empty(B, dtype=torch.float64, device="cuda")

@@ -2,8 +2,9 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
 It imports nothing from paper_2509_04336_b200 (the CUDA path) and the CUDA path imports nothing from here.
-Every function is a thin call into oracle.cpp, whose header lists what pins each part, except the posterior weights at the
-end of this file (reading R:L26), written out here in NumPy/math.fsum and pinned by tests/test_oracle_posterior.py.
+Every function is a thin call into oracle.cpp, whose header lists what pins each part, except the posterior weights and the
+systematic resampling at the end of this file (readings R:L26, R:L27), written out here in NumPy/math.fsum and pinned by
+tests/test_oracle_posterior.py.
 """
 import math
 
