@@ -230,6 +230,10 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * moved the point.  Exact likelihood only. */
 #define NSGW_OPT_INNER_KERNEL 3
 #define NSGW_OPT_SLICE_STEPS 4
+/* key NSGW_OPT_WALK_STAGE: 1 = the PhenomD-form walk kernel stages the table values of each thread's next bin in shared memory
+ * with asynchronous copies (same arithmetic, bit-identical results; costs chunk slots, measured 10 % slower on config 3);
+ * 0 (default) = plain loads.  A tuning switch. */
+#define NSGW_OPT_WALK_STAGE 5
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */

@@ -127,7 +127,8 @@ template <int MODEL, int NDET, int P, int NT>
 __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
                                          const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
                                          const int* slot /*smem [P]: coefficient-block / phasor-table slot of particle p*/,
-                                         double (&acc)[P][AccLayout<MODEL, NDET>::N]) {
+                                         double (&acc)[P][AccLayout<MODEL, NDET>::N],
+                                         double* stage = nullptr /*smem [NT (3 + 3 NDET)] or null: see the MR loop*/) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NW = NT / 32, ND1 = NDET - 1;
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
@@ -230,24 +231,55 @@ __device__ __forceinline__ void bin_loop(const DevCfg& cfg, const Tables& tb, co
 #pragma unroll
       for (int i = 0; i < 4; ++i) am[p][i] = cbp[p][CB_AM + i];
     }
+    auto mr_bin = [&](int p, double f, double f34, double y3, const double2 (&w)[NDET], const double (&wsv)[NDET]) {
+      double q = fma(pm[p][1], f, pm[p][0]);
+      q = fma(pm[p][2], y3, q);
+      q = fma(pm[p][3], f34, q);
+      q = fma(pm[p][4], atan_tab((f - pm[p][5]) * pm[p][6], mt), q);
+      const double fx = f - am[p][0];
+      const double amp = am[p][1] * rcp_nr1(fma(fx, fx, am[p][2])) * ex[p];
+      ex[p] *= exr[p];
+      tail(p, q, amp, w, wsv);
+    };
+    if (stage) {
+      // Walk / slice kernels: with 4 CTAs per SM shared memory leaves L1 some 20 KB, every table load comes from L2 (hit rate
+      // 8 %) and at the 128-register cap the compiler issues the loads right before their use (25 % of the warp samples waited
+      // there).  Each thread therefore stages the seven table values of ITS next bin in a shared-memory slot of its own with
+      // LDGSTS while it works on the current bin: same values, same order of arithmetic, bit-identical sums.
+      double* sf = stage; double* sf34 = stage + NT; double* sy3 = stage + 2 * NT; double* sws = stage + 3 * NT;
+      double2* swd = reinterpret_cast<double2*>(stage + (3 + NDET) * NT);
+      auto issue = [&](int k) {
+        cp_async8(sf + tid, tb.f + k); cp_async8(sf34 + tid, tb.f34 + k); cp_async8(sy3 + tid, &tb.t01[k].y);
+#pragma unroll
+        for (int d = 0; d < NDET; ++d) { cp_async8(sws + d * NT + tid, tb.ws[d] + k); cp_async16(swd + d * NT + tid, tb.wd[d] + k); }
+      };
+      int k = k_mr + tid;
+      if (k < nf) issue(k);
+      for (; k < nf; k += NT) {
+        cp_async_wait_all();
+        const double f = sf[tid], f34 = sf34[tid], y3 = sy3[tid];
+        double2 w[NDET];
+        double wsv[NDET];
+#pragma unroll
+        for (int d = 0; d < NDET; ++d) { w[d] = swd[d * NT + tid]; wsv[d] = sws[d * NT + tid]; }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+          mr_bin(p, f, f34, y3, w, wsv);
+          // the slot is free once its values have been consumed by the first particle: fetch the next bin behind the rest
+          if (p == 0 && k + NT < nf) issue(k + NT);
+        }
+      }
+    } else {
 #pragma unroll 2
-    for (int k = k_mr + tid; k < nf; k += NT) {
-      const double f = __ldg(tb.f + k), f34 = __ldg(tb.f34 + k);
-      const double y3 = __ldg(tb.t01 + k).y;       // 1/f
-      double2 w[NDET];
-      double wsv[NDET];
+      for (int k = k_mr + tid; k < nf; k += NT) {
+        const double f = __ldg(tb.f + k), f34 = __ldg(tb.f34 + k);
+        const double y3 = __ldg(tb.t01 + k).y;       // 1/f
+        double2 w[NDET];
+        double wsv[NDET];
 #pragma unroll
-      for (int d = 0; d < NDET; ++d) { w[d] = __ldg(tb.wd[d] + k); wsv[d] = __ldg(tb.ws[d] + k); }
+        for (int d = 0; d < NDET; ++d) { w[d] = __ldg(tb.wd[d] + k); wsv[d] = __ldg(tb.ws[d] + k); }
 #pragma unroll
-      for (int p = 0; p < P; ++p) {
-        double q = fma(pm[p][1], f, pm[p][0]);
-        q = fma(pm[p][2], y3, q);
-        q = fma(pm[p][3], f34, q);
-        q = fma(pm[p][4], atan_tab((f - pm[p][5]) * pm[p][6], mt), q);
-        const double fx = f - am[p][0];
-        const double amp = am[p][1] * rcp_nr1(fma(fx, fx, am[p][2])) * ex[p];
-        ex[p] *= exr[p];
-        tail(p, q, amp, w, wsv);
+        for (int p = 0; p < P; ++p) mr_bin(p, f, f34, y3, w, wsv);
       }
     }
   }

@@ -22,6 +22,7 @@ struct WalkArgs {
   int* n_accept; int* n_eval; int* n_oob;
   uint8_t* tflags; double* tlogl;
   int trace_stride;
+  int stage;                // GW PhenomD-form exact sweep: 1 = per-thread LDGSTS staging of the table values (bin_loop)
   int spec;                 // speculative steps per chunk: cap (1..kWalkDMax) of the per-walker adaptive length ...
   int spec_fixed;           // ... or, if non-zero, the fixed length
   int spec_cap;             // chunk buffers in shared memory hold this many steps (>= spec)
@@ -134,11 +135,12 @@ constexpr int kWalkSteps = 128;   // steps per chunk (cap): proposals are drawn 
 template <int MODEL, int NDET, int PG, int NT>
 __device__ __forceinline__ void sweep_group(const DevCfg& cfg, const Tables& tb, const double* cbs, const double2* tabL,
                                             const double2* tabW, const double2* step, const MathTables* mt, const bool* active,
-                                            const int* slot, double* red, double* out /*smem [PG][N]*/) {
+                                            const int* slot, double* red, double* out /*smem [PG][N]*/,
+                                            double* stage = nullptr /*smem, see bin_loop*/) {
   using AL = AccLayout<MODEL, NDET>;
   constexpr int NV = PG * AL::N;
   double acc[PG][AL::N];
-  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, mt, active, slot, acc);
+  bin_loop<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, mt, active, slot, acc, stage);
   double v[NV];
 #pragma unroll
   for (int p = 0; p < PG; ++p)
@@ -152,6 +154,9 @@ template <int NDET, int NT>
 constexpr size_t walk_smem_bytes(int dm) {
   return sizeof(double2) * dm * (NDET > 1 ? NDET - 1 : 1) * (32 + NT / 32 + 1) + sizeof(double) * dm * (CB_SIZE + kMaxDim);
 }
+// the per-thread table staging slots of bin_loop's merger-ringdown loop (WalkArgs::stage), carved behind the chunk buffers
+template <int NDET, int NT>
+constexpr size_t walk_stage_bytes() { return sizeof(double) * NT * (3 + 3 * NDET); }
 
 // NT threads per walker: 128 when all walkers of the batch are resident at 4 CTAs per SM, 96 (5 per SM) or 64 (8 per SM) when
 // that keeps a larger batch in one wave (config 4: k = 700 on 148 SMs).
@@ -170,6 +175,7 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
   double* cbs = reinterpret_cast<double*>(step + DM * ND1);        // [DM][CB_SIZE]
   double (*s_prop)[kMaxDim] = reinterpret_cast<double (*)[kMaxDim]>(cbs + DM * CB_SIZE);   // [DM][kMaxDim]
   double2* rbuf = reinterpret_cast<double2*>(cbs + DM * (CB_SIZE + kMaxDim));              // RB: partial sums [32][NT/32][2 NDET]
+  double* stage = (MODEL == 2 && !RB && a.stage) ? cbs + DM * (CB_SIZE + kMaxDim) : nullptr;   // exact PhenomD sweep: table staging
   __shared__ double red[NW * PG * AL::N], out[PG * AL::N], s_logl[DMX];
   __shared__ MathTables mtab;
   __shared__ bool active[PG];
@@ -313,8 +319,8 @@ __global__ void __launch_bounds__(NT, 512 / NT) k_walk_gw(const DevCfg* __restri
           active[tid] = mine >= 0;
         }
         __syncthreads();
-        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
-        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out);
+        if (ng == PG) sweep_group<MODEL, NDET, PG, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out, stage);
+        else sweep_group<MODEL, NDET, 1, NT>(cfg, tb, cbs, tabL, tabW, step, &mtab, active, slot, red, out, stage);
         if (tid < ng) s_logl[slot[tid]] = finish_logl<MODEL, NDET>(cfg, cbs + slot[tid] * CB_SIZE, out + tid * AL::N, nullptr);
         __syncthreads();
       }

@@ -88,6 +88,7 @@ struct ns_handle {
   double* d_lc = nullptr;       // slice kernel: direction factor [ndim][ndim]
   int opt_like = 0;             // 0 exact likelihood, 1 relative binning (sampler and ns_loglike_u_batch)
   int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
+  int opt_walk_stage = 0;       // PhenomD-form exact walk: LDGSTS staging of the sweep's table values (NSGW_OPT_WALK_STAGE; measured slower)
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
@@ -317,12 +318,13 @@ int launch_walk_gw_k(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
   static bool attr_set = false;
   if (!attr_set) {
     CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + extra)));
+                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + extra + walk_stage_bytes<NDET, NT>())));
     attr_set = true;
   }
   a.spec_cap = dm;
   a.spec = std::min(a.spec, dm);
-  kern<<<(unsigned)a.B, NT, walk_smem_bytes<NDET, NT>(dm) + extra, s>>>(h->d_cfg, h->tb, a, h->rb);
+  const size_t stage = (MODEL == 2 && !RB && a.stage) ? walk_stage_bytes<NDET, NT>() : 0;
+  kern<<<(unsigned)a.B, NT, walk_smem_bytes<NDET, NT>(dm) + extra + stage, s>>>(h->d_cfg, h->tb, a, h->rb);
   LAUNCH_CHECK(h);
   return 0;
 }
@@ -335,7 +337,8 @@ int launch_walk_gw_nt(ns_handle* h, const WalkArgs& a, int dm, cudaStream_t s) {
 // Longest chunk buffers (32, 16 or 8 slots) with which `ctas` CTAs of the kernel still fit the SM's shared memory.
 template <int NDET, int NT>
 int walk_chunk_cap(const ns_handle* h, int ctas) {
-  const size_t extra = h->opt_like == 1 ? sizeof(double) * NT * 2 * NDET : 0;
+  const size_t extra = h->opt_like == 1 ? sizeof(double) * NT * 2 * NDET
+                                        : (h->opt_walk_stage && h->cfg.like_kind != NSGW_LIKE_GW_TAYLORF2 ? walk_stage_bytes<NDET, NT>() : 0);
   for (int dm = kWalkDMax; dm > 8; dm /= 2)
     if ((size_t)ctas * (walk_smem_bytes<NDET, NT>(dm) + extra + 10496) <= (size_t)225 * 1024) return dm;
   return 8;
@@ -606,6 +609,7 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
   a.trace_stride = walk_len;
   a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
   a.spec_fixed = h->opt_walk_spec > 0;
+  a.stage = h->opt_walk_stage;
   return launch_walk(h, a, (cudaStream_t)stream);
 }
 
@@ -647,6 +651,7 @@ int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
   a.lstar_dev = &h->d_state->lstar; a.W_dev = &h->d_state->W; a.iter_dev = &h->d_state->iter;
   a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
   a.spec_fixed = h->opt_walk_spec > 0;
+  a.stage = h->opt_walk_stage;
   a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
   a.n_accept = h->d_cnt; a.n_eval = h->d_cnt + k; a.n_oob = h->d_cnt + 2 * k;
   int rc = 0;
@@ -938,6 +943,7 @@ int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (!h) return -3;
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
   if (key == NSGW_OPT_WALK_SPEC && value >= 0 && value <= kWalkDMax) { h->opt_walk_spec = value; return 0; }
+  if (key == NSGW_OPT_WALK_STAGE && (value == 0 || value == 1)) { h->opt_walk_stage = value; return 0; }
   if (key == NSGW_OPT_INNER_KERNEL && (value == 0 || value == 1)) {
     if (value == 1 && h->opt_like == 1) return fail(h, -5, "the slice kernel evaluates the exact likelihood only");
     h->opt_inner = value;

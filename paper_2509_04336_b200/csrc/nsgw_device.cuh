@@ -565,6 +565,16 @@ struct BinBasis {
   double y2, y3, y5, xL, x2;
 };
 
+// Asynchronous global -> shared copies of 8 / 16 bytes (LDGSTS) and the wait for this thread's own copies.  Used where a thread
+// stages the table values of ITS next bin in a shared-memory slot only it reads: no barrier is involved.
+__device__ __forceinline__ void cp_async8(void* smem, const void* gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 __device__ __forceinline__ BinBasis make_basis(const Tables& tb, int k, bool phenom) {
   BinBasis b;
   const double2 a = __ldg(tb.t01 + k), c = __ldg(tb.t23 + k), e = __ldg(tb.t45 + k), g = __ldg(tb.t67 + k);
