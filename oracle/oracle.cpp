@@ -16,7 +16,14 @@
 //   u53 / index / Erlang-4 ... range, mean/variance, KS against scipy gamma CDF
 //   prior transforms ......... CDF-inversion identities
 //   detector geometry ........ light travel times, antenna-pattern invariants, sky average 2/5
-//   TaylorF2 phase ........... mpmath 40-digit evaluation of the printed formula, Newtonian chirp time
+//   TaylorF2 phase ........... every coefficient phi_2..phi_7 and both logarithms DERIVED with sympy from independently typed PN energy and
+//                              flux series (spin-orbit to 3.5PN, spin-spin at 2PN), themselves checked against Kerr geodesics and
+//                              black-hole perturbation theory in the test-mass limit (tests/test_oracle_pn_derivation.py);
+//                              mpmath 40-digit evaluation of the printed formula, Newtonian chirp time
+//   inspiral amplitude ....... spin-independent parts of A_2..A_6 and all of A_3 derived the same way from the (2,2)-mode amplitude and
+//                              the chirp rate; THE SPIN PARTS OF A_4, A_5, A_6 ARE THIS BUILD'S CONSTANTS (recalled, PARITY UNPINNED,
+//                              like the fit table: DESIGN.md A.2)
+//   walk-length tuning ....... R:L13/L14 recurrence on by-hand accept counts: 0.5 floor, maxmcmc cap, k = 1 / k = n/2 / explicit delays
 //   <h,h> .................... closed form |C|^2 A0^2 I_{7/3}; Euler-Maclaurin integral for flat PSD
 //   <d,h> .................... noise-free maximum, exact symmetries, 1/dL scaling, time-shift covariance
 //   PhenomD-form ............. C0/C1 continuity, reduction to TaylorF2, QNM hand values, mpmath twin;
@@ -539,11 +546,25 @@ void orc_amp_phase(const orc_problem* p, const double* theta, const double* f, i
 }
 
 // PhenomD-form derived quantities: [Frd, Fdamp, Fpeak, t0, C1int, C2int, C1mr, C2mr, M_seconds, eta, 19 Lambda values]
+// TaylorF2 phase coefficients phi_k, phi_k^(l) (DESIGN.md A.1) for mass ratio q and aligned spins: accessor for the pin that
+// derives them from the PN energy and flux (tests/test_oracle_pn_derivation.py).  They do not depend on the chirp mass.
+void orc_taylorf2_coeffs(double q, double chi1, double chi2, double* phi, double* phil) {
+  Intrinsic s = make_intrinsic(30.0, q, chi1, chi2);
+  taylorf2_coeffs(s, phi, phil);
+}
+
 void orc_phenomd_info(const orc_problem* p, const double* theta, double* out) {
   PhenomD m = make_phenomd(p, theta[0], theta[1], theta[2], theta[3]);
   out[0] = m.Frd; out[1] = m.Fdamp; out[2] = m.Fpeak; out[3] = m.t0;
   out[4] = m.C1int; out[5] = m.C2int; out[6] = m.C1mr; out[7] = m.C2mr; out[8] = m.s.M; out[9] = m.s.eta;
   for (int r = 0; r < 19; ++r) out[10 + r] = m.L[r];
+}
+
+// Inspiral amplitude PN coefficients A_0..A_6 of the PhenomD-form model (DESIGN.md A.2): accessor for the pin that derives their
+// spin-independent parts and A_3 from the PN energy, flux and (2,2)-mode amplitude (tests/test_oracle_pn_derivation.py).
+void orc_phenomd_amp_coeffs(const orc_problem* p, const double* theta, double* A) {
+  PhenomD m = make_phenomd(p, theta[0], theta[1], theta[2], theta[3]);
+  for (int i = 0; i < 7; ++i) A[i] = m.A[i];
 }
 
 // Detector-frame waveform h_det(f_k) on the problem's grid: out[n_det][n_freq][2].  Used by tests to inject signals.

@@ -164,3 +164,63 @@ def test_logz_2d_gw_quadrature():
         logz, err, _ = S.finalize()
         pulls.append((logz - logz_quad) / err)
     assert np.all(np.abs(pulls) < 4.0), (pulls, logz_quad)
+
+
+# ---- walk-length tuning ("same logic as bilby to target a desired number of accepted proposals", P:116 delay as a function of
+#      the batch size; readings R:L13, R:L14): the recurrence on accept counts that are known without running any arithmetic ----
+def _flat_sampler(n, k, naccept, maxmcmc, walks0, delay=-1.0, seed=1):
+    """Constant likelihood (zero precision matrix): no proposal ever satisfies logL' > L*, so every walker accepts exactly 0 steps."""
+    D = 3
+    spec = dict(like_kind=W.LIKE_GAUSS, ndim=D, prior_kind=[W.UNIFORM] * D, prior_lo=[0.0] * D, prior_hi=[1.0] * D,
+                periodic=[1] * D, toy_mean=[0.0] * D, toy_prec=np.zeros((D, D)), toy_lognorm=0.0, n_det=0, n_freq=0)
+    return O.OracleSampler(O.OracleProblem(spec), n, k, naccept, maxmcmc=maxmcmc, walks0=walks0, delay=delay, seed=seed)
+
+
+def test_walk_length_recurrence_by_hand():
+    # (a) k = n/2: delay = max(100/(10*50) - 1, 0) = 0.  0 accepts -> floor 0.5: r = 0.5/10; naccept/r = 5*10/0.5 = 100 -> walks 100
+    S = _flat_sampler(100, 50, naccept=5, maxmcmc=5000, walks0=10.0)
+    st = S.step()
+    assert st["walk_len"] == 10 and st["accept_mean"] == 0.0 and st["n_stuck"] == 50 and st["n_oob"] == 0 and st["n_eval"] == 500
+    assert st["walks_next"] == 100.0
+    # second step: W = 100, 0 accepts: 5*100/0.5 = 1000 (delay 0: no memory of the 100)
+    st = S.step()
+    assert st["walk_len"] == 100 and st["walks_next"] == 1000.0
+    # (b) the maxmcmc cap: the same with maxmcmc = 60 -> 60, and the next walk has exactly 60 steps
+    S = _flat_sampler(100, 50, naccept=5, maxmcmc=60, walks0=10.0)
+    assert S.step()["walks_next"] == 60.0
+    st = S.step()
+    assert st["walk_len"] == 60 and st["n_eval"] == 50 * 60 and st["walks_next"] == 60.0
+    # (c) sequential limit k = 1: delay = 100/10 - 1 = 9 (bilby's n_live/10 - 1): (10*9 + 100)/10 = 19
+    S = _flat_sampler(100, 1, naccept=5, maxmcmc=5000, walks0=10.0)
+    st = S.step()
+    assert st["walk_len"] == 10 and abs(st["walks_next"] - 19.0) < 1e-12
+    # then W = 19: naccept/r = 5*19/0.5 = 190; (19*9 + 190)/10 = 36.1
+    st = S.step()
+    assert st["walk_len"] == 19 and abs(st["walks_next"] - 36.1) < 1e-12
+    # (d) the smoothing uses the REAL-valued walks, the rate uses the integer W: walks0 = 10.7 -> W = 10; (10.7*9 + 100)/10 = 19.63
+    S = _flat_sampler(100, 1, naccept=5, maxmcmc=5000, walks0=10.7)
+    st = S.step()
+    assert st["walk_len"] == 10 and abs(st["walks_next"] - 19.63) < 1e-12
+    # (e) explicit delay 2 with k = n/2: (10*2 + 100)/3 = 40; in-between batch k = 20 of 1000: delay = 1000/200 - 1 = 4: (10*4 + 100)/5 = 28
+    assert abs(_flat_sampler(100, 50, 5, 5000, 10.0, delay=2.0).step()["walks_next"] - 40.0) < 1e-12
+    assert abs(_flat_sampler(1000, 20, 5, 5000, 10.0).step()["walks_next"] - 28.0) < 1e-12
+
+
+def test_walk_length_recurrence_with_accepts():
+    # cube shell, all dims periodic (no out-of-bounds steps): the reported counts are integers, the update from them is by hand:
+    # walks' = min((walks*delay + naccept*W/max(0.5, mean)) / (delay + 1), maxmcmc) in exact rational arithmetic
+    from fractions import Fraction as Fr
+    spec = W.shell_spec(3, [1, 1, 1])
+    for n, k, maxmcmc in ((60, 30, 5000), (60, 3, 5000), (60, 30, 45)):
+        S = O.OracleSampler(O.OracleProblem(spec), n, k, 4, maxmcmc=maxmcmc, walks0=20.0, seed=5)
+        walks = Fr(20)
+        delay = max(Fr(n, 10 * k) - 1, Fr(0))
+        for it in range(4):
+            st = S.step()
+            Wl = max(1, min(int(walks), maxmcmc))
+            assert st["walk_len"] == Wl and st["n_oob"] == 0 and st["n_eval"] == k * Wl
+            total = round(st["accept_mean"] * k)
+            assert abs(total - st["accept_mean"] * k) < 1e-9 and total > 0
+            mean = max(Fr(1, 2), Fr(total, k))
+            walks = min((walks * delay + 4 * Wl / mean) / (delay + 1), Fr(maxmcmc))
+            assert abs(st["walks_next"] - float(walks)) <= 1e-12 * float(walks), (n, k, it, st["walks_next"], float(walks))
