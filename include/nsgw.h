@@ -234,6 +234,14 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * with asynchronous copies (same arithmetic, bit-identical results; costs chunk slots, measured 10 % slower on config 3);
  * 0 (default) = plain loads.  A tuning switch. */
 #define NSGW_OPT_WALK_STAGE 5
+/* key NSGW_OPT_WALK_KERNEL: how ns_step / ns_run / ns_walk_batch run the acceptance walk on a GW likelihood.  0 = automatic
+ * (2 for the exact likelihood, 1 for relative binning); 1 = one CTA per walker, all steps in one launch (k_walk_gw); 2 = batch-wide
+ * rounds: every walker proposes a chunk of steps, the likelihood of all the batch's in-bounds proposals is evaluated in one launch
+ * of the CTA-per-row kernel, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows
+ * the device two rounds behind, so these calls synchronise with the stream while they run; 3 = as 2 with the lane-per-row kernel
+ * (k_pd_lp; PhenomD-form, otherwise 2).  Decisions, counters, traces and end points are identical for 1, 2 and every chunk length;
+ * 3 sums a row's bins in another (fixed) order. */
+#define NSGW_OPT_WALK_KERNEL 6
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */

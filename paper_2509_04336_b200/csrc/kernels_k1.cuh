@@ -331,8 +331,11 @@ __device__ __forceinline__ double finish_logl(const DevCfg& cfg, const double* c
 
 template <int MODEL, int NDET, int P>
 __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
-                                                           long long B, double* logl, double* parts) {
+                                                           long long B_host, const int* __restrict__ B_dev /*overrides B_host*/,
+                                                           double* logl, double* parts) {
   using AL = AccLayout<MODEL, NDET>;
+  const long long B = B_dev ? (long long)*B_dev : B_host;
+  if ((long long)blockIdx.x * P >= B) return;     // the worklist walk sizes the grid for its row capacity
   constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) double cbs[P * CB_SIZE];
   __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];

@@ -5,8 +5,10 @@
 //                        per-bin PhenomD-form evaluation
 //   kernels_k1.cuh       k_tables / k_i73 / k_math_tables / k_draw_live / k_prior_transform (ns_init), k_setup, k_bins (CTA per
 //                        particle pair), k_bins_lp + k_finish (lane per particle), k_waveform
+//   kernels_pdlp.cuh     k_pd_lp (PhenomD-form: lane per particle over the merger-ringdown bins + warp per particle below), k_finish_rows
 //   kernels_relbin.cuh   k_rb_delta / k_rb_select / k_rb_summary / k_relbin (relative binning, R:L24)
 //   kernels_walk.cuh     de_propose, k_walk_simple, k_walk_gw (speculative chunks; exact or relative-binning likelihood)
+//   kernels_wl.cuh       k_wl_head (the walk as batch-wide rounds: resolve + propose + set-up per walker; rows swept by the K1 kernels)
 //   kernels_slice.cuh    k_slice_simple, k_slice_gw (hit-and-run slice sampling, R:L25)
 //   kernels_k3.cuh       k_rank / k_evidence / k_gather_start / k_writeback / k_adapt / k_finalize, k_dfma_probe
 // This file: ns_handle, launch geometry, argument checks and the extern "C" entry points.
@@ -46,8 +48,10 @@ struct DevState {
 };
 
 #include "kernels_k1.cuh"
+#include "kernels_pdlp.cuh"
 #include "kernels_relbin.cuh"
 #include "kernels_walk.cuh"
+#include "kernels_wl.cuh"
 #include "kernels_slice.cuh"
 #include "kernels_k3.cuh"
 
@@ -89,7 +93,14 @@ struct ns_handle {
   int opt_like = 0;             // 0 exact likelihood, 1 relative binning (sampler and ns_loglike_u_batch)
   int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
   int opt_walk_stage = 0;       // PhenomD-form exact walk: LDGSTS staging of the sweep's table values (NSGW_OPT_WALK_STAGE; measured slower)
-  int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp; TaylorF2 only)
+  int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp / k_pd_lp)
+  int opt_walk_kernel = 0;      // 0 auto, 1 CTA per walker (k_walk_gw), 2 worklist rounds swept by k_bins, 3 swept by k_pd_lp (PhenomD-form)
+  // worklist walk (kernels_wl.cuh): per-walker state, double-buffered row buffers, host-visible progress
+  WlState wl{};
+  long long wl_cap_b = 0, wl_cap_r = 0;
+  int wl_kr = 0;                // bins per range of k_pd_lp on the walk's rows: fixed per handle so a row's logL never depends on the round
+  int* h_wl_nact = nullptr;     // pinned ring [4]
+  cudaEvent_t wl_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
   long long theta_cap = 0;
@@ -218,10 +229,56 @@ int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaS
   return 0;
 }
 
+// Bins per range of k_pd_lp for `rows` rows (multiple of the tile length): the value that minimises rounds x (range + per-task
+// overhead) over the persistent grid, rounds = ceil(tasks / CTA slots).
+int pd_pick_kr(const ns_handle* h, long long rows) {
+  const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
+  const long long slots = (long long)h->n_sm * kPdOCC;
+  int kr = kPdKT;
+  double best = 1e300;
+  for (int c = kPdKT; c <= 1024; c += kPdKT) {
+    const int nr = (h->cfg.n_freq + c - 1) / c;
+    const long long nt = ngroups * nr;
+    const double cost = (double)((nt + slots - 1) / slots) * (c + 24) + 0.25 * nr;
+    if (cost < best - 1e-9) { best = cost; kr = c; }
+  }
+  return kr;
+}
+
+// PhenomD-form rows -> logL through k_pd_lp + k_finish_rows.  cbs [rows][CB_SIZE]; rows_dev (optional, device) overrides `rows` for
+// the task lists (then `rows` is the capacity the buffers and the grid are sized for); kr: bins per range (0: by pd_pick_kr).
+template <int NDET>
+int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* rows_dev, int kr, double* logl, double* parts, cudaStream_t s) {
+  using AL = AccLayout<2, NDET>;
+  if (kr <= 0) kr = pd_pick_kr(h, rows);
+  const int nranges = (h->cfg.n_freq + kr - 1) / kr;
+  int rc = ensure_partial(h, (size_t)rows * (nranges + 1) * AL::N);
+  if (rc) return rc;
+  PdArgs a;
+  a.cbs = cbs; a.n_rows = rows; a.n_rows_dev = rows_dev; a.stride = rows; a.kr = kr; a.nranges = nranges; a.partial = h->d_partial;
+  const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
+  const long long ntasks = ngroups * nranges + (rows + (kPdNT / 32) * kPdLowPer - 1) / ((kPdNT / 32) * kPdLowPer);
+  const long long grid = std::min<long long>(ntasks, (long long)h->n_sm * kPdOCC);
+  cudaEvent_t e0 = nullptr, e1 = nullptr;
+  if (h->prof && h->prof_ev.size() < 4096) {
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, s);
+  }
+  k_pd_lp<NDET><<<(unsigned)grid, kPdNT, 0, s>>>(h->d_cfg, h->tb, a);
+  if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
+  LAUNCH_CHECK(h);
+  const long long gfin = std::min<long long>((rows + 127) / 128, (long long)h->n_sm * 8);
+  k_finish_rows<2, NDET><<<(unsigned)gfin, 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges + 1, rows, rows_dev, rows, logl, parts);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
 template <int MODEL, int NDET>
 int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
   if (MODEL == 1 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kLpMinBatch)))
     return launch_bins_lp<NDET>(h, B, logl, parts, s);
+  if (MODEL == 2 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kLpMinBatch)))
+    return launch_pd_lp<NDET>(h, h->d_cb, B, nullptr, 0, logl, parts, s);
   int P = pick_p(B);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (h->prof && h->prof_ev.size() < 4096) {
@@ -229,9 +286,9 @@ int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaS
     cudaEventRecord(e0, s);
   }
   if (P == 2) {
-    k_bins<MODEL, NDET, 2><<<(unsigned)((B + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, logl, parts);
+    k_bins<MODEL, NDET, 2><<<(unsigned)((B + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, nullptr, logl, parts);
   } else {
-    k_bins<MODEL, NDET, 1><<<(unsigned)B, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, logl, parts);
+    k_bins<MODEL, NDET, 1><<<(unsigned)B, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, nullptr, logl, parts);
   }
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
@@ -315,12 +372,9 @@ template <int MODEL, int NDET, int NT, bool RB>
 int launch_walk_gw_k(ns_handle* h, WalkArgs a, int dm, cudaStream_t s) {
   auto kern = k_walk_gw<MODEL, NDET, NT, RB>;
   const size_t extra = RB ? sizeof(double) * NT * 2 * NDET : 0;   // partial sums of phase B
-  static bool attr_set = false;
-  if (!attr_set) {
-    CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + extra + walk_stage_bytes<NDET, NT>())));
-    attr_set = true;
-  }
+  // (per launch: the attribute is per device and per function, and a process may drive several devices and threads)
+  CU_CHECK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   (int)(walk_smem_bytes<NDET, NT>(kWalkDMax) + extra + walk_stage_bytes<NDET, NT>())));
   a.spec_cap = dm;
   a.spec = std::min(a.spec, dm);
   const size_t stage = (MODEL == 2 && !RB && a.stage) ? walk_stage_bytes<NDET, NT>() : 0;
@@ -356,6 +410,80 @@ int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   return launch_walk_gw_nt<MODEL, NDET, 64>(h, a, walk_chunk_cap<NDET, 64>(h, 8), s);
 }
 
+// ---- the walk as batch-wide rounds (kernels_wl.cuh) -----------------------------------------------------------------------
+// Buffers for B walkers and R = B x e_cap rows per round.  One allocation per kind (int state, step maps, row doubles, counters).
+int ensure_wl(ns_handle* h, long long B, long long R) {
+  if (!h->h_wl_nact) {
+    CU_CHECK(h, cudaMallocHost(&h->h_wl_nact, sizeof(int) * 4));
+    for (auto& e : h->wl_ev) CU_CHECK(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    CU_CHECK(h, cudaMalloc(&h->wl.n_rows, sizeof(int) * 4));
+    h->wl.n_active = h->wl.n_rows + 2;
+  }
+  if (B > h->wl_cap_b) {
+    cudaFree(h->wl.t0); cudaFree(h->wl.step);
+    h->wl.t0 = nullptr; h->wl.step = nullptr; h->wl_cap_b = 0;
+    CU_CHECK(h, cudaMalloc(&h->wl.t0, sizeof(int) * 7 * (size_t)B));
+    CU_CHECK(h, cudaMalloc(&h->wl.step, (size_t)B * kWalkSteps));
+    h->wl.E = h->wl.t0 + B; h->wl.nsteps = h->wl.t0 + 2 * B; h->wl.rowbase = h->wl.t0 + 3 * B; h->wl.cnt = h->wl.t0 + 4 * B;
+    h->wl_cap_b = B;
+  }
+  if (R > h->wl_cap_r) {
+    cudaFree(h->wl.row_u[0]);
+    h->wl.row_u[0] = nullptr; h->wl_cap_r = 0;
+    const size_t per = (size_t)R * (kMaxDim + CB_SIZE + 1);
+    CU_CHECK(h, cudaMalloc(&h->wl.row_u[0], sizeof(double) * 2 * per));
+    for (int i = 0; i < 2; ++i) {
+      double* base = h->wl.row_u[0] + i * per;
+      h->wl.row_u[i] = base; h->wl.row_cb[i] = base + (size_t)R * kMaxDim; h->wl.row_logl[i] = base + (size_t)R * (kMaxDim + CB_SIZE);
+    }
+    h->wl_cap_r = R;
+  }
+  return 0;
+}
+
+// logL of the rows of one round (cbs [R cap][CB_SIZE], count on the device) with the batched K1 kernels.
+template <int MODEL, int NDET>
+int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, double* logl, cudaStream_t s) {
+  if (MODEL == 2 && h->opt_walk_kernel == 3) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
+  if (R >= 4096) k_bins<MODEL, NDET, 2><<<(unsigned)((R + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
+  else k_bins<MODEL, NDET, 1><<<(unsigned)R, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+template <int MODEL, int NDET>
+int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
+  const long long B = a.B;
+  // rows per walker and round: up to 32 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
+  const int e_cap = (int)std::max<long long>(1, std::min<long long>(kWalkDMax, 65536 / B));
+  const long long R = B * e_cap;
+  int rc = ensure_wl(h, B, R);
+  if (rc) return rc;
+  if (h->wl_kr == 0) h->wl_kr = pd_pick_kr(h, (long long)std::max(2, h->cfg.n_delete) * kWalkDMax);
+  WlState st = h->wl;
+  st.e_cap = e_cap;
+  CU_CHECK(h, cudaMemsetAsync(st.n_rows, 0, sizeof(int) * 4, s));
+  const unsigned gh = (unsigned)((B + kWlWarps - 1) / kWlWarps);
+  for (long long r = 0;; ++r) {
+    const int par = (int)(r & 1);
+    k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, (int)std::min<long long>(r, 2 + par));   // only "first round or not" and the parity matter
+    LAUNCH_CHECK(h);
+    CU_CHECK(h, cudaMemcpyAsync(h->h_wl_nact + (r & 3), st.n_active + par, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU_CHECK(h, cudaEventRecord(h->wl_ev[r & 3], s));
+    rc = sweep_rows<MODEL, NDET>(h, st.row_cb[par], R, st.n_rows + par, st.row_logl[par], s);
+    if (rc) return rc;
+    if (r >= 2) {   // the host runs two rounds ahead of what it has seen: rounds enqueued after the last walker finished are no-ops
+      CU_CHECK(h, cudaEventSynchronize(h->wl_ev[(r - 2) & 3]));
+      if (h->h_wl_nact[(r - 2) & 3] == 0) break;
+    }
+  }
+  if (a.n_accept || a.n_eval || a.n_oob) {
+    k_wl_counters<<<(unsigned)((B + 255) / 256), 256, 0, s>>>(st.cnt, B, a.n_accept, a.n_eval, a.n_oob);
+    LAUNCH_CHECK(h);
+  }
+  return 0;
+}
+
 int launch_walk(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   if (a.B == 0) return 0;
   if (!is_gw(h->cfg.like_kind)) {
@@ -364,6 +492,17 @@ int launch_walk(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
     return 0;
   }
   const int nd = h->cfg.n_det;
+  if (h->opt_like == 0 && h->opt_walk_kernel != 1) {   // exact likelihood: batch-wide rounds (kernels_wl.cuh)
+    if (h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2) {
+      if (nd == 1) return run_walk_wl<1, 1>(h, a, s);
+      if (nd == 2) return run_walk_wl<1, 2>(h, a, s);
+      if (nd == 3) return run_walk_wl<1, 3>(h, a, s);
+    } else {
+      if (nd == 1) return run_walk_wl<2, 1>(h, a, s);
+      if (nd == 2) return run_walk_wl<2, 2>(h, a, s);
+      if (nd == 3) return run_walk_wl<2, 3>(h, a, s);
+    }
+  }
   if (h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2) {
     if (nd == 1) return launch_walk_gw<1, 1>(h, a, s);
     if (nd == 2) return launch_walk_gw<1, 2>(h, a, s);
@@ -391,6 +530,9 @@ void ns_free(ns_handle* h) {
   cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_post_lw); cudaFree(h->d_hio);
   if (h->s_own) cudaStreamDestroy(h->s_own);
   cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf); cudaFree(h->d_lc);
+  cudaFree(h->wl.t0); cudaFree(h->wl.step); cudaFree(h->wl.row_u[0]); cudaFree(h->wl.n_rows);
+  if (h->h_wl_nact) cudaFreeHost(h->h_wl_nact);
+  for (auto& e : h->wl_ev) if (e) cudaEventDestroy(e);
   if (h->h_stats) cudaFreeHost(h->h_stats);
   if (h->h_fin) cudaFreeHost(h->h_fin);
   for (auto& pr : h->prof_ev) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
@@ -740,6 +882,9 @@ int64_t ns_run_many(ns_handle** hs, int32_t n_runs, int32_t term_kind, double te
     if (!hs[r]->s_own && cudaStreamCreateWithFlags(&hs[r]->s_own, cudaStreamNonBlocking) != cudaSuccess)
       return fail(hs[r], -2, "cudaStreamCreate");
   }
+  // the runs step on streams of their own (non-blocking): everything the caller enqueued before -- on whatever stream -- must be
+  // complete first; the call returns with every run's stream idle
+  if (cudaDeviceSynchronize() != cudaSuccess) return fail(hs[0], -2, "cudaDeviceSynchronize");
   std::vector<char> active(n_runs, 1);
   std::vector<int64_t> it(n_runs, 0);
   std::vector<ns_stats> st(n_runs);
@@ -781,8 +926,11 @@ int ns_relbin_setup(ns_handle* h, const double* theta0_host, double chi, double 
   if (!theta0_host || !(chi > 0.0) || !(eps > 0.0) || h->cfg.n_freq < 2) return fail(h, -1, "bad arguments");
   cudaStream_t s = (cudaStream_t)stream;
   const int nf = h->cfg.n_freq, nd = h->cfg.n_det;
-  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
-  h->d_rb_edge = nullptr; h->d_rb_buf = nullptr; h->rb_nb = 0;
+  // the new set-up is built in buffers of its own and swapped into the handle only on success: a failed call leaves the earlier
+  // set-up (and a sampler that is using it, NSGW_OPT_LIKELIHOOD = 1) untouched
+  int* new_edge = nullptr;
+  double* new_buf = nullptr;
+  auto drop = [&](int rc) { cudaFree(new_edge); cudaFree(new_buf); return rc; };
   // ---- bin edges: given, or equally spaced in Delta(f) (reading L24)
   std::vector<int> edge;
   if (edges_host) {
@@ -809,9 +957,15 @@ int ns_relbin_setup(ns_handle* h, const double* theta0_host, double chi, double 
   const int nb = (int)edge.size() - 1;
   // ---- device buffers: A0, A1 [nd][nb] complex, B0, B1 [nd][nb], ig0 [nd][nb+1] complex, inv_w [nb], cb0 [CB_SIZE], theta0 [16]
   const size_t n_buf = (size_t)nd * nb * 6 + (size_t)nd * (nb + 1) * 2 + nb + CB_SIZE + 16;
-  CU_CHECK(h, cudaMalloc(&h->d_rb_edge, sizeof(int) * (nb + 1)));
-  CU_CHECK(h, cudaMalloc(&h->d_rb_buf, sizeof(double) * n_buf));
-  double* b = h->d_rb_buf;
+#define RB_CHECK(expr)                                                                            \
+  do {                                                                                            \
+    cudaError_t e_ = (expr);                                                                      \
+    if (e_ != cudaSuccess)                                                                        \
+      return drop(fail(h, e_ == cudaErrorMemoryAllocation ? -4 : -2, std::string(#expr) + ": " + cudaGetErrorString(e_))); \
+  } while (0)
+  RB_CHECK(cudaMalloc(&new_edge, sizeof(int) * (nb + 1)));
+  RB_CHECK(cudaMalloc(&new_buf, sizeof(double) * n_buf));
+  double* b = new_buf;
   double2* A0 = reinterpret_cast<double2*>(b); b += (size_t)nd * nb * 2;
   double2* A1 = reinterpret_cast<double2*>(b); b += (size_t)nd * nb * 2;
   double2* ig0 = reinterpret_cast<double2*>(b); b += (size_t)nd * (nb + 1) * 2;
@@ -820,28 +974,33 @@ int ns_relbin_setup(ns_handle* h, const double* theta0_host, double chi, double 
   double* inv_w = b; b += nb;
   double* cb0 = b; b += CB_SIZE;
   double* th0 = b;
-  CU_CHECK(h, cudaMemcpyAsync(h->d_rb_edge, edge.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, s));
-  CU_CHECK(h, cudaMemcpyAsync(th0, theta0_host, sizeof(double) * 11, cudaMemcpyHostToDevice, s));
+  RB_CHECK(cudaMemcpyAsync(new_edge, edge.data(), sizeof(int) * (nb + 1), cudaMemcpyHostToDevice, s));
+  RB_CHECK(cudaMemcpyAsync(th0, theta0_host, sizeof(double) * 11, cudaMemcpyHostToDevice, s));
   const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
   if (tf2) k_setup<1><<<1, 32, 0, s>>>(h->d_cfg, th0, 1, cb0);
   else k_setup<2><<<1, 32, 0, s>>>(h->d_cfg, th0, 1, cb0);
-  LAUNCH_CHECK(h);
-#define RB_SUMMARY(M, N) k_rb_summary<M, N><<<nb, 128, 0, s>>>(h->d_cfg, h->tb, cb0, h->d_rb_edge, nb, A0, A1, B0, B1, ig0, inv_w)
+  g_launches.fetch_add(1);
+#define RB_SUMMARY(M, N) k_rb_summary<M, N><<<nb, 128, 0, s>>>(h->d_cfg, h->tb, cb0, new_edge, nb, A0, A1, B0, B1, ig0, inv_w)
   if (tf2) { if (nd == 1) RB_SUMMARY(1, 1); else if (nd == 2) RB_SUMMARY(1, 2); else RB_SUMMARY(1, 3); }
   else { if (nd == 1) RB_SUMMARY(2, 1); else if (nd == 2) RB_SUMMARY(2, 2); else RB_SUMMARY(2, 3); }
 #undef RB_SUMMARY
-  LAUNCH_CHECK(h);
+  g_launches.fetch_add(1);
+  RB_CHECK(cudaGetLastError());
   double valid = 0.0;
-  CU_CHECK(h, cudaMemcpyAsync(&valid, cb0 + CB_VALID, sizeof(double), cudaMemcpyDeviceToHost, s));
-  CU_CHECK(h, cudaStreamSynchronize(s));
-  if (valid == 0.0) {
-    cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
-    h->d_rb_edge = nullptr; h->d_rb_buf = nullptr;
-    return fail(h, -1, "fiducial theta0 is unphysical");
-  }
+  RB_CHECK(cudaMemcpyAsync(&valid, cb0 + CB_VALID, sizeof(double), cudaMemcpyDeviceToHost, s));
+  RB_CHECK(cudaStreamSynchronize(s));
+#undef RB_CHECK
+  if (valid == 0.0) return drop(fail(h, -1, "fiducial theta0 is unphysical"));
+  cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf);
+  h->d_rb_edge = new_edge; h->d_rb_buf = new_buf;
   h->rb_nb = nb;
   h->rb.edge = h->d_rb_edge; h->rb.A0 = A0; h->rb.A1 = A1; h->rb.B0 = B0; h->rb.B1 = B1; h->rb.ig0 = ig0; h->rb.inv_w = inv_w; h->rb.nb = nb;
   if (n_bins_host) *n_bins_host = nb;
+  if (h->opt_like == 1 && h->cfg.n_live > 0) {   // a sampler already on relative binning: its live logL must refer to the new summary data
+    int rc = loglike_u(h, h->d_live_u, h->cfg.n_live, h->d_live_l, s);
+    if (rc) return rc;
+    CU_CHECK(h, cudaStreamSynchronize(s));
+  }
   return 0;
 }
 
@@ -944,6 +1103,7 @@ int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
   if (key == NSGW_OPT_BINS_KERNEL && value >= 0 && value <= 2) { h->opt_bins_kernel = value; return 0; }
   if (key == NSGW_OPT_WALK_SPEC && value >= 0 && value <= kWalkDMax) { h->opt_walk_spec = value; return 0; }
   if (key == NSGW_OPT_WALK_STAGE && (value == 0 || value == 1)) { h->opt_walk_stage = value; return 0; }
+  if (key == NSGW_OPT_WALK_KERNEL && value >= 0 && value <= 3) { h->opt_walk_kernel = value; return 0; }
   if (key == NSGW_OPT_INNER_KERNEL && (value == 0 || value == 1)) {
     if (value == 1 && h->opt_like == 1) return fail(h, -5, "the slice kernel evaluates the exact likelihood only");
     h->opt_inner = value;
@@ -956,9 +1116,10 @@ int nsgw_set_option(ns_handle* h, int32_t key, int32_t value) {
     if (value == 1 && h->rb_nb <= 0) return fail(h, -3, "ns_relbin_setup has not been called");
     h->opt_like = value;
     if (h->cfg.n_live > 0) {   // the live points' logL must come from the likelihood the sampler will compare against
+      CU_CHECK(h, cudaDeviceSynchronize());   // the call has no stream argument: order it after all pending work on any stream
       int rc = loglike_u(h, h->d_live_u, h->cfg.n_live, h->d_live_l, nullptr);
       if (rc) return rc;
-      CU_CHECK(h, cudaStreamSynchronize(nullptr));
+      CU_CHECK(h, cudaDeviceSynchronize());
     }
     return 0;
   }

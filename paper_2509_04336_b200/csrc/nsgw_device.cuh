@@ -279,8 +279,17 @@ enum {
   CB_AI = 45,        // inspiral amplitude: degree-9 polynomial in x = f^1/3              (10)
   CB_AH = 55,        // intermediate amplitude: f1, 1/(f3-f1), quartic h0..h4             (7)
   CB_AM = 62,        // merger-ringdown amplitude: f_rd, g1, wh^2, -gamma2/wh             (4)
+  CB_FMR = 66,       // PhenomD-form: max(CB_FP2, CB_FA2) [Hz]: from here up both phase and amplitude are merger-ringdown
   CB_SIZE = 68
 };
+
+// First bin of the branch-free merger-ringdown loops for a region boundary fs [Hz]: every bin k >= k_mr has f_k >= fs (two bins of
+// margin against the rounding of f_k); the bins below go through the general (piecewise) evaluation.
+__device__ __forceinline__ int mr_first_bin(double fs, double f_min, double df, int nf) {
+  const double ks = (fs - f_min) / df + 2.0;
+  if (!(ks < (double)nf)) return nf;
+  return (int)fmax(ks, 0.0) + 1;
+}
 
 struct DetResp { double fp, fx, dt; };
 
@@ -488,6 +497,7 @@ __device__ bool setup_particle(const DevCfg& cfg, const double* th, double* cb) 
   cb[CB_FP2] = Fb / M;
   cb[CB_FA1] = 0.014 / M;
   cb[CB_FA2] = Fpeak / M;
+  cb[CB_FMR] = fmax(Fb, Fpeak) / M;
 
   // -- amplitude --------------------------------------------------------------------------------------
   double A[7];

@@ -47,7 +47,7 @@ EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglik
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
 
 # nsgw_set_option keys (include/nsgw.h)
-OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS = 0, 1, 2, 3, 4
+OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS, OPT_WALK_STAGE, OPT_WALK_KERNEL = 0, 1, 2, 3, 4, 5, 6
 
 _lib = None
 
