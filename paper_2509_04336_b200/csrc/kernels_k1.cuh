@@ -386,9 +386,13 @@ struct LpSmem {
 
 template <int NDET, int NT, int KR, int PP, int UNR, int OCC>
 __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
-                                                     long long B, int kr /*bins per range, <= KR, multiple of UNR*/, int nranges,
-                                                     long long ntasks, double* __restrict__ partial) {
+                                                     long long B_host, const int* __restrict__ B_dev /*overrides the row count; B_host
+                                                     stays the stride of `partial`*/, int kr /*bins per range, <= KR, multiple of UNR*/,
+                                                     int nranges, long long ntasks_host, double* __restrict__ partial) {
   using AL = AccLayout<1, NDET>;
+  const long long B = B_dev ? (long long)*B_dev : B_host;
+  const long long ntasks = B_dev ? (B + NT * PP - 1) / (NT * PP) * nranges : ntasks_host;
+  if (blockIdx.x >= ntasks) return;
   constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) LpSmem<NDET, KR> sm;
   __shared__ MathTables mtab;
@@ -483,7 +487,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       const long long p = (grp * PP + j) * NT + tid;
       if (p < B) {
 #pragma unroll
-        for (int i = 0; i < AL::N; ++i) partial[((long long)rng * AL::N + i) * B + p] = acc[j][i];   // [range][N][B]: coalesced
+        for (int i = 0; i < AL::N; ++i) partial[((long long)rng * AL::N + i) * B_host + p] = acc[j][i];   // [range][N][stride]: coalesced
       }
     }
   }

@@ -15,13 +15,15 @@
 // with, and the speculative steps after an acceptance are redone from the accepted point with the same Philox counters.
 #pragma once
 
-constexpr int kWlWarps = 4;          // walkers per CTA of k_wl_head
+constexpr int kWlWarps = 2;          // walkers per CTA of k_wl_head
+constexpr int kWlEMax = 64;          // rows per walker and round (cap)
 
 struct WlState {
   int* t0;                // [B] steps consumed
   int* E;                 // [B] in-bounds proposals the walker asks for in its next chunk (adaptive: halved after a chunk with an
                           //     acceptance, doubled after one without; or fixed)
   int* nsteps;            // [B] steps of the pending chunk
+  int* nslots;            // [B] in-bounds proposals (rows) of the pending chunk
   int* rowbase;           // [B] first row of the pending chunk in its round's row buffers
   int* cnt;               // [3 B] accepted, evaluated, out-of-bounds
   unsigned char* step;    // [B][kWalkSteps] per step of the pending chunk: 0 out of bounds, else slot + 1
@@ -31,20 +33,22 @@ struct WlState {
   double* row_logl[2];    // [R]
   int* n_rows;            // [2] rows of the round (by parity)
   int* n_active;          // [2] walkers that proposed in the round (by parity)
-  int e_cap;              // rows per walker and round (<= kWalkDMax)
+  int* sum_need;          // [3] by round mod 3: rows the batch still needs (sum over walkers of remaining steps x in-bounds fraction)
+  int e_cap;              // rows per walker and round (<= kWlEMax)
+  int r_target;           // rows per round the chunk lengths aim for
 };
 
 template <int MODEL>
 __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restrict__ cfgp, WalkArgs a, WlState st, int round) {
   __shared__ double s_stage[kWlWarps][32][kMaxDim];
-  __shared__ double s_prop[kWlWarps][kWalkDMax][kMaxDim];
+  __shared__ double s_prop[kWlWarps][kWlEMax][kMaxDim];
   __shared__ double s_cur[kWlWarps][kMaxDim];
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const long long row = blockIdx.x * (long long)kWlWarps + wrp;
   const int par = round & 1;
-  if (blockIdx.x == 0 && threadIdx.x == 0) { st.n_rows[par ^ 1] = 0; st.n_active[par ^ 1] = 0; }
+  if (blockIdx.x == 0 && threadIdx.x == 0) { st.n_rows[par ^ 1] = 0; st.n_active[par ^ 1] = 0; st.sum_need[(round + 1) % 3] = 0; }
   if (row >= a.B) return;
   const int W = a.W_dev ? *a.W_dev : a.W;
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
@@ -52,6 +56,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
   const bool spec_fixed = a.spec_fixed != 0;
   const int spec = max(1, min(st.e_cap, a.spec));
   int t0, E;
+  double inb = 0.25;                    // in-bounds fraction of the walker's proposals (estimate: its last chunk)
   if (round == 0) {
     t0 = 0;
     E = spec_fixed ? spec : min(spec, 2);
@@ -62,6 +67,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
     E = st.E[row];
     const int nsteps = st.nsteps[row];
     if (nsteps > 0) {
+      inb = fmax((double)st.nslots[row], 0.5) / nsteps;
       const int rb = st.rowbase[row];
       const double* rl = st.row_logl[par ^ 1];
       const unsigned char* stp = st.step + row * kWalkSteps;
@@ -118,7 +124,18 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
   int nslots = 0, nsteps = 0;
   int rowbase = 0;
   if (t0 < W) {
-    const int emax = E;
+    // Chunk length.  The walkers differ in how many of their W steps are in bounds, i.e. in how many rows they still need; lengths
+    // in proportion to that need make them finish in the same round, with about r_target rows per round over the batch (the need
+    // of the batch is last round's sum).  The walker's own halve-after-a-hit / double-after-a-miss length caps it: where
+    // acceptances are frequent, long chunks are mostly discarded.  Any choice gives the same chain.
+    const int need = max(1, (int)ceil((W - t0) * inb));
+    if (lane == 0) atomicAdd(&st.sum_need[round % 3], need);
+    int emax = E;
+    if (!spec_fixed) {
+      const double tot = (round == 0) ? 0.25 * (double)W * (double)a.B : (double)st.sum_need[(round + 2) % 3];
+      const int e_pol = (int)ceil(need * (double)st.r_target / fmax(tot, (double)st.r_target));
+      emax = max(1, min(E, min(spec, e_pol)));
+    }
     unsigned char* stp = st.step + row * kWalkSteps;
     while (nslots < emax && nsteps < kWalkSteps && t0 + nsteps < W) {
       const int j = nsteps + lane;
@@ -145,21 +162,21 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
     if (lane == 0 && nslots > 0) rowbase = atomicAdd(&st.n_rows[par], nslots);
     rowbase = __shfl_sync(0xffffffffu, rowbase, 0);
     // prior transform and waveform set-up, one row per lane
-    if (lane < nslots) {
-      double* ru = st.row_u[par] + (size_t)(rowbase + lane) * kMaxDim;
+    for (int sl = lane; sl < nslots; sl += 32) {
+      double* ru = st.row_u[par] + (size_t)(rowbase + sl) * kMaxDim;
       double th[11];
 #pragma unroll
       for (int d = 0; d < 11; ++d) {
-        const double x = s_prop[wrp][lane][d];
+        const double x = s_prop[wrp][sl][d];
         ru[d] = x;
         th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], x);
       }
-      setup_particle<MODEL>(cfg, th, st.row_cb[par] + (size_t)(rowbase + lane) * CB_SIZE);
+      setup_particle<MODEL>(cfg, th, st.row_cb[par] + (size_t)(rowbase + sl) * CB_SIZE);
     }
     if (lane == 0) atomicAdd(&st.n_active[par], 1);
   }
   if (lane == 0) {
-    st.t0[row] = t0; st.E[row] = E; st.nsteps[row] = nsteps; st.rowbase[row] = rowbase;
+    st.t0[row] = t0; st.E[row] = E; st.nsteps[row] = nsteps; st.nslots[row] = nslots; st.rowbase[row] = rowbase;
   }
 }
 

@@ -178,6 +178,7 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 #endif
 constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
 constexpr long long kLpMinBatch = 1024;   // below this the CTA-per-particle kernel fills the machine better
+constexpr long long kPdMinBatch = 32768;  // PhenomD-form: k_pd_lp overtakes k_bins only at large batches (measured: 40 vs 36 M evals/s at 65536)
 
 int ensure_partial(ns_handle* h, size_t n) {
   if (n > h->partial_cap) {
@@ -189,8 +190,9 @@ int ensure_partial(ns_handle* h, size_t n) {
   return 0;
 }
 
+// cbs [B][CB_SIZE]; rows_dev (optional, device) overrides the row count of the task lists (B is then the capacity).
 template <int NDET>
-int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
+int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
   using AL = AccLayout<1, NDET>;
   constexpr int NT = kLpNT, PP = kLpPP;
   const long long ngroups = (B + NT * PP - 1) / (NT * PP);
@@ -220,11 +222,16 @@ int launch_bins_lp(ns_handle* h, long long B, double* logl, double* parts, cudaS
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, kr, nranges, ntasks,
+  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, cbs, B, rows_dev, kr, nranges, ntasks,
                                                                               h->d_partial);
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
-  k_finish<1, NDET><<<(unsigned)((B + 127) / 128), 128, 0, s>>>(h->d_cfg, h->d_cb, h->d_partial, nranges, B, logl, parts);
+  if (rows_dev) {
+    const long long gfin = std::min<long long>((B + 127) / 128, (long long)h->n_sm * 8);
+    k_finish_rows<1, NDET><<<(unsigned)gfin, 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges, B, rows_dev, B, logl, parts);
+  } else {
+    k_finish<1, NDET><<<(unsigned)((B + 127) / 128), 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges, B, logl, parts);
+  }
   LAUNCH_CHECK(h);
   return 0;
 }
@@ -236,7 +243,7 @@ int pd_pick_kr(const ns_handle* h, long long rows) {
   const long long slots = (long long)h->n_sm * kPdOCC;
   int kr = kPdKT;
   double best = 1e300;
-  for (int c = kPdKT; c <= 1024; c += kPdKT) {
+  for (int c = 2 * kPdKT; c <= 384; c += kPdKT) {
     const int nr = (h->cfg.n_freq + c - 1) / c;
     const long long nt = ngroups * nr;
     const double cost = (double)((nt + slots - 1) / slots) * (c + 24) + 0.25 * nr;
@@ -257,8 +264,11 @@ int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* row
   PdArgs a;
   a.cbs = cbs; a.n_rows = rows; a.n_rows_dev = rows_dev; a.stride = rows; a.kr = kr; a.nranges = nranges; a.partial = h->d_partial;
   const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
-  const long long ntasks = ngroups * nranges + (rows + (kPdNT / 32) * kPdLowPer - 1) / ((kPdNT / 32) * kPdLowPer);
+  const long long ntasks = ngroups * nranges;
   const long long grid = std::min<long long>(ntasks, (long long)h->n_sm * kPdOCC);
+  const long long glow = std::min<long long>((rows + kPdLowNT / 32 - 1) / (kPdLowNT / 32), (long long)h->n_sm * kPdLowOCC * 4);
+  k_pd_low<NDET><<<(unsigned)glow, kPdLowNT, 0, s>>>(h->d_cfg, h->tb, a);
+  LAUNCH_CHECK(h);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (h->prof && h->prof_ev.size() < 4096) {
     cudaEventCreate(&e0); cudaEventCreate(&e1);
@@ -276,8 +286,8 @@ int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* row
 template <int MODEL, int NDET>
 int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaStream_t s) {
   if (MODEL == 1 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kLpMinBatch)))
-    return launch_bins_lp<NDET>(h, B, logl, parts, s);
-  if (MODEL == 2 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kLpMinBatch)))
+    return launch_bins_lp<NDET>(h, h->d_cb, B, nullptr, logl, parts, s);
+  if (MODEL == 2 && (h->opt_bins_kernel == 2 || (h->opt_bins_kernel == 0 && B >= kPdMinBatch)))
     return launch_pd_lp<NDET>(h, h->d_cb, B, nullptr, 0, logl, parts, s);
   int P = pick_p(B);
   cudaEvent_t e0 = nullptr, e1 = nullptr;
@@ -416,15 +426,17 @@ int ensure_wl(ns_handle* h, long long B, long long R) {
   if (!h->h_wl_nact) {
     CU_CHECK(h, cudaMallocHost(&h->h_wl_nact, sizeof(int) * 4));
     for (auto& e : h->wl_ev) CU_CHECK(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
-    CU_CHECK(h, cudaMalloc(&h->wl.n_rows, sizeof(int) * 4));
+    CU_CHECK(h, cudaMalloc(&h->wl.n_rows, sizeof(int) * 8));
     h->wl.n_active = h->wl.n_rows + 2;
+    h->wl.sum_need = h->wl.n_rows + 4;
   }
   if (B > h->wl_cap_b) {
     cudaFree(h->wl.t0); cudaFree(h->wl.step);
     h->wl.t0 = nullptr; h->wl.step = nullptr; h->wl_cap_b = 0;
-    CU_CHECK(h, cudaMalloc(&h->wl.t0, sizeof(int) * 7 * (size_t)B));
+    CU_CHECK(h, cudaMalloc(&h->wl.t0, sizeof(int) * 8 * (size_t)B));
     CU_CHECK(h, cudaMalloc(&h->wl.step, (size_t)B * kWalkSteps));
-    h->wl.E = h->wl.t0 + B; h->wl.nsteps = h->wl.t0 + 2 * B; h->wl.rowbase = h->wl.t0 + 3 * B; h->wl.cnt = h->wl.t0 + 4 * B;
+    h->wl.E = h->wl.t0 + B; h->wl.nsteps = h->wl.t0 + 2 * B; h->wl.rowbase = h->wl.t0 + 3 * B; h->wl.nslots = h->wl.t0 + 4 * B;
+    h->wl.cnt = h->wl.t0 + 5 * B;
     h->wl_cap_b = B;
   }
   if (R > h->wl_cap_r) {
@@ -445,6 +457,7 @@ int ensure_wl(ns_handle* h, long long B, long long R) {
 template <int MODEL, int NDET>
 int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, double* logl, cudaStream_t s) {
   if (MODEL == 2 && h->opt_walk_kernel == 3) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
+  if (MODEL == 1 && R >= kLpMinBatch && h->opt_walk_kernel != 2) return launch_bins_lp<NDET>(h, cbs, R, rows_dev, logl, nullptr, s);
   if (R >= 4096) k_bins<MODEL, NDET, 2><<<(unsigned)((R + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
   else k_bins<MODEL, NDET, 1><<<(unsigned)R, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
   LAUNCH_CHECK(h);
@@ -455,18 +468,19 @@ template <int MODEL, int NDET>
 int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const long long B = a.B;
   // rows per walker and round: up to 32 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
-  const int e_cap = (int)std::max<long long>(1, std::min<long long>(kWalkDMax, 65536 / B));
+  const int e_cap = (int)std::max<long long>(1, std::min<long long>(kWlEMax, 65536 / B));
   const long long R = B * e_cap;
   int rc = ensure_wl(h, B, R);
   if (rc) return rc;
-  if (h->wl_kr == 0) h->wl_kr = pd_pick_kr(h, (long long)std::max(2, h->cfg.n_delete) * kWalkDMax);
+  if (h->wl_kr == 0) h->wl_kr = 128;   // short ranges: the rows of a round vary, many small tasks keep the persistent grid balanced
   WlState st = h->wl;
   st.e_cap = e_cap;
-  CU_CHECK(h, cudaMemsetAsync(st.n_rows, 0, sizeof(int) * 4, s));
+  st.r_target = (int)std::min<long long>(R, std::max<long long>(16384, 24 * B));
+  CU_CHECK(h, cudaMemsetAsync(st.n_rows, 0, sizeof(int) * 8, s));
   const unsigned gh = (unsigned)((B + kWlWarps - 1) / kWlWarps);
   for (long long r = 0;; ++r) {
     const int par = (int)(r & 1);
-    k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, (int)std::min<long long>(r, 2 + par));   // only "first round or not" and the parity matter
+    k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, (int)std::min<long long>(r, 6 + r % 6));   // first round or not, parity and round mod 3 matter
     LAUNCH_CHECK(h);
     CU_CHECK(h, cudaMemcpyAsync(h->h_wl_nact + (r & 3), st.n_active + par, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(h, cudaEventRecord(h->wl_ev[r & 3], s));
@@ -749,7 +763,7 @@ int ns_walk_batch(ns_handle* h, const double* donors_u_dev, int32_t m, double* u
   a.k0 = (uint32_t)(seed & 0xFFFFFFFFull); a.k1 = (uint32_t)(seed >> 32); a.stream_id = stream_id; a.slot0 = slot0;
   a.n_accept = n_accept_dev; a.n_eval = n_eval_dev; a.n_oob = n_oob_dev; a.tflags = trace_flags_dev; a.tlogl = trace_logl_dev;
   a.trace_stride = walk_len;
-  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
+  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWlEMax;   // (k_walk_gw clamps it to its own 32-slot buffers)
   a.spec_fixed = h->opt_walk_spec > 0;
   a.stage = h->opt_walk_stage;
   return launch_walk(h, a, (cudaStream_t)stream);
@@ -791,7 +805,7 @@ int step_enqueue(ns_handle* h, double* dead_dev, cudaStream_t s) {
   memset(&a, 0, sizeof(a));
   a.donors = h->d_surv; a.m = m; a.u = h->d_cur_u; a.logl = h->d_cur_l; a.B = k;
   a.lstar_dev = &h->d_state->lstar; a.W_dev = &h->d_state->W; a.iter_dev = &h->d_state->iter;
-  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWalkDMax;
+  a.spec = h->opt_walk_spec > 0 ? h->opt_walk_spec : kWlEMax;
   a.spec_fixed = h->opt_walk_spec > 0;
   a.stage = h->opt_walk_stage;
   a.k0 = k0; a.k1 = k1; a.stream_id = 0u; a.slot0 = 0;
