@@ -33,8 +33,52 @@ def alg_flops_per_bin(n_det, model="taylorf2"):
     FMA = 2: 9-FMA phase (18); table-driven sincos: exact reduction (F2I, I2F on the conversion pipe + 1 subtraction), r^2 (1),
     sin 2 FMA + 1 mul (5), cos 3 FMA (6), complex product with the table entry (6) = 19; detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex
     Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
+    if model == "phenomd":
+        # merger-ringdown bin (about 80 % of the bins) of the CTA-per-row sweep the worklist walk uses (DESIGN.md section 5): phase 47,
+        # amplitude 32 + 3, table-driven sincos 21, detector 0: 10, every further detector 18
+        return 47 + 35 + 21 + 10 + 18 * (n_det - 1)
     assert model == "taylorf2"
     return 18 + 19 + 8 + 14 * (n_det - 1)
+
+
+def _profile_key(name):
+    m = __import__("re").match(r"r(\d+)([a-z]*)_", name)
+    return (int(m.group(1)), len(m.group(2)), m.group(2)) if m else (-1, 0, "")
+
+
+def traffic_from_profile(kernel="k_bins_lp"):
+    """DRAM bytes per launch of the dominant kernel (dram__bytes_read.sum + dram__bytes_write.sum) read from the newest committed
+    `ncu --set full` summary of it under profiles/ (text; the file's first line is the command that made it).  (bytes, file)."""
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", f"r*_{kernel}_ncu_full.txt")), key=lambda q: _profile_key(os.path.basename(q)))
+    if not files:
+        return None, None
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot, seen = 0.0, 0
+    for line in open(files[-1]):
+        f = line.split()
+        if len(f) == 3 and f[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and f[1] in unit:
+            tot += float(f[2]) * unit[f[1]]
+            seen += 1
+    return (tot, os.path.relpath(files[-1], ROOT)) if seen == 2 else (None, None)
+
+
+def spawn_command(n_gpus, argv, port=None):
+    """`bench.py --gpus N` started without a launcher re-executes itself under torch.distributed.run, one rank per GPU."""
+    port = port or (29500 + os.getpid() % 2000)
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n_gpus}", "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.join(ROOT, "bench.py")] + list(argv)
+
+
+def resolve_world(args, environ):
+    """What --gpus means, for both arms: the number of ranks of the job.  Returns "run" (this process is a rank of a job of that
+    size, or N = 1), "spawn" (N > 1 and no launcher: start N ranks) or raises SystemExit when the flag contradicts the launcher."""
+    ws = environ.get("WORLD_SIZE")
+    if ws is None:
+        return "run" if args.gpus <= 1 else "spawn"
+    if int(ws) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={ws} ranks")
+    return "run"
 
 
 class ClockSampler:
@@ -126,7 +170,7 @@ def run_reference(args):
         P.gw_loglike(theta)
     dt = time.perf_counter() - t0
     val = args.steps * B / dt
-    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": int(os.environ.get("WORLD_SIZE", "1")), "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"config2 gw_loglike_batch TaylorF2 H1+L1 4017 bins, bounded sample of {B} rows per step (CPU oracle)"},
@@ -173,29 +217,38 @@ def run_ours(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
     stream = torch.cuda.current_stream()
 
-    def step():
-        h.gw_loglike_batch(theta, out=logl)
+    def timed(nrows, steps, clocks=False):
+        """`steps` timed gw_loglike_batch calls over the first nrows rows: L2 flushed before every call (outside its event pair),
+        CUDA events on the launching stream, max over ranks.  Returns (ms total, dominant-kernel ms total, its launches, library
+        launches, clock summary)."""
+        th_n, out_n = theta[:nrows], logl[:nrows]
+        for _ in range(max(args.warmup, 3)):
+            h.gw_loglike_batch(th_n, out=out_n)
+        barrier()
+        n0 = nsgw.launch_count()
+        h.profile_enable(True)
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        with ClockSampler(local) as clk:
+            barrier()
+            for a, b in ev:
+                flush.zero_()                       # L2 flush between timed iterations (outside the event pair)
+                a.record(stream)
+                h.gw_loglike_batch(th_n, out=out_n)
+                b.record(stream)
+            barrier()
+        h.profile_enable(False)
+        nl = nsgw.launch_count() - n0
+        t = D.max_over_ranks(sum(a.elapsed_time(b) for a, b in ev), "cuda")
+        k_ms, k_n = h.profile_read()
+        return t, k_ms, k_n, nl, clk.summary()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    n0 = nsgw.launch_count()
-    h.profile_enable(True)
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    with ClockSampler(local) as clk:
-        barrier()
-        for a, b in ev:
-            flush.zero_()                       # L2 flush between timed iterations (outside the event pair)
-            a.record(stream)
-            step()
-            b.record(stream)
-        barrier()
-    h.profile_enable(False)
-    launches = nsgw.launch_count() - n0
-    ms = sum(a.elapsed_time(b) for a, b in ev)
-    ms = D.max_over_ranks(ms, "cuda")
+    # batch sizes BASELINE.json lists for config 2, same method each; the largest is the headline step
+    sweep_B = sorted({b for b in (1024, 16384, 65536) if b < B} | {B})
+    sweep_raw = {}
+    for b in sweep_B:
+        sweep_raw[b] = timed(b, args.steps if b == B else max(20, args.steps // 2))
+    ms, kern_ms, kern_n, launches, clocks = sweep_raw[B]
     value = world * B * args.steps / (ms * 1e-3)
-    kern_ms, kern_n = h.profile_read()
 
     # ---- end to end through the host-buffer C-ABI call: pinned theta -> H2D -> set-up + bin sweep -> D2H logL, all timed
     th_host = theta.cpu().pin_memory()
@@ -213,19 +266,20 @@ def run_ours(args):
     barrier()
     e2e_s = D.max_over_ranks(time.perf_counter() - t0, "cuda")
     e2e_val = world * B * args.steps / e2e_s
-    assert torch.equal(out_host, logl.cpu())
+    e2e_diff = float((out_host - logl.cpu()).abs().max())
+    assert e2e_diff == 0.0, e2e_diff        # same kernels, same launch geometry: the identical numbers
 
     line = None
+    fp64_burst = nsgw.measure_fp64_peak(1 << 17) if rank == 0 else None
     if rank == 0:
         peaks = measured_peaks()
-        fp64_burst = nsgw.measure_fp64_peak(1 << 17)
         flops_launch = float(B) * n_freq * alg_flops_per_bin(n_det)
         ach = flops_launch / (kern_ms / kern_n * 1e-3) / 1e12
         # DRAM bytes per launch of the dominant kernel: dram__bytes_read.sum + dram__bytes_write.sum of the committed
         # `ncu --set full` capture of this same command (profiles/r01ad_k_bins_lp_ncu_full.txt); only valid for the default batch
-        traffic = (19319552 + 84992) if (B == 65536 and n_freq == 4017) else None
+        traffic, traffic_file = traffic_from_profile("k_bins_lp") if (B == 65536 and n_freq == 4017) else (None, None)
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
-                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write); algorithmic 96 B x B = %d" % (96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
                 "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
                 "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,
@@ -235,9 +289,21 @@ def run_ours(args):
                 "dtype": "f64", "data": "synthetic",
                 "config": {"workload": f"config2 gw_loglike_batch TaylorF2 H1+L1 {n_freq} bins x {n_det} det, B={B} rows per GPU",
                            "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"rows sharded x{world}, no collective"},
-                "clocks": clk.summary(),
-                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": B * 11 * 8, "d2h_bytes_per_step": B * 8},
+                "clocks": clocks,
+                "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": B * 11 * 8, "d2h_bytes_per_step": B * 8,
+                        "max_abs_dlogl_vs_device_call": e2e_diff},
                 "gpu_launches": int(launches), "roofline": roof}
+        bs = []
+        for b in sweep_B:
+            t, k_ms, k_n, _, ck = sweep_raw[b]
+            nst = args.steps if b == B else max(20, args.steps // 2)
+            fl = float(b) * n_freq * alg_flops_per_bin(n_det)
+            bs.append({"B": b, "ms_per_step": t / nst, "evals_per_s": world * b * nst / (t * 1e-3), "sweep_kernel_ms": k_ms / max(k_n, 1),
+                       "frac_fp64_peak_step": fl / (t / nst * 1e-3) / 1e12 / fp64_burst,
+                       "frac_fp64_peak_sweep_kernel": fl / (k_ms / max(k_n, 1) * 1e-3) / 1e12 / fp64_burst, "sm_mhz": ck["sm_mhz"]})
+        line["batch_sweep"] = {"what": "config 2 (BASELINE.json: B in {1024, 16384, 65536}); same flush + CUDA-event method per size; "
+                                       "fractions of the FP64 peak measured in this run, %d flops per particle-bin" % alg_flops_per_bin(n_det),
+                               "points": bs}
 
     # ---- extras (rank 0, N=1 only): walk throughput and one full nested-sampling run
     if rank == 0 and world == 1 and not args.quick:
@@ -274,6 +340,64 @@ def run_ours(args):
                                     "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
                                     "evals_per_s": st["n_eval_total"] / wall}
         h3.close()
+        # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
+        spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
+        h4 = nsgw.Handle(spec4, smp4, seed=1)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        nit, st = h4.run(smp4["term_kind"], smp4["term_tol"], 4000)
+        logz, err, H = h4.finalize_evidence()
+        wall = time.perf_counter() - t0
+        extras["ns_run_config4"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
+                                    "logz_err": err, "H": H, "walk_len_last": st["walk_len"],
+                                    "accept_mean_last": st["accept_mean"], "evals_per_s": st["n_eval_total"] / wall}
+        h4.close()
+        # first iteration of both runs alone (same seed, same live set: the step the oracle is timed on below)
+        first = {}
+        for name, sp_, sm_ in (("config3", spec3, smp3), ("config4", spec4, smp4)):
+            hf = nsgw.Handle(sp_, sm_, seed=1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            stf = hf.step()
+            first[name] = {"ms": 1e3 * (time.perf_counter() - t0), "walk_len": stf["walk_len"], "n_eval": stf["n_eval"], "n_oob": stf["n_oob"]}
+            hf.close()
+        extras["ns_step_first_iteration"] = first
+        # config 5: divergence and saturation sweep (H1+L1+V1, 16 s at 4096 Hz, 32449 bins): B walkers against a live set of 2B
+        # points scattered about the injection, the lower half deleted, W in {20, 60, 200}, no adaptation.  The whole grid of
+        # BASELINE.json (10 batch sizes x 3 walk lengths); a point is skipped only if the time budget of the sweep runs out.
+        spec5 = W.config5(wf_cuda_for(nsgw, torch))
+        h5 = nsgw.Handle(spec5)
+        fl5 = alg_flops_per_bin(3, "phenomd") * spec5["n_freq"]
+        sweep, skipped = [], []
+        t_sweep = time.perf_counter()
+        for Bw in (256, 512, 1024, 2048, 4096, 8192, 16384, 32768, 65536, 131072):
+            u5 = torch.as_tensor(W.config5_live(spec5, 2 * Bw)).cuda()
+            l5 = h5.loglike_u_batch(u5)
+            order = torch.argsort(l5)
+            donors = u5[order[Bw:]].contiguous()
+            lstar = float(l5[order[Bw - 1]])
+            occ, ctas = h5.sweep_occupancy(min(65536, 64 * Bw))
+            for Wl in (20, 60, 200):
+                if time.perf_counter() - t_sweep > args.sweep_budget_s:
+                    skipped.append([Bw, Wl])
+                    continue
+                uw, lw = donors.clone(), l5[order[Bw:]].clone()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                cnt = h5.walk_batch(donors, uw, lw, lstar, Wl, 4321, 9)
+                b.record(stream)
+                torch.cuda.synchronize()
+                ne, na = int(cnt["n_eval"].sum()), cnt["n_accept"].double()
+                wms = a.elapsed_time(b)
+                sweep.append({"B": Bw, "W": Wl, "ms": wms, "evals": ne, "evals_per_s": ne / (wms * 1e-3),
+                              "accept_mean": float(na.mean()), "accept_std": float(na.std()), "accept_min": int(na.min()),
+                              "accept_max": int(na.max()), "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl),
+                              "warps_active_sweep_kernel": occ, "frac_fp64_peak": ne * fl5 / (wms * 1e-3) / 1e12 / fp64_burst})
+        extras["config5_sweep"] = {"what": "ns_walk_batch, PhenomD-form, 3 detectors x 32449 bins; warps_active = resident warps / 64 of "
+                                           "the row-sweep kernel (occupancy API x grid fill at the rows of a full round); frac_fp64_peak = "
+                                           "%d model flops per particle-bin x bins x evaluations / time / measured peak" % alg_flops_per_bin(3, "phenomd"),
+                                   "points": sweep, "skipped_for_time": skipped}
+        h5.close()
         if args.full_extras:
             # config 3 on the relative-binning likelihood (fiducial = the injection, eps = 0.5), and the batched
             # relative-binning evaluation on the config-2 data
@@ -433,43 +557,6 @@ def run_ours(args):
                                                          "logx": st["logx"]}
             hk.close()
             extras["gw_sequential_limit"] = gseq
-            # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
-            spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
-            h4 = nsgw.Handle(spec4, smp4, seed=1)
-            t0 = time.perf_counter()
-            nit, st = h4.run(smp4["term_kind"], smp4["term_tol"], 4000)
-            logz, err, H = h4.finalize_evidence()
-            wall = time.perf_counter() - t0
-            extras["ns_run_config4"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz,
-                                        "logz_err": err, "H": H, "walk_len_last": st["walk_len"],
-                                        "accept_mean_last": st["accept_mean"], "evals_per_s": st["n_eval_total"] / wall}
-            h4.close()
-            # config 5: divergence and saturation sweep (H1+L1+V1, 16 s at 4096 Hz, 32449 bins); B walkers, live set of 2B points
-            spec5 = W.config5(wf_cuda_for(nsgw, torch))
-            h5 = nsgw.Handle(spec5)
-            sweep = []
-            for Bw in (256, 1024, 4096, 16384, 65536, 131072):
-                u5 = torch.as_tensor(W.config5_live(spec5, 2 * Bw)).cuda()
-                l5 = h5.loglike_u_batch(u5)
-                order = torch.argsort(l5)
-                donors = u5[order[Bw:]].contiguous()
-                lstar = float(l5[order[Bw - 1]])
-                for Wl in (20, 60, 200):
-                    if Bw * Wl > 131072 * 20:          # keep the sweep within ~1 min: larger products are extrapolations of these
-                        continue
-                    uw, lw = donors.clone(), l5[order[Bw:]].clone()
-                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                    a.record(stream)
-                    cnt = h5.walk_batch(donors, uw, lw, lstar, Wl, 4321, 9)
-                    b.record(stream)
-                    torch.cuda.synchronize()
-                    ne, na = int(cnt["n_eval"].sum()), cnt["n_accept"].double()
-                    wms = a.elapsed_time(b)
-                    sweep.append({"B": Bw, "W": Wl, "ms": wms, "evals": ne, "evals_per_s": ne / (wms * 1e-3),
-                                  "accept_mean": float(na.mean()), "accept_std": float(na.std()), "accept_min": int(na.min()),
-                                  "accept_max": int(na.max()), "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl)})
-            extras["config5_sweep"] = sweep
-            h5.close()
             # PP test (stand-in for the paper's 100-injection study): config-3 shape, priors, PSD and sampler
             # settings; injections drawn from the prior, each in its own noise; credible levels of the injected values from the
             # weighted posterior (ns_posterior); KS test of uniformity per parameter
@@ -521,6 +608,34 @@ def run_ours(args):
         line["cpu_baseline"] = {"value": nb / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
                                 "sample": f"first {nb} of the {B} rows x {args.cpu_passes} passes, OpenMP over rows, {dt * args.cpu_passes:.1f} s of CPU work",
                                 "max_abs_dlogl_vs_gpu": float(np.max(np.abs(lg - lo)))}
+        if not args.quick:
+            # the oracle's sampler on the first iteration of configs 3 and 4 (same seed: same live set, walk length and proposals as
+            # the device step above), and its full runs EXTRAPOLATED from that rate to the device runs' evaluation counts
+            ex = line["extras"]
+            steps = {}
+            for name, sp_, sm_, run in (("config3", spec3, smp3, ex["ns_run_config3"]), ("config4", spec4, smp4, ex["ns_run_config4"])):
+                Po = O.OracleProblem(sp_)
+                t0 = time.perf_counter()
+                So = O.OracleSampler(Po, sm_["n_live"], sm_["n_delete"], sm_["naccept"], sm_["maxmcmc"], sm_["walks0"], sm_["delay"], seed=1)
+                t_init = time.perf_counter() - t0
+                t0 = time.perf_counter()
+                so = So.step()
+                t_step = time.perf_counter() - t0
+                rate = so["n_eval"] / t_step
+                dev = ex["ns_step_first_iteration"][name]
+                steps[name] = {"oracle_step_s": t_step, "oracle_init_live_s": t_init, "walk_len": so["walk_len"], "n_eval": so["n_eval"],
+                               "oracle_evals_per_s": rate, "device_step_ms": dev["ms"],
+                               "same_step_as_device": [so["walk_len"], so["n_eval"], so["n_oob"]] == [dev["walk_len"], dev["n_eval"], dev["n_oob"]],
+                               "device_run_wall_s": run["wall_s"], "device_run_evals": run["n_eval_total"],
+                               "oracle_run_wall_s_extrapolated": run["n_eval_total"] / rate,
+                               "note": "extrapolation: device run's likelihood evaluations / oracle evaluations per second on this step"}
+            gold = os.path.join(ROOT, "tests", "golden", "config3_oracle_run.json")
+            if os.path.exists(gold):
+                g = json.load(open(gold))
+                steps["config3"]["oracle_full_run_stored"] = {"wall_s": g["wall_s"], "threads": g["threads"], "iterations": g["iterations"],
+                                                              "n_eval_total": g["n_eval_total"], "logz": g["logz"], "logz_err": g["logz_err"],
+                                                              "file": "tests/golden/config3_oracle_run.json (oracle/make_baseline.py; another machine's cores)"}
+            line["cpu_baseline"]["ns_step"] = steps
     if rank == 0:
         print(json.dumps(line), flush=True)
     h.close()
@@ -549,10 +664,13 @@ def main():
     ap.add_argument("--cpu-rows", type=int, default=65536)
     ap.add_argument("--cpu-passes", type=int, default=3)
     ap.add_argument("--quick", action="store_true", help="skip the walk / full-run extras")
-    ap.add_argument("--full-extras", action="store_true", help="also run the config-4 nested-sampling run and the config-5 sweep")
+    ap.add_argument("--full-extras", action="store_true", help="also: relative binning, posterior, concurrent runs, slice kernel, sequential limit, PP tests")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--pp-injections", type=int, default=100, help="injections of the PP leg of --full-extras")
+    ap.add_argument("--sweep-budget-s", type=float, default=90.0, help="time cap of the config-5 sweep (points past it are listed as skipped)")
     args = ap.parse_args()
+    if resolve_world(args, os.environ) == "spawn":       # `bench.py --gpus N` by itself: start the N ranks
+        os.execvp(sys.executable, spawn_command(args.gpus, sys.argv[1:]))
     if args.impl == "reference":
         run_reference(args)
     else:

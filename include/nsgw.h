@@ -197,6 +197,29 @@ int ns_posterior(ns_handle* h, const double* dead_dev, int64_t n_dead, double* t
 int ns_posterior_resample(ns_handle* h, const double* logp_dev, const double* theta_dev, int64_t N, int64_t n_out, uint64_t seed,
                           double* cum_dev, int64_t* idx_dev, double* theta_out_dev, void* stream);
 
+/* Checkpoint / resume (the paper stores the dead points).  The sampler's whole state is the live set, the
+ * evidence accumulators, the real-valued walk length, the iteration counter and the seed: every random number is a function of
+ * (seed, iteration, walker slot, step), so a handle created from the same configuration and data and given this state continues
+ * bit-for-bit as the original would have.  ns_get_state copies the scalars to *state_host and the live set to live_u_dev
+ * [n_live, ndim] / live_logl_dev [n_live] (device; either may be NULL); ns_set_state installs them (all three required).  Both
+ * synchronise.  Errors: -1 bad arguments / state, -3 no live set. */
+typedef struct {
+  int32_t struct_version;              /* NSGW_STRUCT_VERSION */
+  int32_t pad0;
+  int64_t iteration;                   /* steps done so far */
+  int64_t n_eval_total;
+  double logx, logz, h;                /* accumulators over the dead points */
+  double walks;                        /* real-valued walk length (R:L13) */
+  uint64_t seed;
+} ns_state;
+int ns_get_state(ns_handle* h, ns_state* state_host, double* live_u_dev, double* live_logl_dev, void* stream);
+int ns_set_state(ns_handle* h, const ns_state* state_host, const double* live_u_dev, const double* live_logl_dev, void* stream);
+
+/* Theoretical occupancy of the kernel that evaluates the likelihood of `rows` proposals in one round of the worklist walk
+ * (NSGW_OPT_WALK_KERNEL): resident warps per SM as a fraction of 64 (occupancy API x the share of the SMs' CTA slots the launch
+ * fills) in *warps_active_host, CTAs per SM in *ctas_per_sm_host (either may be NULL).  For the config-5 sweep's report. */
+int nsgw_sweep_occupancy(ns_handle* h, int64_t rows, double* warps_active_host, int32_t* ctas_per_sm_host);
+
 /* Device FP64 FMA throughput probe used for the roofline denominator: runs `iters` dependent-chain DFMAs x 8 chains per
  * thread on a full grid and returns achieved TFLOP/s in *tflops_host (synchronises; timed with CUDA events). */
 int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream);
@@ -239,8 +262,9 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * rounds: every walker proposes a chunk of steps, the likelihood of all the batch's in-bounds proposals is evaluated in one launch
  * of the CTA-per-row kernel, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows
  * the device two rounds behind, so these calls synchronise with the stream while they run; 3 = as 2 with the lane-per-row kernel
- * (k_pd_lp; PhenomD-form, otherwise 2).  Decisions, counters, traces and end points are identical for 1, 2 and every chunk length;
- * 3 sums a row's bins in another (fixed) order. */
+ * for PhenomD-form (k_pd_lp; measured slower at the row counts of a round).  TaylorF2 rows go through the lane-per-row kernel
+ * (k_bins_lp) under 0 and 3.  Decisions, counters, traces and end points are identical for 1, 2 and every chunk length; the
+ * lane-per-row kernels sum a row's bins in another (fixed) order. */
 #define NSGW_OPT_WALK_KERNEL 6
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 

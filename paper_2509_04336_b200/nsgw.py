@@ -42,9 +42,15 @@ class NsStats(C.Structure):
         return {k: getattr(self, k) for k, _ in self._fields_ if k != "pad0"}
 
 
+class NsState(C.Structure):
+    _fields_ = [("struct_version", C.c_int32), ("pad0", C.c_int32), ("iteration", C.c_int64), ("n_eval_total", C.c_int64),
+                ("logx", C.c_double), ("logz", C.c_double), ("h", C.c_double), ("walks", C.c_double), ("seed", C.c_uint64)]
+
+
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
            "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence", "ns_posterior", "ns_posterior_resample",
-           "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option"]
+           "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option",
+           "ns_get_state", "ns_set_state", "nsgw_sweep_occupancy"]
 
 # nsgw_set_option keys (include/nsgw.h)
 OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS, OPT_WALK_STAGE, OPT_WALK_KERNEL = 0, 1, 2, 3, 4, 5, 6
@@ -247,6 +253,22 @@ class Handle:
         l = torch.empty(self.n_live, dtype=torch.float64, device="cuda")
         self._check(lib().ns_get_live(self._h, _ptr(u), _ptr(l), _stream()), "ns_get_live")
         return u, l
+
+    def get_state(self):
+        """ns_get_state: (NsState, live_u, live_logl) -- everything a resumed run needs."""
+        st = NsState()
+        u = torch.empty(self.n_live, self.ndim, dtype=torch.float64, device="cuda")
+        l = torch.empty(self.n_live, dtype=torch.float64, device="cuda")
+        self._check(lib().ns_get_state(self._h, C.byref(st), _ptr(u), _ptr(l), _stream()), "ns_get_state")
+        return st, u, l
+
+    def set_state(self, st, live_u, live_logl):
+        self._check(lib().ns_set_state(self._h, C.byref(st), _ptr(live_u), _ptr(live_logl), _stream()), "ns_set_state")
+
+    def sweep_occupancy(self, rows):
+        f, c = C.c_double(), C.c_int32()
+        self._check(lib().nsgw_sweep_occupancy(self._h, C.c_int64(rows), C.byref(f), C.byref(c)), "nsgw_sweep_occupancy")
+        return f.value, c.value
 
     def profile_enable(self, on=True):
         self._check(lib().nsgw_profile_enable(self._h, C.c_int32(1 if on else 0)), "nsgw_profile_enable")

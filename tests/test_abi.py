@@ -33,10 +33,13 @@ def test_product_does_not_import_oracle():
         for f in files:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert not imp.search(open(os.path.join(dirpath, f)).read()), f
-    back = re.compile(r"^\s*(from|import)\s+paper_2509_04336_b200|#include\s+\S*nsgw", re.M)
+    # the oracle side may use the seeded INPUT generators (workloads.py holds none of the method's arithmetic) and nothing else
+    back = re.compile(r"^\s*(from|import)\s+paper_2509_04336_b200(?!\s+import\s+workloads\b)|#include\s+\S*nsgw", re.M)
     for f in os.listdir(os.path.join(ROOT, "oracle")):
         if f.endswith((".py", ".cpp")):
             assert not back.search(open(os.path.join(ROOT, "oracle", f)).read()), f
+    wl = open(os.path.join(pkg, "workloads.py")).read()
+    assert not re.search(r"^\s*(from|import)\s+(\.|paper_2509_04336_b200|torch|ctypes)", wl, re.M)   # inputs only: no binding, no library
 
 
 def test_no_cpu_fallback():

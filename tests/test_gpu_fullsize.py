@@ -129,3 +129,29 @@ def test_config3_same_seed_first_iterations_match_stored_trajectory(nsgw):
         assert abs(st["logz"] - tr["logz"][it]) < 1e-7 and abs(st["logl_star"] - tr["logl_star"][it]) < 1e-8
         n_match += 1
     assert n_match >= 3, n_match
+
+
+def test_checkpoint_resume_is_bit_exact(nsgw):
+    """ns_get_state / ns_set_state: a fresh handle given the saved state continues exactly as the original (every random number is
+    a function of seed, iteration, slot and step)."""
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 128.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 10.0, wf)
+    smp = dict(n_live=120, n_delete=60, naccept=8, maxmcmc=80, walks0=12.0, delay=-1.0)
+    for sp, sm in ((spec, smp), (W.config1()[0], W.config1()[1])):
+        a = nsgw.Handle(sp, sm, seed=11)
+        for _ in range(4):
+            a.step(want_stats=False)
+        st, u, l = a.get_state()
+        assert st.iteration == 4 and st.seed == 11
+        ref = [a.step() for _ in range(4)]
+        ua, la = a.get_live()
+        b = nsgw.Handle(sp, sm, seed=999)                 # different seed and live set: all of it is replaced
+        b.set_state(st, u, l)
+        got = [b.step() for _ in range(4)]
+        assert got == ref
+        ub, lb = b.get_live()
+        assert torch.equal(ua, ub) and torch.equal(la, lb)
+        assert a.finalize_evidence() == b.finalize_evidence()
+    bad = nsgw.NsState()
+    with pytest.raises(nsgw.NsgwError):
+        b.set_state(bad, u, l)

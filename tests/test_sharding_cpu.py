@@ -6,6 +6,7 @@ import subprocess
 import sys
 
 import numpy as np
+import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -66,3 +67,25 @@ def test_uniform_rows_are_index_keyed():
     b = W.uniform_rows(40, 60, 11, seed=3)
     assert np.array_equal(a[40:60], b) and a.min() > 0.0 and a.max() < 1.0
     assert not np.array_equal(W.uniform_rows(0, 10, 11, seed=4), a[:10])
+
+
+def test_bench_gpus_flag_dispatch():
+    """`bench.py --gpus N`: without a launcher and N > 1 it starts N ranks itself (torch.distributed.run, one per GPU); under a
+    launcher the flag must agree with WORLD_SIZE; both arms read the flag the same way; the traffic figure comes from profiles/."""
+    import argparse
+    import sys
+    sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
+    import bench
+    ns = argparse.Namespace
+    assert bench.resolve_world(ns(gpus=1), {}) == "run"
+    assert bench.resolve_world(ns(gpus=4), {}) == "spawn"
+    assert bench.resolve_world(ns(gpus=4), {"WORLD_SIZE": "4"}) == "run"
+    with pytest.raises(SystemExit):
+        bench.resolve_world(ns(gpus=8), {"WORLD_SIZE": "2"})
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "7", "--impl", "reference"], port=29999)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"] and "--nproc-per-node=4" in cmd
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29999"
+    assert cmd[-6:] == ["--gpus", "4", "--steps", "7", "--impl", "reference"] and cmd[-7].endswith("bench.py")
+    tr, f = bench.traffic_from_profile("k_bins_lp")
+    assert f and f.startswith("profiles/") and 1e6 < tr < 1e9
+    assert bench._profile_key("r02b_x") > bench._profile_key("r01ai_x") > bench._profile_key("r01z_x")
