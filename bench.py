@@ -340,6 +340,28 @@ def run_ours(args):
                                     "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
                                     "evals_per_s": st["n_eval_total"] / wall}
         h3.close()
+        # PhenomD-form batched likelihood on the config-3 data (the model of configs 3-5), B = 65536 prior rows: both sweep kernels
+        hp = nsgw.Handle(spec3)
+        th3 = hp.prior_transform_batch(u)
+        o3 = torch.empty(B, dtype=torch.float64, device="cuda")
+        pd = {}
+        for name, kern in (("k_bins_cta_per_row_pair", 1), ("k_pd_lp_lane_per_row", 2)):
+            hp.set_option(0, kern)
+            for _ in range(3):
+                hp.gw_loglike_batch(th3, out=o3)
+            evp = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+            for a, b in evp:
+                flush.zero_()
+                a.record(stream)
+                hp.gw_loglike_batch(th3, out=o3)
+                b.record(stream)
+            torch.cuda.synchronize()
+            pms = sum(a.elapsed_time(b) for a, b in evp) / len(evp)
+            pd[name] = {"ms_per_step": pms, "evals_per_s": B / (pms * 1e-3),
+                        "frac_fp64_peak": B * n_freq * alg_flops_per_bin(2, "phenomd") / (pms * 1e-3) / 1e12 / fp64_burst}
+        pd["flops_per_particle_bin_model"] = alg_flops_per_bin(2, "phenomd")
+        extras["phenomd_batch_config3_B65536"] = pd
+        hp.close()
         # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
         spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
         h4 = nsgw.Handle(spec4, smp4, seed=1)

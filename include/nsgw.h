@@ -263,8 +263,9 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * of the CTA-per-row kernel, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows
  * the device two rounds behind, so these calls synchronise with the stream while they run; 3 = as 2 with the lane-per-row kernel
  * for PhenomD-form (k_pd_lp; measured slower at the row counts of a round).  TaylorF2 rows go through the lane-per-row kernel
- * (k_bins_lp) under 0 and 3.  Decisions, counters, traces and end points are identical for 1, 2 and every chunk length; the
- * lane-per-row kernels sum a row's bins in another (fixed) order. */
+ * (k_bins_lp) under 0 and 3.  For a given value, decisions, counters, traces and end points are identical for every chunk length and
+ * batch composition; between values the kernels sum a row's bins in different fixed orders, so logL agrees to rounding (1e-12)
+ * and a decision can differ only where logL is that close to logL*. */
 #define NSGW_OPT_WALK_KERNEL 6
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 

@@ -36,6 +36,7 @@ struct WlState {
   int* sum_need;          // [3] by round mod 3: rows the batch still needs (sum over walkers of remaining steps x in-bounds fraction)
   int e_cap;              // rows per walker and round (<= kWlEMax)
   int r_target;           // rows per round the chunk lengths aim for
+  int cap_rows;           // rows the row buffers hold (B x e_cap)
 };
 
 template <int MODEL>
@@ -161,6 +162,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
     // rows for the in-bounds proposals from the batch-wide counter (placement is arbitrary: a row's logL does not depend on it)
     if (lane == 0 && nslots > 0) rowbase = atomicAdd(&st.n_rows[par], nslots);
     rowbase = __shfl_sync(0xffffffffu, rowbase, 0);
+    if (rowbase + nslots > st.cap_rows) __trap();   // cannot happen (every walker asks for <= e_cap rows): a bounds check that stays on
     // prior transform and waveform set-up, one row per lane
     for (int sl = lane; sl < nslots; sl += 32) {
       double* ru = st.row_u[par] + (size_t)(rowbase + sl) * kMaxDim;

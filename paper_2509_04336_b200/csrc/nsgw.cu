@@ -467,7 +467,7 @@ int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev
 template <int MODEL, int NDET>
 int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const long long B = a.B;
-  // rows per walker and round: up to 32 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
+  // rows per walker and round: up to 64 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
   const int e_cap = (int)std::max<long long>(1, std::min<long long>(kWlEMax, 65536 / B));
   const long long R = B * e_cap;
   int rc = ensure_wl(h, B, R);
@@ -475,6 +475,7 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   if (h->wl_kr == 0) h->wl_kr = 128;   // short ranges: the rows of a round vary, many small tasks keep the persistent grid balanced
   WlState st = h->wl;
   st.e_cap = e_cap;
+  st.cap_rows = (int)R;
   st.r_target = (int)std::min<long long>(R, std::max<long long>(16384, 24 * B));
   CU_CHECK(h, cudaMemsetAsync(st.n_rows, 0, sizeof(int) * 8, s));
   const unsigned gh = (unsigned)((B + kWlWarps - 1) / kWlWarps);

@@ -155,3 +155,48 @@ def test_checkpoint_resume_is_bit_exact(nsgw):
     bad = nsgw.NsState()
     with pytest.raises(nsgw.NsgwError):
         b.set_state(bad, u, l)
+
+
+@pytest.mark.parametrize("B", [130, 700])
+def test_walk_kernels_agree(nsgw, B):
+    """NSGW_OPT_WALK_KERNEL: 1 = one CTA per walker (k_walk_gw; 128 threads at B = 130, 96 at B = 700, also with the staged table
+    loads of NSGW_OPT_WALK_STAGE), 2 = batch-wide rounds swept by k_bins, 3 = swept by k_pd_lp.  The kernels sum a row's bins in
+    different fixed orders, so logL agrees to rounding and the decisions agree except at a logL within 1e-8 of L*."""
+    spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1"], 4.0, 256.0, (20.0, 40.0))
+    spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
+    h = nsgw.Handle(spec)
+    rng = np.random.default_rng(31)
+    m, Wlen = 220, 25
+    u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
+    donors = u_inj[None, :] + rng.normal(0, 1, (m, 11)) * np.array(W.C5_SIGMA) * 0.5
+    per = np.array(spec["periodic"], bool)
+    donors[:, per] -= np.floor(donors[:, per])
+    donors[:, ~per] = np.clip(donors[:, ~per], 1e-6, 1 - 1e-6)
+    ld = h.loglike_u_batch(dev(donors)).cpu().numpy()
+    lstar = float(np.quantile(ld, 0.3))
+    start = rng.integers(0, m, B)
+    out = {}
+    for name, wk, stage in (("cta", 1, 0), ("cta_staged", 1, 1), ("rounds", 2, 0), ("rounds_lane", 3, 0)):
+        h.set_option(6, wk)
+        h.set_option(5, stage)
+        ug, lg = dev(donors[start]), dev(ld[start])
+        res = h.walk_batch(dev(donors), ug, lg, lstar, Wlen, 4711, (5 << 24) | 9, slot0=0, trace=True)
+        tl = res["trace_logl"].cpu().numpy()
+        out[name] = (res["flags"].cpu().numpy(), tl, ug.cpu().numpy(), res["n_accept"].cpu().numpy())
+    assert np.array_equal(out["cta"][0], out["cta_staged"][0]) and np.array_equal(out["cta"][2], out["cta_staged"][2])   # staging: same arithmetic
+    ref = out["rounds"]
+    assert ref[3].sum() > B and (ref[0] & 1).any()
+    for name in ("cta", "rounds_lane"):
+        fl, tl, uu, na = out[name]
+        bad_rows = 0
+        for r in range(B):
+            diff = np.nonzero(fl[r] != ref[0][r])[0]
+            if diff.size:
+                t = diff[0]
+                assert (fl[r, t] & 4) and (ref[0][r, t] & 4) and abs(tl[r, t] - lstar) < 1e-8, (name, r, t, tl[r, t], lstar)
+                bad_rows += 1
+                continue
+            ev = (fl[r] & 4) != 0
+            assert np.max(np.abs(tl[r][ev] - ref[1][r][ev]), initial=0.0) < 1e-9
+            np.testing.assert_allclose(uu[r], ref[2][r], rtol=0, atol=1e-13)
+        assert bad_rows <= 2
