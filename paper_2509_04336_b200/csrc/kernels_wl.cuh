@@ -15,7 +15,7 @@
 // with, and the speculative steps after an acceptance are redone from the accepted point with the same Philox counters.
 #pragma once
 
-constexpr int kWlWarps = 2;          // walkers per CTA of k_wl_head
+constexpr int kWlWarps = 2;          // warps of a walker's CTA in k_wl_head: warp 0 resolves and proposes, both set the rows up
 constexpr int kWlEMax = 64;          // rows per walker and round (cap)
 
 struct WlState {
@@ -41,16 +41,17 @@ struct WlState {
 
 template <int MODEL>
 __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restrict__ cfgp, WalkArgs a, WlState st, int round) {
-  __shared__ double s_stage[kWlWarps][32][kMaxDim];
-  __shared__ double s_prop[kWlWarps][kWlEMax][kMaxDim];
-  __shared__ double s_cur[kWlWarps][kMaxDim];
+  __shared__ double s_stage[32][kMaxDim];
+  __shared__ double s_prop[kWlEMax][kMaxDim];
+  __shared__ double s_cur[kMaxDim];
+  __shared__ int s_nslots, s_rowbase;
   const DevCfg& cfg = *cfgp;
   const int D = cfg.ndim;
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
-  const long long row = blockIdx.x * (long long)kWlWarps + wrp;
+  const long long row = blockIdx.x;
   const int par = round & 1;
   if (blockIdx.x == 0 && threadIdx.x == 0) { st.n_rows[par ^ 1] = 0; st.n_active[par ^ 1] = 0; st.sum_need[(round + 1) % 3] = 0; }
-  if (row >= a.B) return;
+  if (wrp == 0) {
   const int W = a.W_dev ? *a.W_dev : a.W;
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;
   const uint32_t sid = a.stream_id | (a.iter_dev ? (uint32_t)(*a.iter_dev & 0xFFFFFF) : 0u);
@@ -120,7 +121,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
   }
   __syncwarp();
   // ---- propose the next chunk from the current point -----------------------------------------------------------------------
-  if (lane < D) s_cur[wrp][lane] = a.u[row * D + lane];
+  if (lane < D) s_cur[lane] = a.u[row * D + lane];
   __syncwarp();
   int nslots = 0, nsteps = 0;
   int rowbase = 0;
@@ -141,7 +142,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
     while (nslots < emax && nsteps < kWalkSteps && t0 + nsteps < W) {
       const int j = nsteps + lane;
       const bool live = j < kWalkSteps && t0 + j < W;
-      const bool inb = live && de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur[wrp], s_stage[wrp][lane]);
+      const bool inb = live && de_propose(cfg, a, sid, (uint32_t)(t0 + j), (uint32_t)(a.slot0 + row), s_cur, s_stage[lane]);
       const unsigned bal = __ballot_sync(0xffffffffu, inb);
       const int rank = __popc(bal & ((1u << lane) - 1u));
       const int room = emax - nslots, cnt = __popc(bal);
@@ -153,7 +154,7 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
       if (lane < consumed) {
         stp[j] = inb ? (unsigned char)(nslots + rank + 1) : 0;
         if (inb)
-          for (int d = 0; d < D; ++d) s_prop[wrp][nslots + rank][d] = s_stage[wrp][lane][d];
+          for (int d = 0; d < D; ++d) s_prop[nslots + rank][d] = s_stage[lane][d];
       }
       nslots += min(cnt, room);
       nsteps += consumed;
@@ -163,22 +164,27 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
     if (lane == 0 && nslots > 0) rowbase = atomicAdd(&st.n_rows[par], nslots);
     rowbase = __shfl_sync(0xffffffffu, rowbase, 0);
     if (rowbase + nslots > st.cap_rows) __trap();   // cannot happen (every walker asks for <= e_cap rows): a bounds check that stays on
-    // prior transform and waveform set-up, one row per lane
-    for (int sl = lane; sl < nslots; sl += 32) {
-      double* ru = st.row_u[par] + (size_t)(rowbase + sl) * kMaxDim;
-      double th[11];
-#pragma unroll
-      for (int d = 0; d < 11; ++d) {
-        const double x = s_prop[wrp][sl][d];
-        ru[d] = x;
-        th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], x);
-      }
-      setup_particle<MODEL>(cfg, th, st.row_cb[par] + (size_t)(rowbase + sl) * CB_SIZE);
-    }
     if (lane == 0) atomicAdd(&st.n_active[par], 1);
   }
   if (lane == 0) {
     st.t0[row] = t0; st.E[row] = E; st.nsteps[row] = nsteps; st.nslots[row] = nslots; st.rowbase[row] = rowbase;
+    s_nslots = nslots; s_rowbase = rowbase;
+  }
+  }   // warp 0
+  __syncthreads();
+  // prior transform and waveform set-up of the chunk's rows, one row per thread of the CTA (the serial set-up chain is the latency
+  // of this kernel: 64 lanes take a 64-row chunk in one pass)
+  const int nslots_all = s_nslots, rowbase_all = s_rowbase;
+  for (int sl = threadIdx.x; sl < nslots_all; sl += 32 * kWlWarps) {
+    double* ru = st.row_u[par] + (size_t)(rowbase_all + sl) * kMaxDim;
+    double th[11];
+#pragma unroll
+    for (int d = 0; d < 11; ++d) {
+      const double x = s_prop[sl][d];
+      ru[d] = x;
+      th[d] = prior_transform_dim(cfg.prior_kind[d], cfg.prior_lo[d], cfg.prior_hi[d], x);
+    }
+    setup_particle<MODEL>(cfg, th, st.row_cb[par] + (size_t)(rowbase_all + sl) * CB_SIZE);
   }
 }
 

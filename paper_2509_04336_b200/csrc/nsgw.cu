@@ -478,7 +478,7 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   st.cap_rows = (int)R;
   st.r_target = (int)std::min<long long>(R, std::max<long long>(16384, 24 * B));
   CU_CHECK(h, cudaMemsetAsync(st.n_rows, 0, sizeof(int) * 8, s));
-  const unsigned gh = (unsigned)((B + kWlWarps - 1) / kWlWarps);
+  const unsigned gh = (unsigned)B;   // one CTA (kWlWarps warps) per walker
   for (long long r = 0;; ++r) {
     const int par = (int)(r & 1);
     k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, (int)std::min<long long>(r, 6 + r % 6));   // first round or not, parity and round mod 3 matter
