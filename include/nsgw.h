@@ -232,8 +232,8 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
 
 /* Tuning / test options of a handle.  key NSGW_OPT_BINS_KERNEL selects the kernel behind gw_loglike_batch (and the initial
  * live-set evaluation): 0 = automatic (by model and batch size), 1 = CTA per particle (pair), bins strided over threads
- * (k_bins; both models), 2 = lane per particle, bin tiles staged in shared memory (k_bins_lp; TaylorF2 only -- for
- * PhenomD-form the value 2 falls back to 1).  Both compute the same sums in a different, fixed order.
+ * (k_bins; both models), 2 = lane per particle, bin tiles staged in shared memory (k_bins_lp for TaylorF2, k_pd_lp for
+ * PhenomD-form).  Both compute the same sums in a different, fixed order.
  * Returns -1 for an unknown key or value. */
 #define NSGW_OPT_BINS_KERNEL 0
 /* key NSGW_OPT_WALK_SPEC: speculative chunk size of the GW walk kernel.  k_walk_gw proposes consecutive steps of a walker from
@@ -258,14 +258,13 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * 0 (default) = plain loads.  A tuning switch. */
 #define NSGW_OPT_WALK_STAGE 5
 /* key NSGW_OPT_WALK_KERNEL: how ns_step / ns_run / ns_walk_batch run the acceptance walk on a GW likelihood.  0 = automatic
- * (2 for the exact likelihood, 1 for relative binning); 1 = one CTA per walker, all steps in one launch (k_walk_gw); 2 = batch-wide
- * rounds: every walker proposes a chunk of steps, the likelihood of all the batch's in-bounds proposals is evaluated in one launch
- * of the CTA-per-row kernel, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows
- * the device two rounds behind, so these calls synchronise with the stream while they run; 3 = as 2 with the lane-per-row kernel
- * for PhenomD-form (k_pd_lp; measured slower at the row counts of a round).  TaylorF2 rows go through the lane-per-row kernel
- * (k_bins_lp) under 0 and 3.  For a given value, decisions, counters, traces and end points are identical for every chunk length and
- * batch composition; between values the kernels sum a row's bins in different fixed orders, so logL agrees to rounding (1e-12)
- * and a decision can differ only where logL is that close to logL*. */
+ * (3 for the exact likelihood, 1 for relative binning); 1 = one CTA per walker, all steps in one launch (k_walk_gw); 2 and 3 =
+ * batch-wide rounds: every walker proposes a chunk of steps, the likelihood of all the batch's in-bounds proposals is evaluated in one
+ * launch, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows the device two rounds
+ * behind, so these calls synchronise with the stream while they run.  2 sweeps the rows with the CTA-per-row-pair kernel (k_bins),
+ * 3 with the lane-per-row kernels (k_pd_lp for PhenomD-form, k_bins_lp for TaylorF2).  For a given value, decisions, counters,
+ * traces and end points are identical for every chunk length and batch composition; between values the kernels sum a row's bins
+ * in different fixed orders, so logL agrees to rounding (1e-12) and a decision can differ only where logL is that close to logL*. */
 #define NSGW_OPT_WALK_KERNEL 6
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 

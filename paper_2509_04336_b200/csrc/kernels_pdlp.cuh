@@ -1,40 +1,46 @@
-// kernels_pdlp.cuh -- K1 for PhenomD-form at large batches and for the worklist walk: k_pd_lp (lane per particle over the
-// merger-ringdown bins + warp per particle over the low-frequency bins) and k_finish_rows.
+// kernels_pdlp.cuh -- K1 for PhenomD-form, lane = row: k_pd_lp (used for the rows of the worklist walk and for large batches) and
+// k_finish_rows (the finishing pass of the TaylorF2 rows of the worklist walk).
 // Part of libnsgw (one translation unit): included by nsgw.cu inside its anonymous namespace, after kernels_k1.cuh.
 //
-// Why two mappings in one kernel.  About 80 % of a particle's bins (all above max(f_RD/2, f_peak), CB_FMR) use
-// ONE formula -- phase = a + b f + c/f + d f^3/4 + e atan((f - f0)/fd), amplitude = Lorentzian x exponential -- and differ between
-// particles only in the coefficients: that part runs lane = particle, coefficients in registers, the bins' table values broadcast
-// from a shared-memory tile, no cross-lane reduction, no per-bin global traffic (the design that took TaylorF2 to 0.64 of the FP64
-// peak).  Where that region starts depends on the particle (total mass, final spin), so the lanes of a warp disagree on the formula
-// for the lowest 10-30 % of bins: those bins run warp = particle, lanes strided over bins, where the three phase and three amplitude
-// regions are contiguous in the bin index and the branches are uniform but for one lane at each boundary.
+// Design.  About 80 % of a row's bins (all above max(f_RD/2, f_peak), CB_FMR) use ONE formula -- phase =
+// a + b f + c/f + d f^3/4 + e atan((f - f0)/fd), amplitude = Lorentzian x exponential -- and differ between rows only in the
+// coefficients: lane = row, coefficients in registers, the bins' table values broadcast from a shared-memory tile, no cross-lane
+// reduction, no per-bin global traffic (the design that took TaylorF2 to 0.63 of the FP64 peak).  Consecutive bins of a lane let the
+// expensive functions be CARRIED: atan by atan y' = atan y - atan((y - y') / (1 + y y')), the exponential as a geometric sequence, the
+// detector phasors by Horner's rule -- 56 FP64 instructions per particle-bin against 77 in the bins-strided-over-threads k_bins.
+// Where the merger-ringdown region starts depends on the row (total mass, final spin), so below the highest start of a warp's rows
+// the lanes disagree on the formula: those tiles evaluate the candidate formulas of the regions present and select per lane by the row's
+// own boundaries, with the extra coefficients read from a shared-memory block staged per task (conflict-free: consecutive lanes,
+// consecutive words).  Three tile classes, chosen per warp and tile: all merger-ringdown (registers only); intermediate or
+// merger-ringdown (f >= 0.018/M for every row: + 13 coefficients); any region (+ 25 more and six more table values per bin).
 //
-// Two launches: k_pd_low (warp per row, many resident warps: that part is latency-bound) and k_pd_lp (nranges x ngroups tasks: group of
-// NT x PP rows, range of `kr` bins on the fixed tile grid, persistent CTAs).  Every task writes its rows' partial sums to
-// partial[slot][N][stride] (slot = range index, or nranges for the low part); k_finish_rows adds the slots in order.  A row's sums do not depend on which other rows share
-// its warp, its task or the launch (masked bins contribute exact zeros; tiles sit on a grid fixed by `kr`), so the likelihood of a
-// proposal is the same number whatever batch it is evaluated in -- the walk's chunking stays invisible.
+// Task = (group of NT x PP rows, range of `kr` bins on the fixed tile grid), persistent CTAs over the task list.  A task writes its rows'
+// partial sums to partial[range][N][stride]; the CTA that finishes a group's LAST range (a ticket per group) adds the ranges in range
+// order and writes logL -- no finishing launch, and the order of the sum does not depend on which CTA came last.  A row's sums do not
+// depend on the rows it shares a warp, a task or a launch with, so the likelihood of a proposal is the same number whatever batch it is
+// evaluated in: the walk's chunking stays invisible.
 #pragma once
 
 #ifndef NSGW_PD_PP
-#define NSGW_PD_PP 2
+#define NSGW_PD_PP 1
 #define NSGW_PD_OCC 3
-#define NSGW_PD_UNR 2
+#define NSGW_PD_UNR 4
 #endif
-constexpr int kPdNT = 128;            // threads per CTA of the lane kernel
+#ifndef NSGW_PD_KT
+#define NSGW_PD_KT 128
+#endif
+constexpr int kPdNT = 128;            // threads per CTA
 constexpr int kPdPP = NSGW_PD_PP;     // rows per thread
-constexpr int kPdKT = 64;             // bins per shared-memory tile
+constexpr int kPdKT = NSGW_PD_KT;     // bins per shared-memory tile
 constexpr int kPdOCC = NSGW_PD_OCC;   // CTAs per SM
 constexpr int kPdUNR = NSGW_PD_UNR;   // bins per unrolled loop body
-constexpr int kPdLowNT = 256;         // threads per CTA of the low kernel (warp = row)
-constexpr int kPdLowOCC = 3;
 
 template <int NDET>
 struct PdTile {
   double f[kPdKT], f34[kPdKT], y3[kPdKT], lnf[kPdKT];
   double2 wd[NDET][kPdKT];
   double ws[NDET][kPdKT];
+  double y5[kPdKT], y2[kPdKT], y1[kPdKT], x1[kPdKT], xl[kPdKT], x2[kPdKT];   // class-2 tiles only: f^-5/3, f^-2/3, f^-1/3, f^1/3, f^1/3 ln f, f^2/3
 };
 
 // Rows to evaluate: `n_rows_dev` (device, optional) overrides n_rows -- the worklist walk sizes its rounds on the device.
@@ -45,125 +51,38 @@ struct PdArgs {
   long long stride;           // row stride of `partial` (>= rows)
   int kr;                     // bins per range (multiple of kPdKT)
   int nranges;
-  double* partial;            // [nranges + 1][N][stride]
+  double* partial;            // [nranges][N][stride]
+  int* ticket;                // [groups] zero on entry, zero again on exit: ranges of the group finished so far
+  double* logl;               // [rows]
+  double* parts;              // optional [rows][2 NDET]
 };
 
-// Odd Taylor coefficients of atan beyond the linear term: -1/3, 1/5, -1/7, 1/9.
-__constant__ double kAtanR[4] = {-1.0 / 3.0, 0.2, -1.0 / 7.0, 1.0 / 9.0};
+// Odd Taylor coefficients of atan beyond the linear term: -1/3, 1/5, -1/7.
+__constant__ double kAtanR[3] = {-1.0 / 3.0, 0.2, -1.0 / 7.0};
 
-// ---------------------------------------------------------------------------------------------------------------------
-// low kernel: warp = row, lanes strided over the bins below the row's merger-ringdown start (general piecewise evaluation;
-// the regions are contiguous in the bin index, so a warp diverges at one lane per boundary only).  Writes slot `nranges`.
-// ---------------------------------------------------------------------------------------------------------------------
-template <int NDET>
-__global__ void __launch_bounds__(kPdLowNT, kPdLowOCC) k_pd_low(const DevCfg* __restrict__ cfgp, Tables tb, PdArgs a) {
-  using AL = AccLayout<2, NDET>;
-  constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1, NWARP = kPdLowNT / 32;
-  __shared__ MathTables mtab;
-  const DevCfg& cfg = *cfgp;
-  const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
-  const int nf = cfg.n_freq;
-  const double f_min = cfg.f_min, df = cfg.df;
-  const long long B = a.n_rows_dev ? (long long)*a.n_rows_dev : a.n_rows;
-  if ((long long)blockIdx.x * NWARP >= B) return;
-  load_math_tables(&mtab, tb.mt, tid, kPdLowNT);
-  __syncthreads();
-  for (long long p = (long long)blockIdx.x * NWARP + wrp; p < B; p += (long long)gridDim.x * NWARP) {
-    const double* cb = a.cbs + p * CB_SIZE;
-    const bool valid = __ldg(cb + CB_VALID) != 0.0;
-    const int kmr = valid ? mr_first_bin(__ldg(cb + CB_FP1), f_min, df, nf) : 0;   // the lane kernel takes over from here
-    double acc[AL::N];
-#pragma unroll
-    for (int j = 0; j < AL::N; ++j) acc[j] = 0.0;
-    if (kmr > 0) {
-      const CbPtr cbp{cb};
-      // detector phasors R_d(f_k) = C_d exp(i dtq_d f_k) at this lane's first bin, advanced by 32 bins per iteration
-      double2 R[ND1s], St[ND1s];
-#pragma unroll
-      for (int d = 0; d < ND1; ++d) {
-        const double cr = __ldg(cb + CB_DET + 4 * (d + 1)), ci = __ldg(cb + CB_DET + 4 * (d + 1) + 1);
-        const double dtq = __ldg(cb + CB_DET + 4 * (d + 1) + 2);
-        double sn, cs;
-        sincos_qt(dtq * (f_min + df * lane), sn, cs);
-        R[d] = make_double2(cr * cs - ci * sn, cr * sn + ci * cs);
-        sincos_qt(dtq * (df * 32), sn, cs);
-        St[d] = make_double2(cs, sn);
-      }
-      const double c3 = __ldg(cb + CB_AM + 3), frd = __ldg(cb + CB_AM);
-      double ex = exp_tab(c3 * (f_min + df * lane - frd), &mtab);
-      const double exr = exp_tab(c3 * (df * 32), &mtab);
-      for (int k = lane; k < kmr; k += 32) {
-        const BinBasis b = make_basis(tb, k, true);
-        double2 w[NDET];
-        double wsv[NDET];
-#pragma unroll
-        for (int d = 0; d < NDET; ++d) { w[d] = __ldg(tb.wd[d] + k); wsv[d] = __ldg(tb.ws[d] + k); }
-        double q, amp;
-        phenom_bin_t(cbp, b, &mtab, ex, q, amp);
-        ex *= exr;
-        double sn, cs;
-        sincos_lut(64.0 * q, &mtab, sn, cs);
-        sn *= amp; cs *= amp;
-        acc[0] = fma(w[0].x, cs, acc[0]);
-        acc[1] = fma(-w[0].x, sn, acc[1]);
-        acc[0] = fma(-w[0].y, sn, acc[0]);
-        acc[1] = fma(-w[0].y, cs, acc[1]);
-        const double a2 = amp * amp;
-#pragma unroll
-        for (int d = 0; d < NDET; ++d) acc[AL::kHh + d] = fma(a2, wsv[d], acc[AL::kHh + d]);
-#pragma unroll
-        for (int d = 0; d < ND1; ++d) {
-          const double rx = R[d].x, ry = R[d].y;
-          const double gr = fma(cs, rx, sn * ry);
-          const double gi = fma(cs, ry, -(sn * rx));
-          acc[AL::kDh + d] = fma(w[d + 1].x, gr, acc[AL::kDh + d]);
-          acc[AL::kDh + d] = fma(w[d + 1].y, gi, acc[AL::kDh + d]);
-          R[d].x = fma(rx, St[d].x, -(ry * St[d].y));
-          R[d].y = fma(rx, St[d].y, ry * St[d].x);
-        }
-      }
-#pragma unroll
-      for (int j = 0; j < AL::N; ++j) {
-        double x = acc[j];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
-        acc[j] = x;
-      }
-    }
-    if (lane < AL::N) {
-      double v = 0.0;
-#pragma unroll
-      for (int j = 0; j < AL::N; ++j) v = (lane == j) ? acc[j] : v;
-      a.partial[((long long)a.nranges * AL::N + lane) * a.stride + p] = v;
-    }
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------------------------
-// lane kernel: lane = row (PP per thread) over the bins of a range from the row's intermediate-phase start (f >= 0.018/M, CB_FP1)
-// upwards.  Task = (group of NT x PP rows, range); writes slot `range`.  Tiles wholly inside every row's merger-ringdown region
-// (f >= CB_FMR, most of them) take the branch-free loop with that region's coefficients in registers; the tiles below evaluate,
-// per row and bin, both candidate phases (intermediate / merger-ringdown) and both candidate amplitudes (intermediate quartic /
-// Lorentzian) and select by the row's own boundaries, with the intermediate regions' coefficients read from a shared-memory
-// block staged per task (conflict-free: consecutive lanes, consecutive words).
-// ---------------------------------------------------------------------------------------------------------------------
-constexpr int kPdMix = 13;   // per row: 64 PB0..3 (phase, 1/256 turn), AH0..6 (quartic), FP2, FA2 [Hz]
+// Shared-memory coefficient block of a task, [kPdMixAll][NT PP] (row-minor).  Classes 1 and 2 read the first kPdMix1 entries per row:
+// 64 PB0..3 (intermediate phase, 1/256 turn), AH0..6 (intermediate amplitude), FP2, FA2 [Hz]; class 2 also 64 PH0..12 (inspiral phase),
+// AI0..9 (inspiral amplitude), FP1, FA1.
+constexpr int kPdMix1 = 13, kPdMixAll = 13 + 25;
+template <int PP>
+constexpr size_t pd_mix_bytes() { return sizeof(double) * kPdMixAll * kPdNT * PP; }
 
 template <int NDET, int PP>
 struct PdRow {
   static constexpr int ND1s = NDET > 1 ? NDET - 1 : 1;
   double pm[PP][5], yA[PP], yB[PP], am[PP][3], exd[PP];
   double2 St[PP][ND1s];
-  int klo[PP];
   double acc[PP][AccLayout<2, NDET>::N];
   // per tile
   double ex[PP], yp[PP], At[PP];
   double2 S[PP][ND1s];
 };
 
-template <int NDET, int PP, bool MIXED>
-__device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<NDET>& sm, const double* __restrict__ mix /*smem [kPdMix][NT PP]*/,
-                                             const MathTables* mt, int t_lo, int n, int tid) {
+// One tile, bins in descending order.  CLS 0: every row of the warp is in its merger-ringdown region; 1: intermediate or
+// merger-ringdown; 2: any region.
+template <int NDET, int PP, int CLS>
+__device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<NDET>& sm, const double* __restrict__ mix, const MathTables* mt,
+                                             int n, int tid) {
   using AL = AccLayout<2, NDET>;
   constexpr int ND1 = NDET - 1, NR = kPdNT * PP;
 #pragma unroll kPdUNR
@@ -173,8 +92,12 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
     double wsv[NDET];
 #pragma unroll
     for (int d = 0; d < NDET; ++d) { w[d] = sm.wd[d][kk]; wsv[d] = sm.ws[d][kk]; }
-    double L = 0.0, if3 = 0.0;
-    if (MIXED) { L = sm.lnf[kk]; if3 = y3 * y3 * y3; }
+    double L = 0.0, if3 = 0.0, y5 = 0.0, y2 = 0.0, y1 = 0.0, x1 = 0.0, xl = 0.0, x2 = 0.0, fx = 0.0, fx2 = 0.0, ff = 0.0;
+    if (CLS >= 1) { L = sm.lnf[kk]; if3 = y3 * y3 * y3; }
+    if (CLS == 2) {
+      y5 = sm.y5[kk]; y2 = sm.y2[kk]; y1 = sm.y1[kk]; x1 = sm.x1[kk]; xl = sm.xl[kk]; x2 = sm.x2[kk];
+      fx = f * x1; fx2 = fx * x1; ff = f * f;
+    }
 #pragma unroll
     for (int j = 0; j < PP; ++j) {
       // atan((f - f0)/fd) carried down from the bin above: atan(y') = atan(y) - atan((y - y') / (1 + y y'))
@@ -189,10 +112,10 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
       q = fma(r.pm[j][2], y3, q);
       q = fma(r.pm[j][3], f34, q);
       q = fma(r.pm[j][4], r.At[j], q);
-      const double fx = f - r.am[j][0];
-      double amp = rcp_nr1(fma(fx, fx, r.am[j][2])) * r.ex[j];       // ex carries the Lorentzian's numerator
+      const double fr = f - r.am[j][0];
+      double amp = rcp_nr1(fma(fr, fr, r.am[j][2])) * r.ex[j];       // ex carries the Lorentzian's numerator
       r.ex[j] *= r.exd[j];
-      if (MIXED) {
+      if (CLS >= 1) {
         const double* m = mix + j * kPdNT + tid;
         double qi = fma(m[1 * NR], L, m[0 * NR]);
         qi = fma(m[2 * NR], f, qi);
@@ -205,7 +128,26 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
         ph = fma(ph, xh, m[7 * NR]);
         ph = fma(ph, xh, m[6 * NR]);
         amp = (f < m[12 * NR]) ? ph : amp;
-        amp = (t_lo + kk >= r.klo[j]) ? amp : 0.0;      // bins below the row's intermediate-phase start belong to the low kernel
+        if (CLS == 2) {
+          const double* c = m + kPdMix1 * NR;       // PH0..12: y5 y3 y2 y 1 L x xL x2 f | fx fx2 ff
+          double qs = fma(c[0 * NR], y5, c[4 * NR]);
+          qs = fma(c[1 * NR], y3, qs);
+          qs = fma(c[2 * NR], y2, qs);
+          qs = fma(c[3 * NR], y1, qs);
+          qs = fma(c[5 * NR], L, qs);
+          qs = fma(c[6 * NR], x1, qs);
+          qs = fma(c[7 * NR], xl, qs);
+          qs = fma(c[8 * NR], x2, qs);
+          qs = fma(c[9 * NR], f, qs);
+          qs = fma(c[10 * NR], fx, qs);
+          qs = fma(c[11 * NR], fx2, qs);
+          qs = fma(c[12 * NR], ff, qs);
+          q = (f < c[23 * NR]) ? qs : q;
+          double pi_ = c[22 * NR];                  // AI9..AI0: degree-9 polynomial in x = f^1/3
+#pragma unroll
+          for (int i = 8; i >= 0; --i) pi_ = fma(pi_, x1, c[(13 + i) * NR]);
+          amp = (f < c[24 * NR]) ? pi_ : amp;
+        }
       }
       double sn, cs;
       sincos_lut<true>(q, mt, sn, cs);
@@ -233,18 +175,18 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
 template <int NDET>
 __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restrict__ cfgp, Tables tb, PdArgs a) {
   using AL = AccLayout<2, NDET>;
-  constexpr int NT = kPdNT, PP = kPdPP, KT = kPdKT, ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1, NWARP = NT / 32;
+  constexpr int NT = kPdNT, PP = kPdPP, KT = kPdKT, ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1, NWARP = NT / 32, NR = NT * PP;
   __shared__ __align__(16) PdTile<NDET> sm;
   __shared__ MathTables mtab;
-  __shared__ double mix[kPdMix * NT * PP];
-  __shared__ int s_kmin[NWARP], s_kmax[NWARP];
+  __shared__ int s_k1[NWARP], s_k2[NWARP], s_last;
+  extern __shared__ __align__(16) double mix[];          // [kPdMixAll][NR]
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const int nf = cfg.n_freq;
   const double f_min = cfg.f_min, df = cfg.df;
   const long long B = a.n_rows_dev ? (long long)*a.n_rows_dev : a.n_rows;
   if (B <= 0) return;
-  const long long ngroups = (B + NT * PP - 1) / (NT * PP);
+  const long long ngroups = (B + NR - 1) / NR;
   const long long ntasks = ngroups * a.nranges;
   if (blockIdx.x >= ntasks) return;
   load_math_tables(&mtab, tb.mt, tid, NT);
@@ -253,30 +195,31 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
     const long long grp = task / a.nranges;
     const int rng = (int)(task % a.nranges);
     const int k0 = rng * a.kr, k1 = min(nf, k0 + a.kr);
-    // per row: phase a + b f + c/f + d f^3/4 + e atan(yA f + yB) in 1/256 turn; amplitude g1 / ((f - f_RD)^2 + w^2) x ex(f)
+    // per row: phase a + b f + c/f + d f^3/4 + e atan(yA f + yB) in 1/256 turn; amplitude g1 / ((f - f_RD)^2 + w^2) x ex(f).
+    // An invalid row (unphysical theta: logL = -inf whatever the sums) gets zero coefficients, so nothing undefined is evaluated.
     PdRow<NDET, PP> r;
-    int kmr[PP];
-    int kmin = nf, kmax = 0;            // over this thread's rows: lowest bin any row wants, highest merger-ringdown start
+    double c3[PP], g1[PP];
+    int k1max = 0, k2max = 0;          // over this thread's rows: first bin past the inspiral phase region / in the merger-ringdown region
 #pragma unroll
     for (int j = 0; j < PP; ++j) {
       const long long p = (grp * PP + j) * NT + tid;
-      const bool have = p < B;
-      const double* cb = a.cbs + (have ? p : 0) * CB_SIZE;
-      const bool valid = have && __ldg(cb + CB_VALID) != 0.0;
-      r.klo[j] = valid ? mr_first_bin(__ldg(cb + CB_FP1), f_min, df, nf) : nf;   // nf: every bin masked
-      kmr[j] = valid ? mr_first_bin(__ldg(cb + CB_FMR), f_min, df, nf) : 0;
-      kmin = min(kmin, r.klo[j]);
-      kmax = max(kmax, kmr[j]);
+      const double* cb = a.cbs + (p < B ? p : 0) * CB_SIZE;
+      const bool valid = p < B && __ldg(cb + CB_VALID) != 0.0;
+      k1max = max(k1max, valid ? mr_first_bin(__ldg(cb + CB_FP1), f_min, df, nf) : 0);
+      k2max = max(k2max, valid ? mr_first_bin(__ldg(cb + CB_FMR), f_min, df, nf) : 0);
 #pragma unroll
-      for (int i = 0; i < 5; ++i) r.pm[j][i] = 64.0 * __ldg(cb + CB_PM + i);     // quarter turns -> 1/256 turn (exact)
-      r.yA[j] = __ldg(cb + CB_PM + 6);
-      r.yB[j] = -__ldg(cb + CB_PM + 5) * r.yA[j];
-      r.am[j][0] = __ldg(cb + CB_AM); r.am[j][1] = __ldg(cb + CB_AM + 1); r.am[j][2] = __ldg(cb + CB_AM + 2);
-      r.exd[j] = exp_tab(-__ldg(cb + CB_AM + 3) * df, &mtab);                     // ex(f - df) = ex(f) exd
+      for (int i = 0; i < 5; ++i) r.pm[j][i] = valid ? 64.0 * __ldg(cb + CB_PM + i) : 0.0;     // quarter turns -> 1/256 turn (exact)
+      r.yA[j] = valid ? __ldg(cb + CB_PM + 6) : 0.0;
+      r.yB[j] = valid ? -__ldg(cb + CB_PM + 5) * r.yA[j] : 0.0;
+      r.am[j][0] = valid ? __ldg(cb + CB_AM) : 0.0;
+      g1[j] = valid ? __ldg(cb + CB_AM + 1) : 0.0;
+      r.am[j][2] = valid ? __ldg(cb + CB_AM + 2) : 1.0;
+      c3[j] = valid ? __ldg(cb + CB_AM + 3) : 0.0;
+      r.exd[j] = exp_tab(-c3[j] * df, &mtab);                                                   // ex(f - df) = ex(f) exd
 #pragma unroll
       for (int d = 0; d < ND1; ++d) {
         double sn, cs;
-        sincos_qt(__ldg(cb + CB_DET + 4 * (d + 1) + 2) * df, sn, cs);
+        sincos_qt((valid ? __ldg(cb + CB_DET + 4 * (d + 1) + 2) : 0.0) * df, sn, cs);
         r.St[j][d] = make_double2(cs, sn);
       }
 #pragma unroll
@@ -284,68 +227,82 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-      kmin = min(kmin, __shfl_xor_sync(0xffffffffu, kmin, o));
-      kmax = max(kmax, __shfl_xor_sync(0xffffffffu, kmax, o));
+      k1max = max(k1max, __shfl_xor_sync(0xffffffffu, k1max, o));
+      k2max = max(k2max, __shfl_xor_sync(0xffffffffu, k2max, o));
     }
     __syncthreads();                       // previous task's readers of sm / mix / s_k* are done
-    if (lane == 0) { s_kmin[wrp] = kmin; s_kmax[wrp] = kmax; }
+    if (lane == 0) { s_k1[wrp] = k1max; s_k2[wrp] = k2max; }
     __syncthreads();
-    int kmin_cta = s_kmin[0], kmax_cta = s_kmax[0];
+    int k1cta = s_k1[0], k2cta = s_k2[0];
 #pragma unroll
-    for (int w = 1; w < NWARP; ++w) { kmin_cta = min(kmin_cta, s_kmin[w]); kmax_cta = max(kmax_cta, s_kmax[w]); }
-    if (k0 < kmax_cta) {                   // CTA-uniform: some tile of this range needs the intermediate regions' coefficients
+    for (int w = 1; w < NWARP; ++w) { k1cta = max(k1cta, s_k1[w]); k2cta = max(k2cta, s_k2[w]); }
+    if (k0 < k2cta) {                      // CTA-uniform: some tile of this range needs the other regions' coefficients
 #pragma unroll
       for (int j = 0; j < PP; ++j) {
         const long long p = (grp * PP + j) * NT + tid;
         const double* cb = a.cbs + (p < B ? p : 0) * CB_SIZE;
+        const bool valid = p < B && __ldg(cb + CB_VALID) != 0.0;
         double* m = mix + j * NT + tid;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) m[i * NT * PP] = 64.0 * __ldg(cb + CB_PB + i);
+        for (int i = 0; i < 4; ++i) m[i * NR] = valid ? 64.0 * __ldg(cb + CB_PB + i) : 0.0;
 #pragma unroll
-        for (int i = 0; i < 7; ++i) m[(4 + i) * NT * PP] = __ldg(cb + CB_AH + i);
-        m[11 * NT * PP] = __ldg(cb + CB_FP2);
-        m[12 * NT * PP] = __ldg(cb + CB_FA2);
+        for (int i = 0; i < 7; ++i) m[(4 + i) * NR] = valid ? __ldg(cb + CB_AH + i) : 0.0;
+        m[11 * NR] = valid ? __ldg(cb + CB_FP2) : 0.0;
+        m[12 * NR] = valid ? __ldg(cb + CB_FA2) : 0.0;
+        if (k0 < k1cta) {
+          double* c = m + kPdMix1 * NR;
+#pragma unroll
+          for (int i = 0; i < 13; ++i) c[i * NR] = valid ? 64.0 * __ldg(cb + CB_PH + i) : 0.0;
+#pragma unroll
+          for (int i = 0; i < 10; ++i) c[(13 + i) * NR] = valid ? __ldg(cb + CB_AI + i) : 0.0;
+          c[23 * NR] = valid ? __ldg(cb + CB_FP1) : 0.0;
+          c[24 * NR] = valid ? __ldg(cb + CB_FA1) : 0.0;
+        }
       }
     }
     for (int t_lo = k0; t_lo < k1; t_lo += KT) {
       const int n = min(KT, k1 - t_lo);
-      if (t_lo + n <= kmin_cta) continue;  // CTA-uniform: the whole tile lies below every row's start
       __syncthreads();
+      const bool need2 = t_lo < k1cta;     // CTA-uniform: some warp evaluates this tile with the inspiral formulas
       for (int i = tid; i < n; i += NT) {
         const int k = t_lo + i;
-        sm.f[i] = __ldg(tb.f + k); sm.f34[i] = __ldg(tb.f34 + k); sm.y3[i] = __ldg(tb.t01 + k).y; sm.lnf[i] = __ldg(tb.t45 + k).x;
+        const double2 t01 = __ldg(tb.t01 + k), t45 = __ldg(tb.t45 + k);
+        sm.f[i] = __ldg(tb.f + k); sm.f34[i] = __ldg(tb.f34 + k); sm.y3[i] = t01.y; sm.lnf[i] = t45.x;
 #pragma unroll
         for (int d = 0; d < NDET; ++d) { sm.wd[d][i] = __ldg(tb.wd[d] + k); sm.ws[d][i] = __ldg(tb.ws[d] + k); }
+        if (need2) {
+          const double2 t23 = __ldg(tb.t23 + k), t67 = __ldg(tb.t67 + k);
+          sm.y5[i] = t01.x; sm.y2[i] = t23.x; sm.y1[i] = t23.y; sm.x1[i] = t45.y; sm.xl[i] = t67.x; sm.x2[i] = t67.y;
+        }
       }
       __syncthreads();
-      if (t_lo + n <= kmin) continue;      // warp-uniform (no barrier below)
       // tile start (top bin, the loop runs downwards): ex by exp_tab, the atan term by atan_tab one bin ABOVE the top, from where
       // it is carried down; the steps have one sign, so a relative error of 2^-40 in the reciprocal is 2^-40 of the tile's total
       // change (<= pi); the next tile starts afresh
       const double f_top = sm.f[n - 1];
 #pragma unroll
       for (int j = 0; j < PP; ++j) {
-        const long long p = (grp * PP + j) * NT + tid;
-        const double c3 = __ldg(a.cbs + (p < B ? p : 0) * CB_SIZE + CB_AM + 3);
-        r.ex[j] = r.am[j][1] * exp_tab(c3 * (f_top - r.am[j][0]), &mtab);
+        r.ex[j] = g1[j] * exp_tab(c3[j] * (f_top - r.am[j][0]), &mtab);
         r.yp[j] = fma(f_top + df, r.yA[j], r.yB[j]);
         r.At[j] = atan_tab(r.yp[j], &mtab);
 #pragma unroll
         for (int d = 0; d < ND1s; ++d) r.S[j][d] = make_double2(0.0, 0.0);
       }
-      if (t_lo >= kmax) pd_tile_loop<NDET, PP, false>(r, sm, mix, &mtab, t_lo, n, tid);   // warp-uniform: all merger-ringdown
-      else pd_tile_loop<NDET, PP, true>(r, sm, mix, &mtab, t_lo, n, tid);
+      if (t_lo >= k2max) pd_tile_loop<NDET, PP, 0>(r, sm, mix, &mtab, n, tid);          // warp-uniform choices
+      else if (t_lo >= k1max) pd_tile_loop<NDET, PP, 1>(r, sm, mix, &mtab, n, tid);
+      else pd_tile_loop<NDET, PP, 2>(r, sm, mix, &mtab, n, tid);
       // close the tile: dh_d += Re(R_d(f_tlo) S), R_d(f) = C_d exp(i dtq f)
       const double f_lo = sm.f[0];
 #pragma unroll
       for (int j = 0; j < PP; ++j) {
         const long long p = (grp * PP + j) * NT + tid;
         const double* cb = a.cbs + (p < B ? p : 0) * CB_SIZE;
+        const bool valid = p < B && __ldg(cb + CB_VALID) != 0.0;
 #pragma unroll
         for (int d = 0; d < ND1; ++d) {
-          const double cr = __ldg(cb + CB_DET + 4 * (d + 1)), ci = __ldg(cb + CB_DET + 4 * (d + 1) + 1);
+          const double cr = valid ? __ldg(cb + CB_DET + 4 * (d + 1)) : 0.0, ci = valid ? __ldg(cb + CB_DET + 4 * (d + 1) + 1) : 0.0;
           double sn, cs;
-          sincos_qt(__ldg(cb + CB_DET + 4 * (d + 1) + 2) * f_lo, sn, cs);
+          sincos_qt((valid ? __ldg(cb + CB_DET + 4 * (d + 1) + 2) : 0.0) * f_lo, sn, cs);
           const double rx = cr * cs - ci * sn, ry = cr * sn + ci * cs;
           r.acc[j][AL::kDh + d] += fma(rx, r.S[j][d].x, -(ry * r.S[j][d].y));
         }
@@ -358,6 +315,28 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
 #pragma unroll
         for (int i = 0; i < AL::N; ++i) a.partial[((long long)rng * AL::N + i) * a.stride + p] = r.acc[j][i];
       }
+    }
+    // the CTA that finishes the group's last range adds the ranges in range order and writes logL (a ticket per group)
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = (atomicAdd(a.ticket + grp, 1) == a.nranges - 1) ? 1 : 0;
+    __syncthreads();
+    if (s_last) {
+      __threadfence();
+#pragma unroll
+      for (int j = 0; j < PP; ++j) {
+        const long long p = (grp * PP + j) * NT + tid;
+        if (p < B) {
+          double sums[AL::N];
+#pragma unroll
+          for (int i = 0; i < AL::N; ++i) sums[i] = 0.0;
+          for (int c = 0; c < a.nranges; ++c)
+#pragma unroll
+            for (int i = 0; i < AL::N; ++i) sums[i] += __ldcg(a.partial + ((long long)c * AL::N + i) * a.stride + p);
+          a.logl[p] = finish_logl<2, NDET>(cfg, a.cbs + p * CB_SIZE, sums, a.parts ? a.parts + p * 2 * NDET : nullptr);
+        }
+      }
+      if (tid == 0) a.ticket[grp] = 0;
     }
   }
 }

@@ -5,7 +5,7 @@
 //                        per-bin PhenomD-form evaluation
 //   kernels_k1.cuh       k_tables / k_i73 / k_math_tables / k_draw_live / k_prior_transform (ns_init), k_setup, k_bins (CTA per
 //                        particle pair), k_bins_lp + k_finish (lane per particle), k_waveform
-//   kernels_pdlp.cuh     k_pd_lp (PhenomD-form: lane per particle over the merger-ringdown bins + warp per particle below), k_finish_rows
+//   kernels_pdlp.cuh     k_pd_lp (PhenomD-form, lane per row, atan / exp / phasors carried from bin to bin, ticketed finish), k_finish_rows
 //   kernels_relbin.cuh   k_rb_delta / k_rb_select / k_rb_summary / k_relbin (relative binning, R:L24)
 //   kernels_walk.cuh     de_propose, k_walk_simple, k_walk_gw (speculative chunks; exact or relative-binning likelihood)
 //   kernels_wl.cuh       k_wl_head (the walk as batch-wide rounds: resolve + propose + set-up per walker; rows swept by the K1 kernels)
@@ -84,8 +84,10 @@ struct ns_handle {
   double* d_cur_l = nullptr;
   int* d_cnt = nullptr;         // 3 * k
   double* d_cb = nullptr;       // coefficient blocks scratch
-  double* d_partial = nullptr;  // k_bins_lp: per-range partial sums [n_ranges][N][B]
+  double* d_partial = nullptr;  // k_bins_lp / k_pd_lp: per-range partial sums [n_ranges][N][B]
   size_t partial_cap = 0;
+  int* d_ticket = nullptr;      // k_pd_lp: ranges finished per row group (zero between launches)
+  long long ticket_cap = 0;
   int n_sm = 148;
   int opt_inner = 0;            // 0 acceptance walk, 1 hit-and-run slice sampling inside ns_step
   int opt_slice_steps = 0;      // slice steps per replacement (0: 5 per free dimension)
@@ -94,7 +96,7 @@ struct ns_handle {
   int opt_walk_spec = 0;        // 0 auto (per-walker adaptive), 1..32 fixed speculative chunk length
   int opt_walk_stage = 0;       // PhenomD-form exact walk: LDGSTS staging of the sweep's table values (NSGW_OPT_WALK_STAGE; measured slower)
   int opt_bins_kernel = 0;      // 0 auto, 1 CTA-per-particle (k_bins), 2 lane-per-particle (k_bins_lp / k_pd_lp)
-  int opt_walk_kernel = 0;      // 0 auto, 1 CTA per walker (k_walk_gw), 2 worklist rounds swept by k_bins, 3 swept by k_pd_lp (PhenomD-form)
+  int opt_walk_kernel = 0;      // 0 auto (3), 1 CTA per walker (k_walk_gw), 2 worklist rounds swept by k_bins, 3 swept by the lane-per-row kernels
   // worklist walk (kernels_wl.cuh): per-walker state, double-buffered row buffers, host-visible progress
   WlState wl{};
   long long wl_cap_b = 0, wl_cap_r = 0;
@@ -178,7 +180,7 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 #endif
 constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
 constexpr long long kLpMinBatch = 1024;   // below this the CTA-per-particle kernel fills the machine better
-constexpr long long kPdMinBatch = 32768;  // PhenomD-form: k_pd_lp overtakes k_bins only at large batches (measured: 40 vs 36 M evals/s at 65536)
+constexpr long long kPdMinBatch = 16384;  // PhenomD-form: from here k_pd_lp is faster than k_bins (measured: 35.9 vs 34.6 M evals/s at 16384, 44.5 vs 35.9 at 65536)
 
 int ensure_partial(ns_handle* h, size_t n) {
   if (n > h->partial_cap) {
@@ -252,33 +254,36 @@ int pd_pick_kr(const ns_handle* h, long long rows) {
   return kr;
 }
 
-// PhenomD-form rows -> logL through k_pd_lp + k_finish_rows.  cbs [rows][CB_SIZE]; rows_dev (optional, device) overrides `rows` for
-// the task lists (then `rows` is the capacity the buffers and the grid are sized for); kr: bins per range (0: by pd_pick_kr).
+// PhenomD-form rows -> logL through k_pd_lp (which also finishes).  cbs [rows][CB_SIZE]; rows_dev (optional, device) overrides `rows`
+// for the task list (then `rows` is the capacity the buffers and the grid are sized for); kr: bins per range (0: by pd_pick_kr).
 template <int NDET>
 int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* rows_dev, int kr, double* logl, double* parts, cudaStream_t s) {
   using AL = AccLayout<2, NDET>;
   if (kr <= 0) kr = pd_pick_kr(h, rows);
   const int nranges = (h->cfg.n_freq + kr - 1) / kr;
-  int rc = ensure_partial(h, (size_t)rows * (nranges + 1) * AL::N);
+  int rc = ensure_partial(h, (size_t)rows * nranges * AL::N);
   if (rc) return rc;
+  const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
+  if (ngroups > h->ticket_cap) {
+    if (h->d_ticket) cudaFree(h->d_ticket);
+    h->d_ticket = nullptr; h->ticket_cap = 0;
+    CU_CHECK(h, cudaMalloc(&h->d_ticket, sizeof(int) * (size_t)ngroups));
+    CU_CHECK(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(int) * (size_t)ngroups, s));   // the kernel leaves every ticket at zero again
+    h->ticket_cap = ngroups;
+  }
   PdArgs a;
   a.cbs = cbs; a.n_rows = rows; a.n_rows_dev = rows_dev; a.stride = rows; a.kr = kr; a.nranges = nranges; a.partial = h->d_partial;
-  const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
+  a.ticket = h->d_ticket; a.logl = logl; a.parts = parts;
   const long long ntasks = ngroups * nranges;
   const long long grid = std::min<long long>(ntasks, (long long)h->n_sm * kPdOCC);
-  const long long glow = std::min<long long>((rows + kPdLowNT / 32 - 1) / (kPdLowNT / 32), (long long)h->n_sm * kPdLowOCC * 4);
-  k_pd_low<NDET><<<(unsigned)glow, kPdLowNT, 0, s>>>(h->d_cfg, h->tb, a);
-  LAUNCH_CHECK(h);
+  CU_CHECK(h, cudaFuncSetAttribute(k_pd_lp<NDET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pd_mix_bytes<kPdPP>()));
   cudaEvent_t e0 = nullptr, e1 = nullptr;
   if (h->prof && h->prof_ev.size() < 4096) {
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  k_pd_lp<NDET><<<(unsigned)grid, kPdNT, 0, s>>>(h->d_cfg, h->tb, a);
+  k_pd_lp<NDET><<<(unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s>>>(h->d_cfg, h->tb, a);
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
-  LAUNCH_CHECK(h);
-  const long long gfin = std::min<long long>((rows + 127) / 128, (long long)h->n_sm * 8);
-  k_finish_rows<2, NDET><<<(unsigned)gfin, 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges + 1, rows, rows_dev, rows, logl, parts);
   LAUNCH_CHECK(h);
   return 0;
 }
@@ -456,7 +461,7 @@ int ensure_wl(ns_handle* h, long long B, long long R) {
 // logL of the rows of one round (cbs [R cap][CB_SIZE], count on the device) with the batched K1 kernels.
 template <int MODEL, int NDET>
 int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, double* logl, cudaStream_t s) {
-  if (MODEL == 2 && h->opt_walk_kernel == 3) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
+  if (MODEL == 2 && h->opt_walk_kernel != 2) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
   if (MODEL == 1 && R >= kLpMinBatch && h->opt_walk_kernel != 2) return launch_bins_lp<NDET>(h, cbs, R, rows_dev, logl, nullptr, s);
   if (R >= 4096) k_bins<MODEL, NDET, 2><<<(unsigned)((R + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
   else k_bins<MODEL, NDET, 1><<<(unsigned)R, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
@@ -472,7 +477,9 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const long long R = B * e_cap;
   int rc = ensure_wl(h, B, R);
   if (rc) return rc;
-  if (h->wl_kr == 0) h->wl_kr = 128;   // short ranges: the rows of a round vary, many small tasks keep the persistent grid balanced
+  // about 32 ranges per row group whatever the band (measured on configs 3 and 4: 8 and 127 ranges are 10-25 % slower): the rows of a
+  // round vary, many tasks keep the persistent grid balanced; fixed per handle, so a row's sums never depend on the round
+  if (h->wl_kr == 0) h->wl_kr = std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
   WlState st = h->wl;
   st.e_cap = e_cap;
   st.cap_rows = (int)R;
@@ -542,7 +549,7 @@ void ns_free(ns_handle* h) {
   if (!h) return;
   cudaFree(h->d_cfg); cudaFree(h->d_state); cudaFree(h->d_tab); cudaFree(h->d_mtab); cudaFree(h->d_wd); cudaFree(h->d_ws);
   cudaFree(h->d_live_u); cudaFree(h->d_live_l); cudaFree(h->d_order); cudaFree(h->d_surv); cudaFree(h->d_cur_u);
-  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_post_lw); cudaFree(h->d_hio);
+  cudaFree(h->d_cur_l); cudaFree(h->d_cnt); cudaFree(h->d_cb); cudaFree(h->d_partial); cudaFree(h->d_ticket); cudaFree(h->d_theta); cudaFree(h->d_fin); cudaFree(h->d_post_lw); cudaFree(h->d_hio);
   if (h->s_own) cudaStreamDestroy(h->s_own);
   cudaFree(h->d_rb_edge); cudaFree(h->d_rb_buf); cudaFree(h->d_lc);
   cudaFree(h->wl.t0); cudaFree(h->wl.step); cudaFree(h->wl.row_u[0]); cudaFree(h->wl.n_rows);
