@@ -34,9 +34,14 @@ def alg_flops_per_bin(n_det, model="taylorf2"):
     sin 2 FMA + 1 mul (5), cos 3 FMA (6), complex product with the table entry (6) = 19; detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex
     Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
     if model == "phenomd":
-        # merger-ringdown bin (about 80 % of the bins) of the CTA-per-row sweep the worklist walk uses (DESIGN.md section 5): phase 47,
+        # merger-ringdown bin (about 80 % of the bins) as k_bins evaluates it (bins strided over threads; DESIGN.md section 5): phase 47,
         # amplitude 32 + 3, table-driven sincos 21, detector 0: 10, every further detector 18
         return 47 + 35 + 21 + 10 + 18 * (n_det - 1)
+    if model == "phenomd_lane":
+        # the same bin as k_pd_lp evaluates it (lane per row, consecutive bins: the cheaper formulation, so this is the model its
+        # fractions are quoted on): atan carried by the subtraction formula 19, phase 8, Lorentzian with the exponential as a geometric
+        # sequence 9, table-driven sincos 19 + scaling by the amplitude 2, detector 0: 8 + <h,h> 3, every further detector: Horner step 14 + <h,h> 2
+        return 19 + 8 + 9 + 21 + 11 + 16 * (n_det - 1)
     assert model == "taylorf2"
     return 18 + 19 + 8 + 14 * (n_det - 1)
 
@@ -331,15 +336,6 @@ def run_ours(args):
                           "oob_frac": float(cnt["n_oob"].sum()) / (Bw * Wl)}
         # full run: config 3 (PhenomD-form, H1+L1, n_live 1000, k 500, naccept 60, dlogz < 0.1)
         spec3, smp3 = W.config3(wf_cuda_for(nsgw, torch))
-        h3 = nsgw.Handle(spec3, smp3, seed=1)
-        t0 = time.perf_counter()
-        nit, st = h3.run(smp3["term_kind"], smp3["term_tol"], 4000)
-        logz, err, H = h3.finalize_evidence()
-        wall = time.perf_counter() - t0
-        extras["ns_run_config3"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz, "logz_err": err,
-                                    "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
-                                    "evals_per_s": st["n_eval_total"] / wall}
-        h3.close()
         # PhenomD-form batched likelihood on the config-3 data (the model of configs 3-5), B = 65536 prior rows: both sweep kernels
         hp = nsgw.Handle(spec3)
         th3 = hp.prior_transform_batch(u)
@@ -357,11 +353,20 @@ def run_ours(args):
                 b.record(stream)
             torch.cuda.synchronize()
             pms = sum(a.elapsed_time(b) for a, b in evp) / len(evp)
-            pd[name] = {"ms_per_step": pms, "evals_per_s": B / (pms * 1e-3),
-                        "frac_fp64_peak": B * n_freq * alg_flops_per_bin(2, "phenomd") / (pms * 1e-3) / 1e12 / fp64_burst}
-        pd["flops_per_particle_bin_model"] = alg_flops_per_bin(2, "phenomd")
+            mdl = "phenomd" if kern == 1 else "phenomd_lane"
+            pd[name] = {"ms_per_step": pms, "evals_per_s": B / (pms * 1e-3), "flops_per_particle_bin_model": alg_flops_per_bin(2, mdl),
+                        "frac_fp64_peak": B * n_freq * alg_flops_per_bin(2, mdl) / (pms * 1e-3) / 1e12 / fp64_burst}
         extras["phenomd_batch_config3_B65536"] = pd
         hp.close()
+        h3 = nsgw.Handle(spec3, smp3, seed=1)
+        t0 = time.perf_counter()
+        nit, st = h3.run(smp3["term_kind"], smp3["term_tol"], 4000)
+        logz, err, H = h3.finalize_evidence()
+        wall = time.perf_counter() - t0
+        extras["ns_run_config3"] = {"wall_s": wall, "iterations": nit, "n_eval_total": st["n_eval_total"], "logz": logz, "logz_err": err,
+                                    "H": H, "walk_len_last": st["walk_len"], "accept_mean_last": st["accept_mean"],
+                                    "evals_per_s": st["n_eval_total"] / wall}
+        h3.close()
         # config 4: longer segment (8 s at 4096 Hz, 16225 bins), n_live 1400, k 700, live-evidence-fraction rule
         spec4, smp4 = W.config4(wf_cuda_for(nsgw, torch))
         h4 = nsgw.Handle(spec4, smp4, seed=1)
@@ -389,7 +394,7 @@ def run_ours(args):
         # BASELINE.json (10 batch sizes x 3 walk lengths); a point is skipped only if the time budget of the sweep runs out.
         spec5 = W.config5(wf_cuda_for(nsgw, torch))
         h5 = nsgw.Handle(spec5)
-        fl5 = alg_flops_per_bin(3, "phenomd") * spec5["n_freq"]
+        fl5 = alg_flops_per_bin(3, "phenomd_lane") * spec5["n_freq"]
         sweep, skipped = [], []
         t_sweep = time.perf_counter()
         for Bw in (256, 512, 1024, 2048, 4096, 8192, 16384, 32768, 65536, 131072):
@@ -417,7 +422,7 @@ def run_ours(args):
                               "warps_active_sweep_kernel": occ, "frac_fp64_peak": ne * fl5 / (wms * 1e-3) / 1e12 / fp64_burst})
         extras["config5_sweep"] = {"what": "ns_walk_batch, PhenomD-form, 3 detectors x 32449 bins; warps_active = resident warps / 64 of "
                                            "the row-sweep kernel (occupancy API x grid fill at the rows of a full round); frac_fp64_peak = "
-                                           "%d model flops per particle-bin x bins x evaluations / time / measured peak" % alg_flops_per_bin(3, "phenomd"),
+                                           "%d model flops per particle-bin (k_pd_lp's formulation; k_bins' costs %d) x bins x evaluations / time / measured peak" % (alg_flops_per_bin(3, "phenomd_lane"), alg_flops_per_bin(3, "phenomd")),
                                    "points": sweep, "skipped_for_time": skipped}
         h5.close()
         if args.full_extras:

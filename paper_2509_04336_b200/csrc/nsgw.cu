@@ -460,9 +460,9 @@ int ensure_wl(ns_handle* h, long long B, long long R) {
 
 // logL of the rows of one round (cbs [R cap][CB_SIZE], count on the device) with the batched K1 kernels.
 template <int MODEL, int NDET>
-int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, double* logl, cudaStream_t s) {
-  if (MODEL == 2 && h->opt_walk_kernel != 2) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
-  if (MODEL == 1 && R >= kLpMinBatch && h->opt_walk_kernel != 2) return launch_bins_lp<NDET>(h, cbs, R, rows_dev, logl, nullptr, s);
+int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, bool lane, double* logl, cudaStream_t s) {
+  if (MODEL == 2 && lane) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
+  if (MODEL == 1 && lane && R >= kLpMinBatch) return launch_bins_lp<NDET>(h, cbs, R, rows_dev, logl, nullptr, s);
   if (R >= 4096) k_bins<MODEL, NDET, 2><<<(unsigned)((R + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
   else k_bins<MODEL, NDET, 1><<<(unsigned)R, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
   LAUNCH_CHECK(h);
@@ -480,6 +480,21 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   // about 32 ranges per row group whatever the band (measured on configs 3 and 4: 8 and 127 ranges are 10-25 % slower): the rows of a
   // round vary, many tasks keep the persistent grid balanced; fixed per handle, so a row's sums never depend on the round
   if (h->wl_kr == 0) h->wl_kr = std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
+  // Which kernel sweeps the rows: the lane-per-row kernels win once a round holds enough rows (persistent grid, a lane walks 128 bins
+  // serially), the CTA-per-row-pair kernel below that.  Rows per round are known on the device only, so the choice is made once per
+  // call from what the host knows -- walkers x expected chunk length, the chunk length following the acceptance rate the walk length
+  // is tuned to (naccept accepted steps per W): a function of (B, W, naccept), so a call's results do not depend on its chunking.
+  bool lane = h->opt_walk_kernel == 3;
+  if (h->opt_walk_kernel == 0) {
+    int W = a.W;
+    if (a.W_dev) {
+      CU_CHECK(h, cudaMemcpyAsync(h->h_wl_nact, a.W_dev, sizeof(int), cudaMemcpyDeviceToHost, s));
+      CU_CHECK(h, cudaStreamSynchronize(s));
+      W = h->h_wl_nact[0];
+    }
+    const double chunk = std::min<double>(e_cap, std::max(1.0, 0.3 * W / std::max(1, h->cfg.naccept)));
+    lane = (double)B * chunk >= 8192.0;
+  }
   WlState st = h->wl;
   st.e_cap = e_cap;
   st.cap_rows = (int)R;
@@ -492,7 +507,7 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
     LAUNCH_CHECK(h);
     CU_CHECK(h, cudaMemcpyAsync(h->h_wl_nact + (r & 3), st.n_active + par, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(h, cudaEventRecord(h->wl_ev[r & 3], s));
-    rc = sweep_rows<MODEL, NDET>(h, st.row_cb[par], R, st.n_rows + par, st.row_logl[par], s);
+    rc = sweep_rows<MODEL, NDET>(h, st.row_cb[par], R, st.n_rows + par, lane, st.row_logl[par], s);
     if (rc) return rc;
     if (r >= 2) {   // the host runs two rounds ahead of what it has seen: rounds enqueued after the last walker finished are no-ops
       CU_CHECK(h, cudaEventSynchronize(h->wl_ev[(r - 2) & 3]));
@@ -1213,11 +1228,20 @@ int nsgw_sweep_occupancy(ns_handle* h, int64_t rows, double* warps_active_host, 
   if (!is_gw(h->cfg.like_kind) || rows < 1) return fail(h, -1, "bad arguments");
   const int nd = h->cfg.n_det, n_sm = h->n_sm;
   const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
-  if (tf2 && rows >= kLpMinBatch) {
+  if (tf2 && rows >= kLpMinBatch && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 8192))) {
     const long long grid = std::min<long long>((rows + kLpNT * kLpPP - 1) / (kLpNT * kLpPP) * 16, (long long)n_sm * kLpOCC);
     if (nd == 1) return occ_of(k_bins_lp<1, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
     if (nd == 2) return occ_of(k_bins_lp<2, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
     return occ_of(k_bins_lp<3, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
+  }
+  if (!tf2 && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 8192))) {
+    const int kr = h->wl_kr > 0 ? h->wl_kr : std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
+    const long long grid = std::min<long long>((rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP) * ((h->cfg.n_freq + kr - 1) / kr), (long long)n_sm * kPdOCC);
+    const size_t dyn = pd_mix_bytes<kPdPP>();
+    if (nd == 1) { cudaFuncSetAttribute(k_pd_lp<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); return occ_of(k_pd_lp<1>, kPdNT, dyn, grid, n_sm, warps_active_host, ctas_per_sm_host); }
+    if (nd == 2) { cudaFuncSetAttribute(k_pd_lp<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn); return occ_of(k_pd_lp<2>, kPdNT, dyn, grid, n_sm, warps_active_host, ctas_per_sm_host); }
+    cudaFuncSetAttribute(k_pd_lp<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+    return occ_of(k_pd_lp<3>, kPdNT, dyn, grid, n_sm, warps_active_host, ctas_per_sm_host);
   }
   const bool p2 = rows >= 4096;
   const long long grid = p2 ? (rows + 1) / 2 : rows;

@@ -45,12 +45,14 @@ def _midrun_walk_case(nsgw, spec, smp, n_iter, seed):
     return h, donors, ld, lstar
 
 
-@pytest.mark.parametrize("cfg,n_iter,Wlen", [(3, 30, 600), (4, 2, 100)])
-def test_walk_trace_parity_full_shape(nsgw, cfg, n_iter, Wlen):
+# wk = NSGW_OPT_WALK_KERNEL: 2 rounds swept by k_bins, 3 by the lane-per-row kernel (what a full run's long walks use)
+@pytest.mark.parametrize("cfg,n_iter,Wlen,wk", [(3, 30, 600, 2), (3, 30, 600, 3), (4, 2, 100, 2), (4, 2, 100, 3)])
+def test_walk_trace_parity_full_shape(nsgw, cfg, n_iter, Wlen, wk):
     spec, smp = (W.config3 if cfg == 3 else W.config4)(wf)
     assert spec["n_freq"] == (4017 if cfg == 3 else 16225)
     P = O.OracleProblem(spec)
     h, donors, ld, lstar = _midrun_walk_case(nsgw, spec, smp, n_iter, seed=1)
+    h.set_option(6, wk)
     # the live set's logL came from the GPU: the oracle must agree on it (scaled 1e-10 is checked elsewhere; here 1e-8 absolute)
     np.testing.assert_allclose(P.loglike_u(donors[::25]), ld[::25], rtol=0, atol=1e-8)
     B = smp["n_delete"]

@@ -312,12 +312,15 @@ def test_walk_decision_parity(nsgw, kind, B, Wlen, spec_len):
     assert (fl & 1).any() and (fl & 2).any() and ((fl & 4) > (fl & 2) * 2).any()      # the case exercises oob, accept and reject
 
 
-def test_walk_speculation_is_invisible(nsgw):
-    """The speculative chunk length is a scheduling choice: end points, logL, counters and the whole trace are bit-identical
+@pytest.mark.parametrize("wk", [0, 1, 3])
+def test_walk_speculation_is_invisible(nsgw, wk):
+    """wk = NSGW_OPT_WALK_KERNEL (0: automatic = rounds swept by k_bins at this size, 1: one CTA per walker, 3: rounds swept by the
+    lane-per-row kernel).  The speculative chunk length is a scheduling choice: end points, logL, counters and the whole trace are bit-identical
     for every value (the discarded steps are redone from the accepted point with the same Philox counters)."""
     spec = W.gw_spec(W.LIKE_PHENOMD, ["H1", "L1", "V1"], 4.0, 256.0, (20.0, 40.0))
     spec = W.make_data(spec, W.INJ_C3, 12.0, wf)
     h = nsgw.Handle(spec)
+    h.set_option(6, wk)
     rng = np.random.default_rng(11)
     m, B, Wlen = 200, 130, 37
     u_inj = np.array([0.4, 0.771, 0.652, 0.399, 0.0041, 0.0395, 0.8467, 0.2069, 0.5, 0.2196, 0.0317])
