@@ -403,11 +403,14 @@ def run_ours(args):
             order = torch.argsort(l5)
             donors = u5[order[Bw:]].contiguous()
             lstar = float(l5[order[Bw - 1]])
-            occ, ctas = h5.sweep_occupancy(min(65536, 64 * Bw))
             for Wl in (20, 60, 200):
                 if time.perf_counter() - t_sweep > args.sweep_budget_s:
                     skipped.append([Bw, Wl])
                     continue
+                # rows a round is expected to hold (the library's own estimate: walkers x chunk length from W and naccept = 60)
+                occ, ctas = h5.sweep_occupancy(int(Bw * max(1.0, min(64.0, 65536.0 / Bw, 0.3 * Wl / 60.0))))
+                if Wl == 20:        # the first walk of a batch size allocates the round buffers: not part of the timed call
+                    h5.walk_batch(donors, donors.clone(), l5[order[Bw:]].clone(), lstar, 2, 4321, 8)
                 uw, lw = donors.clone(), l5[order[Bw:]].clone()
                 a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 a.record(stream)

@@ -258,7 +258,7 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * 0 (default) = plain loads.  A tuning switch. */
 #define NSGW_OPT_WALK_STAGE 5
 /* key NSGW_OPT_WALK_KERNEL: how ns_step / ns_run / ns_walk_batch run the acceptance walk on a GW likelihood.  0 = automatic
- * (exact likelihood: 3 when walkers x expected chunk length -- from the walk length and naccept -- reaches 8192 rows per round, else 2;
+ * (exact likelihood: 3 when walkers x expected chunk length -- from the walk length and naccept -- reaches 12000 rows per round, else 2;
  * relative binning: 1); 1 = one CTA per walker, all steps in one launch (k_walk_gw); 2 and 3 =
  * batch-wide rounds: every walker proposes a chunk of steps, the likelihood of all the batch's in-bounds proposals is evaluated in one
  * launch, every walker resolves its chunk (first acceptance discards the later steps), repeat; the host follows the device two rounds

@@ -254,14 +254,9 @@ int pd_pick_kr(const ns_handle* h, long long rows) {
   return kr;
 }
 
-// PhenomD-form rows -> logL through k_pd_lp (which also finishes).  cbs [rows][CB_SIZE]; rows_dev (optional, device) overrides `rows`
-// for the task list (then `rows` is the capacity the buffers and the grid are sized for); kr: bins per range (0: by pd_pick_kr).
-template <int NDET>
-int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* rows_dev, int kr, double* logl, double* parts, cudaStream_t s) {
-  using AL = AccLayout<2, NDET>;
-  if (kr <= 0) kr = pd_pick_kr(h, rows);
-  const int nranges = (h->cfg.n_freq + kr - 1) / kr;
-  int rc = ensure_partial(h, (size_t)rows * nranges * AL::N);
+// Scratch of k_pd_lp for `rows` rows: per-range partial sums and one ticket per row group.
+int ensure_pd_scratch(ns_handle* h, long long rows, int nranges, int nacc, cudaStream_t s) {
+  int rc = ensure_partial(h, (size_t)rows * nranges * nacc);
   if (rc) return rc;
   const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
   if (ngroups > h->ticket_cap) {
@@ -271,6 +266,19 @@ int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* row
     CU_CHECK(h, cudaMemsetAsync(h->d_ticket, 0, sizeof(int) * (size_t)ngroups, s));   // the kernel leaves every ticket at zero again
     h->ticket_cap = ngroups;
   }
+  return 0;
+}
+
+// PhenomD-form rows -> logL through k_pd_lp (which also finishes).  cbs [rows][CB_SIZE]; rows_dev (optional, device) overrides `rows`
+// for the task list (then `rows` is the capacity the buffers and the grid are sized for); kr: bins per range (0: by pd_pick_kr).
+template <int NDET>
+int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* rows_dev, int kr, double* logl, double* parts, cudaStream_t s) {
+  using AL = AccLayout<2, NDET>;
+  if (kr <= 0) kr = pd_pick_kr(h, rows);
+  const int nranges = (h->cfg.n_freq + kr - 1) / kr;
+  int rc = ensure_pd_scratch(h, rows, nranges, AL::N, s);
+  if (rc) return rc;
+  const long long ngroups = (rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
   PdArgs a;
   a.cbs = cbs; a.n_rows = rows; a.n_rows_dev = rows_dev; a.stride = rows; a.kr = kr; a.nranges = nranges; a.partial = h->d_partial;
   a.ticket = h->d_ticket; a.logl = logl; a.parts = parts;
@@ -469,17 +477,30 @@ int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev
   return 0;
 }
 
-template <int MODEL, int NDET>
-int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
-  const long long B = a.B;
-  // rows per walker and round: up to 64 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
-  const int e_cap = (int)std::max<long long>(1, std::min<long long>(kWlEMax, 65536 / B));
-  const long long R = B * e_cap;
+// rows per walker and round: up to 64 while that keeps a round near 64 Ki rows (large batches fill the machine with short chunks)
+int wl_e_cap(long long B) { return (int)std::max<long long>(1, std::min<long long>(kWlEMax, 65536 / std::max<long long>(B, 1))); }
+
+// Buffers of the worklist walk for B walkers (and the lane kernel's scratch for PhenomD-form), so that the first walk of a handle does
+// not pay for allocations.
+int wl_prepare(ns_handle* h, long long B, cudaStream_t s) {
+  const long long R = B * wl_e_cap(B);
   int rc = ensure_wl(h, B, R);
   if (rc) return rc;
   // about 32 ranges per row group whatever the band (measured on configs 3 and 4: 8 and 127 ranges are 10-25 % slower): the rows of a
   // round vary, many tasks keep the persistent grid balanced; fixed per handle, so a row's sums never depend on the round
   if (h->wl_kr == 0) h->wl_kr = std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
+  if (h->cfg.like_kind == NSGW_LIKE_GW_PHENOMD_FORM && h->opt_walk_kernel != 2)
+    return ensure_pd_scratch(h, R, (h->cfg.n_freq + h->wl_kr - 1) / h->wl_kr, 2 + (h->cfg.n_det - 1) + h->cfg.n_det, s);
+  return 0;
+}
+
+template <int MODEL, int NDET>
+int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
+  const long long B = a.B;
+  const int e_cap = wl_e_cap(B);
+  const long long R = B * e_cap;
+  int rc = wl_prepare(h, B, s);
+  if (rc) return rc;
   // Which kernel sweeps the rows: the lane-per-row kernels win once a round holds enough rows (persistent grid, a lane walks 128 bins
   // serially), the CTA-per-row-pair kernel below that.  Rows per round are known on the device only, so the choice is made once per
   // call from what the host knows -- walkers x expected chunk length, the chunk length following the acceptance rate the walk length
@@ -493,7 +514,7 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
       W = h->h_wl_nact[0];
     }
     const double chunk = std::min<double>(e_cap, std::max(1.0, 0.3 * W / std::max(1, h->cfg.naccept)));
-    lane = (double)B * chunk >= 8192.0;
+    lane = (double)B * chunk >= 12000.0;
   }
   WlState st = h->wl;
   st.e_cap = e_cap;
@@ -710,6 +731,10 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
     }
     int rc = loglike_u(h, h->d_live_u, n, h->d_live_l, s);
     if (rc) return bail(rc);
+    if (gw) {
+      rc = wl_prepare(h, k, s);
+      if (rc) return bail(rc);
+    }
   }
   INIT_CHECK(cudaStreamSynchronize(s), -2);
   INIT_CHECK(cudaGetLastError(), -2);
@@ -1228,13 +1253,13 @@ int nsgw_sweep_occupancy(ns_handle* h, int64_t rows, double* warps_active_host, 
   if (!is_gw(h->cfg.like_kind) || rows < 1) return fail(h, -1, "bad arguments");
   const int nd = h->cfg.n_det, n_sm = h->n_sm;
   const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
-  if (tf2 && rows >= kLpMinBatch && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 8192))) {
+  if (tf2 && rows >= kLpMinBatch && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 12000))) {
     const long long grid = std::min<long long>((rows + kLpNT * kLpPP - 1) / (kLpNT * kLpPP) * 16, (long long)n_sm * kLpOCC);
     if (nd == 1) return occ_of(k_bins_lp<1, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
     if (nd == 2) return occ_of(k_bins_lp<2, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
     return occ_of(k_bins_lp<3, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
   }
-  if (!tf2 && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 8192))) {
+  if (!tf2 && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 12000))) {
     const int kr = h->wl_kr > 0 ? h->wl_kr : std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
     const long long grid = std::min<long long>((rows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP) * ((h->cfg.n_freq + kr - 1) / kr), (long long)n_sm * kPdOCC);
     const size_t dyn = pd_mix_bytes<kPdPP>();
