@@ -96,6 +96,22 @@ int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* l
  * Synchronises before returning. */
 int gw_loglike_batch_host(ns_handle* h, const double* theta_host, int64_t B, double* logl_host, void* stream);
 
+/* gw_loglike_batch for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
+ * the same kernels (k_setup -> k_bins_lp + k_finish for TaylorF2, k_setup -> k_pd_lp for PhenomD-form; R:L1) with their scratch
+ * -- coefficient blocks, per-range partial sums, tickets -- in ONE file-scope device array of NSGW_NOALLOC_SCRATCH_BYTES
+ * (16.1 MiB) that every GPU loading the library holds until exit.  Calls no cudaMalloc / cudaFree and no allocating library
+ * routine; enqueues on `stream` and does not synchronise.  theta_dev [B, 11] and logl_dev [B] are the caller's device buffers.
+ * Limits: B <= NSGW_NOALLOC_MAX_ROWS and the handle's n_freq <= NSGW_NOALLOC_MAX_BINS; beyond either the call returns -5 with
+ * the limit in ns_last_error and launches nothing (split the batch, or use gw_loglike_batch).  Every call on a device shares
+ * the array: calls that overlap on the GPU (two streams, two handles, two host threads) race -- keep them on one stream or order
+ * them with events.  The array keeps the last call's contents; the call clears what must start at zero itself.  Ranges are
+ * 256 bins whatever B is, so logl_dev agrees with gw_loglike_batch to rounding order (1e-10 relative), not bit for bit.
+ * Errors as gw_loglike_batch; the current device must be the handle's. */
+#define NSGW_NOALLOC_MAX_ROWS 4096
+#define NSGW_NOALLOC_MAX_BINS 16384
+#define NSGW_NOALLOC_SCRATCH_BYTES 16908544
+int gw_loglike_batch_noalloc(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, void* stream);
+
 /* Detector-frame signal of ONE parameter row on the handle's grid: out_dev [n_det, n_freq, 2] (R:L3). Used to build injections. */
 int gw_waveform(ns_handle* h, const double* theta_dev, double* out_dev, void* stream);
 

@@ -1328,3 +1328,113 @@ int nsgw_measure_fp64_peak(int64_t iters, double* tflops_host, void* stream) {
 }
 
 }  // extern "C"
+
+// ======================================================================================================
+// gw_loglike_batch_noalloc: the batched likelihood for callers that cannot allocate (include/nsgw.h)
+// ======================================================================================================
+// The coefficient blocks, the per-range partial sums and the tickets of k_bins_lp / k_pd_lp live in ONE file-scope device array of
+// fixed size instead of the handle's grow-on-demand buffers.  Every device that loads the library holds the array until exit; every
+// call on a device shares it.  In host code `g_na_scratch` is a host-side stand-in, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, once per device, with that device current.
+constexpr long long kNaMaxRows = NSGW_NOALLOC_MAX_ROWS;
+constexpr int kNaMaxBins = NSGW_NOALLOC_MAX_BINS;
+constexpr int kNaKr = 256;                                    // bins per range in this entry point (both kernels)
+constexpr int kNaMaxRanges = (kNaMaxBins + kNaKr - 1) / kNaKr;
+constexpr int kNaMaxAcc = 7;                                  // AccLayout<2, 3>::N, the widest row of partial sums
+constexpr int kNaTickets = 64;                                // ints; >= row groups of kNaMaxRows rows
+constexpr size_t kNaCbDoubles = (size_t)kNaMaxRows * CB_SIZE;
+constexpr size_t kNaPartialDoubles = (size_t)kNaMaxRows * kNaMaxRanges * kNaMaxAcc;
+constexpr size_t kNaDoubles = kNaCbDoubles + kNaPartialDoubles + kNaTickets / 2;
+static_assert(AccLayout<2, 3>::N == kNaMaxAcc && AccLayout<1, 3>::N <= kNaMaxAcc, "partial-sum width");
+static_assert((kNaMaxRows + kPdNT * kPdPP - 1) / (kPdNT * kPdPP) <= kNaTickets, "tickets");
+static_assert(kNaKr % kPdKT == 0 && kNaKr <= kLpKR && kNaKr % kLpUNR == 0, "range length fits both kernels");
+static_assert(kNaDoubles * sizeof(double) <= (size_t)NSGW_NOALLOC_SCRATCH_BYTES, "scratch size stated in nsgw.h");
+
+static __device__ __align__(256) double g_na_scratch[kNaDoubles];   // 16.1 MiB: [rows][CB_SIZE] | [ranges][N][rows] | tickets
+
+namespace {
+
+constexpr int kNaMaxDevices = 64;
+std::atomic<double*> g_na_ptr[kNaMaxDevices];   // device address of g_na_scratch per device ordinal (null: not asked yet)
+
+// Device address of the current device's copy of g_na_scratch.
+int na_scratch(ns_handle* h, double** out) {
+  int dev = -1;
+  CU_CHECK(h, cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNaMaxDevices) return fail(h, -5, "gw_loglike_batch_noalloc: device ordinal beyond 63");
+  double* p = g_na_ptr[dev].load(std::memory_order_acquire);
+  if (!p) {
+    CU_CHECK(h, cudaGetSymbolAddress((void**)&p, g_na_scratch));
+    if (!p) return fail(h, -2, "gw_loglike_batch_noalloc: cudaGetSymbolAddress returned a null address");
+    g_na_ptr[dev].store(p, std::memory_order_release);   // two first callers get the same address: the race is benign
+  }
+  *out = p;
+  return 0;
+}
+
+template <int NDET>
+int na_launch(ns_handle* h, const double* theta_dev, long long B, double* logl, cudaStream_t s, double* scratch) {
+  const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
+  double* cbs = scratch;
+  double* partial = scratch + kNaCbDoubles;
+  int* ticket = reinterpret_cast<int*>(scratch + kNaCbDoubles + kNaPartialDoubles);
+  const int nranges = (h->cfg.n_freq + kNaKr - 1) / kNaKr;
+  const unsigned gs = (unsigned)((B + 127) / 128);
+  if (tf2) {
+    constexpr int NT = kLpNT, PP = kLpPP;
+    const long long ngroups = (B + NT * PP - 1) / (NT * PP);
+    const long long ntasks = ngroups * nranges;
+    const long long grid = std::min<long long>(ntasks, (long long)h->n_sm * kLpOCC);
+    k_setup<1><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, cbs);
+    LAUNCH_CHECK(h);
+    // every (range, sum, row < B) entry of `partial` the finishing pass reads is written by this launch: nothing to clear
+    k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, cbs, B, nullptr, kNaKr, nranges, ntasks, partial);
+    LAUNCH_CHECK(h);
+    k_finish<1, NDET><<<gs, 128, 0, s>>>(h->d_cfg, cbs, partial, nranges, B, logl, nullptr);
+    LAUNCH_CHECK(h);
+    return 0;
+  }
+  const long long ngroups = (B + kPdNT * kPdPP - 1) / (kPdNT * kPdPP);
+  const long long ntasks = ngroups * nranges;
+  const long long grid = std::min<long long>(ntasks, (long long)h->n_sm * kPdOCC);
+  // the tickets must start at zero; the array keeps whatever the last call (possibly an aborted one) left
+  CU_CHECK(h, cudaMemsetAsync(ticket, 0, sizeof(int) * kNaTickets, s));
+  k_setup<2><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, cbs);
+  LAUNCH_CHECK(h);
+  PdArgs a;
+  a.cbs = cbs; a.n_rows = B; a.n_rows_dev = nullptr; a.stride = B; a.kr = kNaKr; a.nranges = nranges; a.partial = partial;
+  a.ticket = ticket; a.logl = logl; a.parts = nullptr;
+  CU_CHECK(h, cudaFuncSetAttribute(k_pd_lp<NDET>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)pd_mix_bytes<kPdPP>()));
+  k_pd_lp<NDET><<<(unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s>>>(h->d_cfg, h->tb, a);
+  LAUNCH_CHECK(h);
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gw_loglike_batch_noalloc(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, void* stream) {
+  if (!h) return -3;
+  if (!is_gw(h->cfg.like_kind)) return fail(h, -3, "handle has no GW likelihood");
+  if (B < 0 || (B > 0 && (!theta_dev || !logl_dev))) return fail(h, -1, "bad arguments");
+  if (B > kNaMaxRows)
+    return fail(h, -5, "gw_loglike_batch_noalloc: B = " + std::to_string((long long)B) + " rows exceed NSGW_NOALLOC_MAX_ROWS = " +
+                           std::to_string(kNaMaxRows) + " (split the batch, or use gw_loglike_batch)");
+  if (h->cfg.n_freq > kNaMaxBins)
+    return fail(h, -5, "gw_loglike_batch_noalloc: n_freq = " + std::to_string(h->cfg.n_freq) + " bins exceed NSGW_NOALLOC_MAX_BINS = " +
+                           std::to_string(kNaMaxBins) + " (use gw_loglike_batch)");
+  if (B == 0) return 0;
+  double* scratch = nullptr;
+  int rc = na_scratch(h, &scratch);
+  if (rc) return rc;
+  cudaStream_t s = (cudaStream_t)stream;
+  switch (h->cfg.n_det) {
+    case 1: return na_launch<1>(h, theta_dev, B, logl_dev, s, scratch);
+    case 2: return na_launch<2>(h, theta_dev, B, logl_dev, s, scratch);
+    case 3: return na_launch<3>(h, theta_dev, B, logl_dev, s, scratch);
+    default: return fail(h, -5, "n_det must be 1..3 for the GW kernels");
+  }
+}
+
+}  // extern "C"

@@ -50,9 +50,10 @@ class NsState(C.Structure):
 EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglike_batch_host", "gw_waveform", "ns_prior_transform_batch",
            "ns_loglike_u_batch", "ns_walk_batch", "ns_step", "ns_run", "ns_run_many", "ns_slice_batch", "ns_relbin_setup", "ns_relbin_get", "gw_loglike_relbin_batch", "ns_get_live", "ns_finalize_evidence", "ns_posterior", "ns_posterior_resample",
            "nsgw_measure_fp64_peak", "nsgw_launch_count", "nsgw_profile_enable", "nsgw_profile_read", "nsgw_set_option",
-           "ns_get_state", "ns_set_state", "nsgw_sweep_occupancy"]
+           "ns_get_state", "ns_set_state", "nsgw_sweep_occupancy", "gw_loglike_batch_noalloc"]
 
 # nsgw_set_option keys (include/nsgw.h)
+NOALLOC_MAX_ROWS, NOALLOC_MAX_BINS = 4096, 16384     # gw_loglike_batch_noalloc (include/nsgw.h)
 OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS, OPT_WALK_STAGE, OPT_WALK_KERNEL = 0, 1, 2, 3, 4, 5, 6
 
 _lib = None
@@ -188,6 +189,15 @@ class Handle:
         self._check(lib().gw_loglike_batch_host(self._h, C.c_void_p(theta_host.data_ptr()), C.c_int64(B),
                                                 C.c_void_p(out_host.data_ptr()), _stream()), "gw_loglike_batch_host")
         return out_host
+
+    def gw_loglike_batch_noalloc(self, theta, out):
+        """gw_loglike_batch with the kernels' scratch in the library's fixed device array: no allocation inside the call (the
+        caller passes `out` [B]).  B <= NOALLOC_MAX_ROWS, n_freq <= NOALLOC_MAX_BINS, else NsgwError; calls that overlap on the
+        GPU race on the shared array."""
+        assert theta.dtype == torch.float64 and out.dtype == torch.float64 and out.shape[0] == theta.shape[0]
+        self._check(lib().gw_loglike_batch_noalloc(self._h, _ptr(theta), C.c_int64(theta.shape[0]), _ptr(out), _stream()),
+                    "gw_loglike_batch_noalloc")
+        return out
 
     def gw_waveform(self, theta):
         out = torch.empty(self.n_det, self.n_freq, 2, dtype=torch.float64, device="cuda")
