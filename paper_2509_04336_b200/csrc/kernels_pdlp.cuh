@@ -57,6 +57,16 @@ struct PdArgs {
   double* parts;              // optional [rows][2 NDET]
 };
 
+// Takes a ticket of a row group on behalf of the CTA: one thread, behind a CTA-wide barrier that follows the CTA's stores.  Returns the
+// number of tickets taken before.  acq_rel at device scope: the release half orders the CTA's stores (observed through the barrier)
+// before the ticket, the acquire half orders the ticket before the loads that follow the next barrier.  (One MEMBAR + one L1
+// invalidate by one thread per task; __threadfence() by every thread before and after cost 0.5 % of a config-3 run.)
+__device__ __forceinline__ int pd_ticket_take(int* t) {
+  int old;
+  asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(t) : "memory");
+  return old;
+}
+
 // Odd Taylor coefficients of atan beyond the linear term: -1/3, 1/5, -1/7.
 __constant__ double kAtanR[3] = {-1.0 / 3.0, 0.2, -1.0 / 7.0};
 
@@ -317,12 +327,11 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
       }
     }
     // the CTA that finishes the group's last range adds the ranges in range order and writes logL (a ticket per group)
-    __threadfence();
+    // (release: the CTA's stores -> barrier -> thread 0's acq_rel ticket; acquire: ticket -> barrier -> the CTA's L2 loads)
     __syncthreads();
-    if (tid == 0) s_last = (atomicAdd(a.ticket + grp, 1) == a.nranges - 1) ? 1 : 0;
+    if (tid == 0) s_last = (pd_ticket_take(a.ticket + grp) == a.nranges - 1) ? 1 : 0;
     __syncthreads();
     if (s_last) {
-      __threadfence();
 #pragma unroll
       for (int j = 0; j < PP; ++j) {
         const long long p = (grp * PP + j) * NT + tid;

@@ -61,7 +61,10 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
   double inb = 0.25;                    // in-bounds fraction of the walker's proposals (estimate: its last chunk)
   if (round == 0) {
     t0 = 0;
-    E = spec_fixed ? spec : min(spec, 2);
+    // first chunk: about the number of rows to the first acceptance when the walk length is tuned to naccept acceptances (W / 100 for
+    // the usual 60 of a third of the steps in bounds) -- 2 for the short walks of the first iterations, where most chunks end early,
+    // near the cap for long walks, where doubling up from 2 costs four half-empty rounds
+    E = spec_fixed ? spec : min(spec, max(2, W / 100));
     if (lane < 3) st.cnt[lane * a.B + row] = 0;
   } else {
     // ---- resolve the pending chunk: steps in order, the first acceptance ends it ---------------------------------------
