@@ -194,12 +194,13 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const int nf = cfg.n_freq;
   const double f_min = cfg.f_min, df = cfg.df;
+  load_math_tables(&mtab, tb.mt, tid, NT);     // built at ns_init: not the previous kernel's output
+  pdl_wait();                                  // the rows (count, coefficient blocks) are
   const long long B = a.n_rows_dev ? (long long)*a.n_rows_dev : a.n_rows;
   if (B <= 0) return;
   const long long ngroups = (B + NR - 1) / NR;
   const long long ntasks = ngroups * a.nranges;
   if (blockIdx.x >= ntasks) return;
-  load_math_tables(&mtab, tb.mt, tid, NT);
   __syncthreads();
   for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
     const long long grp = task / a.nranges;

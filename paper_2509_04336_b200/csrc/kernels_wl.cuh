@@ -9,8 +9,8 @@
 //                                  and waveform set-up one row per lane;
 //   row sweep   (nsgw.cu)          the likelihood of EVERY row of the batch in one launch of the batched likelihood kernels
 //                                  (k x E = 16 000 rows on config 3: the machine is full, tables are reused across rows);
-// chained on the stream; the host reads back the number of walkers still walking two rounds behind the device and stops enqueuing
-// when it reaches zero (rounds enqueued past the end are no-ops).  Decisions, counters, trace and end points are exactly those of
+// chained on the stream; round r + 1's kernel publishes the number of walkers that still walked in round r to mapped host memory, the
+// host follows the device two rounds behind and stops enqueuing when the number reaches zero (rounds enqueued past the end are no-ops).  Decisions, counters, trace and end points are exactly those of
 // the sequential algorithm and of k_walk_gw for every chunk length: a row's logL does not depend on the rows it shares a launch
 // with, and the speculative steps after an acceptance are redone from the accepted point with the same Philox counters.
 #pragma once
@@ -34,6 +34,8 @@ struct WlState {
   int* n_rows;            // [2] rows of the round (by parity)
   int* n_active;          // [2] walkers that proposed in the round (by parity)
   int* sum_need;          // [3] by round mod 3: rows the batch still needs (sum over walkers of remaining steps x in-bounds fraction)
+  int* host_nact;         // [4] pinned host memory the device can write: n_active of round r at [r & 3], published by round r + 1's kernel
+  int nact_slot;          // (r - 1) & 3 for the launch of round r
   int e_cap;              // rows per walker and round (<= kWlEMax)
   int r_target;           // rows per round the chunk lengths aim for
   int cap_rows;           // rows the row buffers hold (B x e_cap)
@@ -50,7 +52,13 @@ __global__ void __launch_bounds__(32 * kWlWarps) k_wl_head(const DevCfg* __restr
   const int lane = threadIdx.x & 31, wrp = threadIdx.x >> 5;
   const long long row = blockIdx.x;
   const int par = round & 1;
-  if (blockIdx.x == 0 && threadIdx.x == 0) { st.n_rows[par ^ 1] = 0; st.n_active[par ^ 1] = 0; st.sum_need[(round + 1) % 3] = 0; }
+  pdl_wait();   // the sweep of the previous round wrote the rows' logL
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    // the previous round's walker count goes to the host by a store into mapped memory (a copy in the stream between this kernel and
+    // the sweep would serialise kernel -> copy engine -> kernel every round); the host reads it behind an event that follows this kernel
+    if (round > 0) { st.host_nact[st.nact_slot] = st.n_active[par ^ 1]; __threadfence_system(); }
+    st.n_rows[par ^ 1] = 0; st.n_active[par ^ 1] = 0; st.sum_need[(round + 1) % 3] = 0;
+  }
   if (wrp == 0) {
   const int W = a.W_dev ? *a.W_dev : a.W;
   const double lstar = a.lstar_dev ? *a.lstar_dev : a.lstar;

@@ -101,7 +101,8 @@ struct ns_handle {
   WlState wl{};
   long long wl_cap_b = 0, wl_cap_r = 0;
   int wl_kr = 0;                // bins per range of k_pd_lp on the walk's rows: fixed per handle so a row's logL never depends on the round
-  int* h_wl_nact = nullptr;     // pinned ring [4]
+  int* h_wl_nact = nullptr;     // pinned, mapped ring [4]: walkers of a round, written by the next round's kernel
+  int* d_wl_nact = nullptr;     // its device address
   cudaEvent_t wl_ev[4] = {nullptr, nullptr, nullptr, nullptr};
   long long cb_cap = 0;
   double* d_theta = nullptr;    // scratch theta
@@ -238,6 +239,19 @@ int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows
   return 0;
 }
 
+// Launch with programmatic stream serialization: the kernel may become resident while the kernel before it on the stream still runs;
+// it calls pdl_wait() before it reads what that kernel wrote.
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(grid); lc.blockDim = dim3(block); lc.dynamicSmemBytes = smem; lc.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  return cudaLaunchKernelEx(&lc, kern, KArgs(args)...);
+}
+
 // Bins per range of k_pd_lp for `rows` rows (multiple of the tile length): the value that minimises rounds x (range + per-task
 // overhead) over the persistent grid, rounds = ceil(tasks / CTA slots).
 int pd_pick_kr(const ns_handle* h, long long rows) {
@@ -290,7 +304,11 @@ int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* row
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  k_pd_lp<NDET><<<(unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s>>>(h->d_cfg, h->tb, a);
+  if (rows_dev) {   // a round of the worklist walk: programmatic dependent launch behind k_wl_head (kernels_wl.cuh)
+    CU_CHECK(h, launch_pdl(k_pd_lp<NDET>, (unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s, (const DevCfg*)h->d_cfg, h->tb, a));
+  } else {
+    k_pd_lp<NDET><<<(unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s>>>(h->d_cfg, h->tb, a);
+  }
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
   return 0;
@@ -437,7 +455,8 @@ int launch_walk_gw(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
 // Buffers for B walkers and R = B x e_cap rows per round.  One allocation per kind (int state, step maps, row doubles, counters).
 int ensure_wl(ns_handle* h, long long B, long long R) {
   if (!h->h_wl_nact) {
-    CU_CHECK(h, cudaMallocHost(&h->h_wl_nact, sizeof(int) * 4));
+    CU_CHECK(h, cudaHostAlloc((void**)&h->h_wl_nact, sizeof(int) * 4, cudaHostAllocMapped));
+    CU_CHECK(h, cudaHostGetDevicePointer((void**)&h->d_wl_nact, h->h_wl_nact, 0));
     for (auto& e : h->wl_ev) CU_CHECK(h, cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     CU_CHECK(h, cudaMalloc(&h->wl.n_rows, sizeof(int) * 8));
     h->wl.n_active = h->wl.n_rows + 2;
@@ -517,6 +536,7 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
     lane = (double)B * chunk >= 12000.0;
   }
   WlState st = h->wl;
+  st.host_nact = h->d_wl_nact;
   st.e_cap = e_cap;
   st.cap_rows = (int)R;
   st.r_target = (int)std::min<long long>(R, std::max<long long>(16384, 24 * B));
@@ -524,14 +544,17 @@ int run_walk_wl(ns_handle* h, const WalkArgs& a, cudaStream_t s) {
   const unsigned gh = (unsigned)B;   // one CTA (kWlWarps warps) per walker
   for (long long r = 0;; ++r) {
     const int par = (int)(r & 1);
-    k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, (int)std::min<long long>(r, 6 + r % 6));   // first round or not, parity and round mod 3 matter
+    st.nact_slot = (int)((r + 3) & 3);
+    const int rcode = (int)std::min<long long>(r, 6 + r % 6);   // first round or not, parity and round mod 3 matter
+    if (r == 0) k_wl_head<MODEL><<<gh, 32 * kWlWarps, 0, s>>>(h->d_cfg, a, st, rcode);
+    else CU_CHECK(h, launch_pdl(k_wl_head<MODEL>, gh, 32 * kWlWarps, 0, s, (const DevCfg*)h->d_cfg, a, st, rcode));   // behind the sweep
     LAUNCH_CHECK(h);
-    CU_CHECK(h, cudaMemcpyAsync(h->h_wl_nact + (r & 3), st.n_active + par, sizeof(int), cudaMemcpyDeviceToHost, s));
     CU_CHECK(h, cudaEventRecord(h->wl_ev[r & 3], s));
     rc = sweep_rows<MODEL, NDET>(h, st.row_cb[par], R, st.n_rows + par, lane, st.row_logl[par], s);
     if (rc) return rc;
-    if (r >= 2) {   // the host runs two rounds ahead of what it has seen: rounds enqueued after the last walker finished are no-ops
-      CU_CHECK(h, cudaEventSynchronize(h->wl_ev[(r - 2) & 3]));
+    if (r >= 2) {   // round r - 1's kernel published the walkers of round r - 2; the host runs ahead of what it has seen, and rounds
+                    // enqueued after the last walker finished are no-ops
+      CU_CHECK(h, cudaEventSynchronize(h->wl_ev[(r - 1) & 3]));
       if (h->h_wl_nact[(r - 2) & 3] == 0) break;
     }
   }

@@ -185,6 +185,14 @@ __device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, doubl
   s = fma(T.y, pc, T.x * ps);
 }
 
+// Programmatic dependent launch (a kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start while the
+// kernel before it on the stream still runs): pdl_wait() returns once that kernel has completed and its writes are visible -- everything
+// it produced is read after this (a no-op in a kernel launched the ordinary way).  The kernels here never signal early
+// (griddepcontrol.launch_dependents): the next kernel's CTAs then become resident as this one's exit, which hides the launch latency;
+// signalling at the start of k_wl_head and k_pd_lp, or after k_wl_head's proposals, made the config-3 run 25 % and 4 % SLOWER (the early
+// CTAs of the persistent sweep land where there is room and wait there).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // 1/d for finite normal d well inside the exponent range (no special cases): MUFU.RCP64H seed (>= 20 bits) and two Newton
 // steps (relative error 2^-20 -> 2^-40 -> 2^-80, i.e. rounding-limited).  The hot loops only divide by sums of squares of
 // O(1..1e6) magnitude.
