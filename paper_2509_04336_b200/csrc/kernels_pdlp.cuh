@@ -6,8 +6,9 @@
 // a + b f + c/f + d f^3/4 + e atan((f - f0)/fd), amplitude = Lorentzian x exponential -- and differ between rows only in the
 // coefficients: lane = row, coefficients in registers, the bins' table values broadcast from a shared-memory tile, no cross-lane
 // reduction, no per-bin global traffic (the design that took TaylorF2 to 0.63 of the FP64 peak).  Consecutive bins of a lane let the
-// expensive functions be CARRIED: atan by atan y' = atan y - atan((y - y') / (1 + y y')), the exponential as a geometric sequence, the
-// detector phasors by Horner's rule -- 56 FP64 instructions per particle-bin against 77 in the bins-strided-over-threads k_bins.
+// expensive functions be CARRIED: atan by atan y' = atan y - atan((y - y') / (1 + y y')) with y - y' = yA df the same for every bin, the
+// exponential as a geometric sequence, the detector phasors by Horner's rule -- 54 FP64 instructions per particle-bin against 77 in the
+// bins-strided-over-threads k_bins.
 // Where the merger-ringdown region starts depends on the row (total mass, final spin), so below the highest start of a warp's rows
 // the lanes disagree on the formula: those tiles evaluate the candidate formulas of the regions present and select per lane by the row's
 // own boundaries, with the extra coefficients read from a shared-memory block staged per task (conflict-free: consecutive lanes,
@@ -80,7 +81,7 @@ constexpr size_t pd_mix_bytes() { return sizeof(double) * kPdMixAll * kPdNT * PP
 template <int NDET, int PP>
 struct PdRow {
   static constexpr int ND1s = NDET > 1 ? NDET - 1 : 1;
-  double pm[PP][5], yA[PP], yB[PP], am[PP][3], exd[PP];
+  double pm[PP][5], yA[PP], yB[PP], dy[PP], am[PP][3], exd[PP];
   double2 St[PP][ND1s];
   double acc[PP][AccLayout<2, NDET>::N];
   // per tile
@@ -112,12 +113,13 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
     for (int j = 0; j < PP; ++j) {
       // atan((f - f0)/fd) carried down from the bin above: atan(y') = atan(y) - atan((y - y') / (1 + y y'))
       const double y = fma(f, r.yA[j], r.yB[j]);
-      const double t = (r.yp[j] - y) * rcp_nr1(fma(y, r.yp[j], 1.0));
+      const double t = r.dy[j] * rcp_nr1(fma(y, r.yp[j], 1.0));     // the bins are equally spaced: y' - y = yA df
       r.yp[j] = y;
       const double z = t * t;
       double pa = fma(z, kAtanR[2], kAtanR[1]);     // |t| <= df / fd < 0.03: t^9/9 < 1e-15
       pa = fma(pa, z, kAtanR[0]);
-      r.At[j] -= fma(t * z, pa, t);
+      pa = fma(pa, z, 1.0);
+      r.At[j] = fma(-t, pa, r.At[j]);
       double q = fma(r.pm[j][1], f, r.pm[j][0]);
       q = fma(r.pm[j][2], y3, q);
       q = fma(r.pm[j][3], f34, q);
@@ -222,6 +224,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
       for (int i = 0; i < 5; ++i) r.pm[j][i] = valid ? 64.0 * __ldg(cb + CB_PM + i) : 0.0;     // quarter turns -> 1/256 turn (exact)
       r.yA[j] = valid ? __ldg(cb + CB_PM + 6) : 0.0;
       r.yB[j] = valid ? -__ldg(cb + CB_PM + 5) * r.yA[j] : 0.0;
+      r.dy[j] = r.yA[j] * df;                                                                   // y(f + df) - y(f)
       r.am[j][0] = valid ? __ldg(cb + CB_AM) : 0.0;
       g1[j] = valid ? __ldg(cb + CB_AM + 1) : 0.0;
       r.am[j][2] = valid ? __ldg(cb + CB_AM + 2) : 1.0;
