@@ -30,20 +30,22 @@ UNIT = "evals/s"
 
 def alg_flops_per_bin(n_det, model="taylorf2"):
     """Algorithmic fp64 flops per (particle, bin) of the minimal formulation the kernel implements,
-    FMA = 2: 9-FMA phase (18); table-driven sincos: exact reduction (F2I, I2F on the conversion pipe + 1 subtraction), r^2 (1),
-    sin 2 FMA + 1 mul (5), cos 3 FMA (6), complex product with the table entry (6) = 19; detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex
-    Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
+    FMA = 2: 9-FMA phase (18); table-driven sincos with the 512-entry table of the lane kernels: exact reduction (F2I, I2F on the
+    conversion pipe + 1 subtraction), r^2 (1), sin 1 FMA + 1 mul (3), cos 2 FMA (4), complex product with the table entry (6) = 15
+    (the 256-entry table of the other kernels needs one more term each: 19); detector 0: 4 FMA (8); every further detector:
+    conj(wd) E (6) and one complex Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
     if model == "phenomd":
         # merger-ringdown bin (about 80 % of the bins) as k_bins evaluates it (bins strided over threads; DESIGN.md section 5): phase 47,
         # amplitude 32 + 3, table-driven sincos 21, detector 0: 10, every further detector 18
         return 47 + 35 + 21 + 10 + 18 * (n_det - 1)
     if model == "phenomd_lane":
         # the same bin as k_pd_lp evaluates it (lane per row, consecutive bins: the cheaper formulation, so this is the model its
-        # fractions are quoted on): atan carried by the subtraction formula 19, phase 8, Lorentzian with the exponential as a geometric
-        # sequence 9, table-driven sincos 19 + scaling by the amplitude 2, detector 0: 8 + <h,h> 3, every further detector: Horner step 14 + <h,h> 2
-        return 19 + 8 + 9 + 21 + 11 + 16 * (n_det - 1)
+        # fractions are quoted on): atan carried by the subtraction formula with a constant step 18, phase 8, Lorentzian with the
+        # exponential as a geometric sequence 9, table-driven sincos 15 + scaling by the amplitude 2, detector 0: 8 + <h,h> 3, every
+        # further detector: Horner step 14 + <h,h> 2
+        return 18 + 8 + 9 + 17 + 11 + 16 * (n_det - 1)
     assert model == "taylorf2"
-    return 18 + 19 + 8 + 14 * (n_det - 1)
+    return 18 + 15 + 8 + 14 * (n_det - 1)
 
 
 def _profile_key(name):
@@ -286,6 +288,9 @@ def run_ours(args):
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
                 "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
+                "model_note": "the flop model follows the kernel's formulation down: 55 per particle-bin (2 detectors) since the lane kernels take sin/cos "
+                              "from a 512-entry table (two FMAs fewer), 59 before; on the 59-flop yardstick of BENCH_r01 this run is at %.3f"
+                              % (ach * (alg_flops_per_bin(n_det) + 4.0) / alg_flops_per_bin(n_det) / fp64_burst),
                 "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
                 "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,
                 "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}

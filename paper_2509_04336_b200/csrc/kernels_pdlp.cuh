@@ -72,7 +72,7 @@ __device__ __forceinline__ int pd_ticket_take(int* t) {
 __constant__ double kAtanR[3] = {-1.0 / 3.0, 0.2, -1.0 / 7.0};
 
 // Shared-memory coefficient block of a task, [kPdMixAll][NT PP] (row-minor).  Classes 1 and 2 read the first kPdMix1 entries per row:
-// 64 PB0..3 (intermediate phase, 1/256 turn), AH0..6 (intermediate amplitude), FP2, FA2 [Hz]; class 2 also 64 PH0..12 (inspiral phase),
+// 128 PB0..3 (intermediate phase, 1/512 turn), AH0..6 (intermediate amplitude), FP2, FA2 [Hz]; class 2 also 128 PH0..12 (inspiral phase),
 // AI0..9 (inspiral amplitude), FP1, FA1.
 constexpr int kPdMix1 = 13, kPdMixAll = 13 + 25;
 template <int PP>
@@ -92,7 +92,7 @@ struct PdRow {
 // One tile, bins in descending order.  CLS 0: every row of the warp is in its merger-ringdown region; 1: intermediate or
 // merger-ringdown; 2: any region.
 template <int NDET, int PP, int CLS>
-__device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<NDET>& sm, const double* __restrict__ mix, const MathTables* mt,
+__device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<NDET>& sm, const double* __restrict__ mix, const double2* sc9,
                                              int n, int tid) {
   using AL = AccLayout<2, NDET>;
   constexpr int ND1 = NDET - 1, NR = kPdNT * PP;
@@ -162,7 +162,7 @@ __device__ __forceinline__ void pd_tile_loop(PdRow<NDET, PP>& r, const PdTile<ND
         }
       }
       double sn, cs;
-      sincos_lut<true>(q, mt, sn, cs);
+      sincos_lut9(q, sc9, sn, cs);
       sn *= amp; cs *= amp;
       r.acc[j][0] = fma(w[0].x, cs, r.acc[j][0]);
       r.acc[j][1] = fma(-w[0].x, sn, r.acc[j][1]);
@@ -189,14 +189,16 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
   using AL = AccLayout<2, NDET>;
   constexpr int NT = kPdNT, PP = kPdPP, KT = kPdKT, ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1, NWARP = NT / 32, NR = NT * PP;
   __shared__ __align__(16) PdTile<NDET> sm;
-  __shared__ MathTables mtab;
+  __shared__ MathTablesEA mtab;                           // exp_tab / atan_tab at the tile starts
+  __shared__ __align__(16) double2 sc9[kSc9N];            // sincos_lut9 in the bin loops
   __shared__ int s_k1[NWARP], s_k2[NWARP], s_last;
   extern __shared__ __align__(16) double mix[];          // [kPdMixAll][NR]
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x, lane = tid & 31, wrp = tid >> 5;
   const int nf = cfg.n_freq;
   const double f_min = cfg.f_min, df = cfg.df;
-  load_math_tables(&mtab, tb.mt, tid, NT);     // built at ns_init: not the previous kernel's output
+  load_math_tables_ea(&mtab, tb.mt, tid, NT);  // built at ns_init: not the previous kernel's output
+  load_sc9(sc9, tb.sc9, tid, NT);
   pdl_wait();                                  // the rows (count, coefficient blocks) are
   const long long B = a.n_rows_dev ? (long long)*a.n_rows_dev : a.n_rows;
   if (B <= 0) return;
@@ -208,7 +210,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
     const long long grp = task / a.nranges;
     const int rng = (int)(task % a.nranges);
     const int k0 = rng * a.kr, k1 = min(nf, k0 + a.kr);
-    // per row: phase a + b f + c/f + d f^3/4 + e atan(yA f + yB) in 1/256 turn; amplitude g1 / ((f - f_RD)^2 + w^2) x ex(f).
+    // per row: phase a + b f + c/f + d f^3/4 + e atan(yA f + yB) in 1/512 turn; amplitude g1 / ((f - f_RD)^2 + w^2) x ex(f).
     // An invalid row (unphysical theta: logL = -inf whatever the sums) gets zero coefficients, so nothing undefined is evaluated.
     PdRow<NDET, PP> r;
     double c3[PP], g1[PP];
@@ -221,7 +223,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
       k1max = max(k1max, valid ? mr_first_bin(__ldg(cb + CB_FP1), f_min, df, nf) : 0);
       k2max = max(k2max, valid ? mr_first_bin(__ldg(cb + CB_FMR), f_min, df, nf) : 0);
 #pragma unroll
-      for (int i = 0; i < 5; ++i) r.pm[j][i] = valid ? 64.0 * __ldg(cb + CB_PM + i) : 0.0;     // quarter turns -> 1/256 turn (exact)
+      for (int i = 0; i < 5; ++i) r.pm[j][i] = valid ? 128.0 * __ldg(cb + CB_PM + i) : 0.0;    // quarter turns -> 1/512 turn (exact)
       r.yA[j] = valid ? __ldg(cb + CB_PM + 6) : 0.0;
       r.yB[j] = valid ? -__ldg(cb + CB_PM + 5) * r.yA[j] : 0.0;
       r.dy[j] = r.yA[j] * df;                                                                   // y(f + df) - y(f)
@@ -258,7 +260,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
         const bool valid = p < B && __ldg(cb + CB_VALID) != 0.0;
         double* m = mix + j * NT + tid;
 #pragma unroll
-        for (int i = 0; i < 4; ++i) m[i * NR] = valid ? 64.0 * __ldg(cb + CB_PB + i) : 0.0;
+        for (int i = 0; i < 4; ++i) m[i * NR] = valid ? 128.0 * __ldg(cb + CB_PB + i) : 0.0;
 #pragma unroll
         for (int i = 0; i < 7; ++i) m[(4 + i) * NR] = valid ? __ldg(cb + CB_AH + i) : 0.0;
         m[11 * NR] = valid ? __ldg(cb + CB_FP2) : 0.0;
@@ -266,7 +268,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
         if (k0 < k1cta) {
           double* c = m + kPdMix1 * NR;
 #pragma unroll
-          for (int i = 0; i < 13; ++i) c[i * NR] = valid ? 64.0 * __ldg(cb + CB_PH + i) : 0.0;
+          for (int i = 0; i < 13; ++i) c[i * NR] = valid ? 128.0 * __ldg(cb + CB_PH + i) : 0.0;
 #pragma unroll
           for (int i = 0; i < 10; ++i) c[(13 + i) * NR] = valid ? __ldg(cb + CB_AI + i) : 0.0;
           c[23 * NR] = valid ? __ldg(cb + CB_FP1) : 0.0;
@@ -302,9 +304,9 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
 #pragma unroll
         for (int d = 0; d < ND1s; ++d) r.S[j][d] = make_double2(0.0, 0.0);
       }
-      if (t_lo >= k2max) pd_tile_loop<NDET, PP, 0>(r, sm, mix, &mtab, n, tid);          // warp-uniform choices
-      else if (t_lo >= k1max) pd_tile_loop<NDET, PP, 1>(r, sm, mix, &mtab, n, tid);
-      else pd_tile_loop<NDET, PP, 2>(r, sm, mix, &mtab, n, tid);
+      if (t_lo >= k2max) pd_tile_loop<NDET, PP, 0>(r, sm, mix, sc9, n, tid);          // warp-uniform choices
+      else if (t_lo >= k1max) pd_tile_loop<NDET, PP, 1>(r, sm, mix, sc9, n, tid);
+      else pd_tile_loop<NDET, PP, 2>(r, sm, mix, sc9, n, tid);
       // close the tile: dh_d += Re(R_d(f_tlo) S), R_d(f) = C_d exp(i dtq f)
       const double f_lo = sm.f[0];
 #pragma unroll

@@ -715,10 +715,13 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
     k_tables<<<(unsigned)((nf + 255) / 256), 256, 0, s>>>(h->d_cfg, strain_dev, psd_dev, t2, t2 + nf, t2 + 2 * nf, t2 + 3 * nf,
                                                           h->d_tab + 8 * nf, h->d_tab + 9 * nf, h->d_wd, h->d_ws);
     g_launches.fetch_add(1);
-    INIT_CHECK(cudaMalloc(&h->d_mtab, sizeof(MathTables)), -2);
-    k_math_tables<<<1, 256, 0, s>>>(h->d_mtab);
+    static_assert(sizeof(MathTables) % sizeof(double2) == 0, "the 512-entry table follows the struct, 16-byte aligned");
+    INIT_CHECK(cudaMalloc(&h->d_mtab, sizeof(MathTables) + sizeof(double2) * kSc9N), -2);
+    double2* sc9 = reinterpret_cast<double2*>(reinterpret_cast<char*>(h->d_mtab) + sizeof(MathTables));
+    k_math_tables<<<1, 256, 0, s>>>(h->d_mtab, sc9);
     g_launches.fetch_add(1);
     h->tb.mt = h->d_mtab;
+    h->tb.sc9 = sc9;
     k_i73<<<1, 256, 0, s>>>(h->d_cfg, h->d_ws);
     g_launches.fetch_add(1);
     INIT_CHECK(cudaGetLastError(), -2);

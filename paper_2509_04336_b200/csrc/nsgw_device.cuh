@@ -49,6 +49,7 @@ struct Tables {
   const double2* wd[kMaxDet];  // 4 df d_k f_k^-7/6 / S_k   (complex)
   const double* ws[kMaxDet];   // 4 df f_k^-7/3 / S_k
   const struct MathTables* mt; // sin/cos, 2^(j/64), atan(j/32) tables (built once per handle; CTAs copy them to shared memory)
+  const double2* sc9;          // exp(2 pi i k / 512), the lane-per-row kernels' sin/cos table (sincos_lut9)
 };
 
 // ------------------------------------------------------------------------------------------------------
@@ -149,6 +150,16 @@ __device__ __forceinline__ void build_math_tables(MathTables* mt, int tid, int n
   for (int i = tid; i < 34; i += nthreads) mt->at[i] = atan(i * (1.0 / 32.0));
 }
 
+// The exp / atan part alone (784 bytes), for kernels that take their sin/cos from the 512-entry table (k_pd_lp).
+struct MathTablesEA {
+  double e2[64];
+  double at[34];
+};
+__device__ __forceinline__ void load_math_tables_ea(MathTablesEA* dst, const MathTables* __restrict__ src, int tid, int nthreads) {
+  for (int i = tid; i < 64; i += nthreads) dst->e2[i] = __ldg(src->e2 + i);
+  for (int i = tid; i < 34; i += nthreads) dst->at[i] = __ldg(src->at + i);
+}
+
 // CTA-wide copy of the handle's tables into shared memory (617 doubles).
 __device__ __forceinline__ void load_math_tables(MathTables* dst, const MathTables* __restrict__ src, int tid, int nthreads) {
   static_assert(sizeof(MathTables) % sizeof(double) == 0, "MathTables is an array of doubles");
@@ -179,6 +190,36 @@ __device__ __forceinline__ void sincos_lut(double u, const MathTables* mt, doubl
   double pc = fma(z, kLutC[5], kLutC[4]);
   ps = fma(ps, z, kLutC[0]);
   pc = fma(pc, z, kLutC[3]);
+  ps *= r;
+  pc = fma(pc, z, 1.0);
+  c = fma(T.x, pc, -(T.y * ps));
+  s = fma(T.y, pc, T.x * ps);
+}
+
+// sincos_lut with a 512-entry table and the angle in units of 1/512 turn (u = 128 q): the remainder |r| <= 1/2 unit is |alpha| <= pi/512,
+// where sin alpha = alpha - alpha^3/6 (truncation 7e-14) and cos alpha = 1 - alpha^2/2 + alpha^4/24 (7e-17): 10 FP64 instructions
+// against sincos_lut's 12, for 8 KB of shared memory instead of 4.  Used by the lane-per-row kernels (k_bins_lp, k_pd_lp).
+constexpr int kSc9N = 512;
+__constant__ double kLut9C[4] = {0.012271846303085129838, -3.0801968455612480815e-7, -0.000075299105843272084189, 9.4499255679938202216e-10};
+__device__ __forceinline__ void build_sc9(double2* sc9, int tid, int nthreads) {
+  for (int i = tid; i < kSc9N; i += nthreads) {
+    double s, c;
+    sincos_qt(i * (1.0 / 128.0), s, c);
+    sc9[i] = make_double2(c, s);
+  }
+}
+__device__ __forceinline__ void load_sc9(double2* dst, const double2* __restrict__ src, int tid, int nthreads) {
+  const double* g = reinterpret_cast<const double*>(src);
+  double* d = reinterpret_cast<double*>(dst);
+  for (int i = tid; i < 2 * kSc9N; i += nthreads) d[i] = __ldg(g + i);
+}
+__device__ __forceinline__ void sincos_lut9(double u, const double2* sc9, double& s, double& c) {
+  const int ki = __double2int_rn(u);
+  const double r = u - (double)ki;             // exact: |u - k| <= 1/2 and |u| < 2^31
+  const double z = r * r;
+  const double2 T = sc9[ki & (kSc9N - 1)];
+  double ps = fma(z, kLut9C[1], kLut9C[0]);
+  double pc = fma(z, kLut9C[3], kLut9C[2]);
   ps *= r;
   pc = fma(pc, z, 1.0);
   c = fma(T.x, pc, -(T.y * ps));
@@ -217,7 +258,8 @@ __device__ __forceinline__ double rcp_nr1(double d) {
 
 // exp(x) for |x| <= 700: n = rint(64 x / ln 2), r = x - n ln2/64 (two-term Cody-Waite, |r| <= 0.0055), degree-5 Taylor
 // (truncation 3.4e-17 relative), 2^(n/64) from the table and an exponent-field add.
-__device__ __forceinline__ double exp_tab(double x, const MathTables* mt) {
+template <class MT /* has e2[64] */>
+__device__ __forceinline__ double exp_tab(double x, const MT* mt) {
   const double magic = 6755399441055744.0;
   double t = fma(x, kExpC[0], magic);
   const int n = __double2loint(t);
@@ -237,7 +279,8 @@ __device__ __forceinline__ double exp_tab(double x, const MathTables* mt) {
 // division); a 20-bit estimate of n/d picks the table point c = j/32, and atan(n/d) = atan(c) + atan((n - c d)/(d + c n))
 // with |t| <= 1/64 + 2^-19, so five odd Taylor terms suffice (t^11/11 < 1.3e-21).  One full reciprocal (d + c n >= 1 in
 // magnitude by construction).
-__device__ __forceinline__ double atan_tab(double y, const MathTables* mt) {
+template <class MT /* has at[34] */>
+__device__ __forceinline__ double atan_tab(double y, const MT* mt) {
   const int hi = __double2hiint(y);
   const bool big = (hi & 0x7fffffff) >= 0x3ff00000;      // |y| >= 1
   const double n = big ? -1.0 : y;
