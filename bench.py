@@ -30,10 +30,11 @@ UNIT = "evals/s"
 
 def alg_flops_per_bin(n_det, model="taylorf2"):
     """Algorithmic fp64 flops per (particle, bin) of the minimal formulation the kernel implements,
-    FMA = 2: 9-FMA phase (18); table-driven sincos with the 512-entry table of the lane kernels: exact reduction (F2I, I2F on the
-    conversion pipe + 1 subtraction), r^2 (1), sin 1 FMA + 1 mul (3), cos 2 FMA (4), complex product with the table entry (6) = 15
-    (the 256-entry table of the other kernels needs one more term each: 19); detector 0: 4 FMA (8); every further detector:
-    conj(wd) E (6) and one complex Horner step in the detector's per-bin phasor (4 FMA = 8) = 14."""
+    FMA = 2: 9-FMA phase (18); table-driven sincos with k_bins_lp's 2048-entry table: exact reduction (F2I, I2F on the
+    conversion pipe + 1 subtraction), r^2 (1), sin 1 FMA + 1 mul (3), cos 1 FMA (2), complex product with the table entry (6) = 13
+    (k_pd_lp's 512-entry table needs one more cos term: 15; the 256-entry table of the other kernels one more each: 19);
+    detector 0: 4 FMA (8); every further detector: conj(wd) E (6) and one complex Horner step in the detector's per-bin
+    phasor (4 FMA = 8) = 14."""
     if model == "phenomd":
         # merger-ringdown bin (about 80 % of the bins) as k_bins evaluates it (bins strided over threads; DESIGN.md section 5): phase 47,
         # amplitude 32 + 3, table-driven sincos 21, detector 0: 10, every further detector 18
@@ -45,7 +46,7 @@ def alg_flops_per_bin(n_det, model="taylorf2"):
         # further detector: Horner step 14 + <h,h> 2
         return 18 + 8 + 9 + 17 + 11 + 16 * (n_det - 1)
     assert model == "taylorf2"
-    return 18 + 15 + 8 + 14 * (n_det - 1)
+    return 18 + 13 + 8 + 14 * (n_det - 1)
 
 
 def _profile_key(name):
@@ -286,11 +287,11 @@ def run_ours(args):
         # `ncu --set full` capture of this same command (profiles/r01ad_k_bins_lp_ncu_full.txt); only valid for the default batch
         traffic, traffic_file = traffic_from_profile("k_bins_lp") if (B == 65536 and n_freq == 4017) else (None, None)
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
-                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, 128 thr x 2 particles, 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, one CTA of 384 thr x 2 particles per SM from 6144 rows, three of 128 below; 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
-                "model_note": "the flop model follows the kernel's formulation down: 55 per particle-bin (2 detectors) since the lane kernels take sin/cos "
-                              "from a 512-entry table (two FMAs fewer), 59 before; on the 59-flop yardstick of BENCH_r01 this run is at %.3f"
-                              % (ach * (alg_flops_per_bin(n_det) + 4.0) / alg_flops_per_bin(n_det) / fp64_burst),
+                "model_note": "the flop model follows the kernel's formulation down: 53 per particle-bin (2 detectors) since k_bins_lp takes sin/cos "
+                              "from a 2048-entry table (three FMAs fewer), 59 before; on the 59-flop yardstick of BENCH_r01 this run is at %.3f"
+                              % (ach * (alg_flops_per_bin(n_det) + 6.0) / alg_flops_per_bin(n_det) / fp64_burst),
                 "peak_source": "measured here: nsgw_measure_fp64_peak (8 independent DFMA chains/thread, 8 CTAs x 256 thr per SM), burst",
                 "frac_of_nominal_37.2": ach / NOMINAL_FP64_TFLOPS,
                 "hbm_peak_gbs_measured": peaks.get("hbm_gbs")}

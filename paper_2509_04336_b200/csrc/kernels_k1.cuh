@@ -28,9 +28,10 @@ __global__ void k_tables(DevCfg* cfg, const double* __restrict__ strain, const d
   }
 }
 
-__global__ void k_math_tables(MathTables* mt, double2* sc9) {
+__global__ void k_math_tables(MathTables* mt, double2* sc9, double2* sc11) {
   build_math_tables(mt, threadIdx.x, blockDim.x);
   build_sc9(sc9, threadIdx.x, blockDim.x);
+  build_sc11(sc11, threadIdx.x, blockDim.x);
 }
 
 // I_{7/3} per detector: deterministic single-CTA tree sum.
@@ -387,6 +388,9 @@ struct LpSmem {
   double f[KR];
 };
 
+constexpr double kLpLutScale = 512.0;                          // quarter turns -> 1/2048 turn
+constexpr size_t kLpDynSmem = sizeof(double2) * kSc11N;        // the sin/cos table (32 KB)
+
 template <int NDET, int NT, int KR, int PP, int UNR, int OCC>
 __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ cfgp, Tables tb, const double* __restrict__ cbs_g,
                                                      long long B_host, const int* __restrict__ B_dev /*overrides the row count; B_host
@@ -398,11 +402,11 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
   if (blockIdx.x >= ntasks) return;
   constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) LpSmem<NDET, KR> sm;
-  __shared__ __align__(16) double2 sc9[kSc9N];
+  extern __shared__ __align__(16) double2 sc11[];          // kSc11N entries (dynamic: with the tile it is past the 48 KB static limit)
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x;
   const int nf = cfg.n_freq;
-  load_sc9(sc9, tb.sc9, tid, NT);
+  for (int i = tid; i < 2 * kSc11N; i += NT) reinterpret_cast<double*>(sc11)[i] = __ldg(reinterpret_cast<const double*>(tb.sc11) + i);
   for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
     const long long grp = task / nranges;
     const int rng = (int)(task % nranges);
@@ -428,7 +432,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       const bool have = p < B;
       const double* cb = cbs_g + (have ? p : 0) * CB_SIZE;
 #pragma unroll
-      for (int i = 0; i < 10; ++i) a[j][i] = have ? 128.0 * __ldg(cb + CB_PH + i) : 0.0;   // quarter turns -> 1/512 turn (exact)
+      for (int i = 0; i < 10; ++i) a[j][i] = have ? kLpLutScale * __ldg(cb + CB_PH + i) : 0.0;   // quarter turns -> table units (exact)
 #pragma unroll
       for (int d = 0; d < ND1; ++d) {
         const double cr = have ? __ldg(cb + CB_DET + 4 * (d + 1)) : 0.0, ci = have ? __ldg(cb + CB_DET + 4 * (d + 1) + 1) : 0.0;
@@ -466,7 +470,7 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
       for (int j = 0; j < PP; ++j) {
         const double q = phase_pn_qt(a[j], b);
         double sn, cs;
-        sincos_lut9(q, sc9, sn, cs);
+        sincos_lut11(q, sc11, sn, cs);
         acc[j][0] = fma(w[0].x, cs, acc[j][0]);
         acc[j][1] = fma(-w[0].x, sn, acc[j][1]);
         acc[j][0] = fma(-w[0].y, sn, acc[j][0]);

@@ -180,6 +180,11 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 #define NSGW_LP_OCC 3
 #endif
 constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
+// From kLpBigBatch rows on: ONE CTA of 384 threads per SM instead of three of 128 -- the SM then holds one copy of the 32 KB sin/cos
+// table instead of three and a tile serves 768 rows (measured, config 2: 0.1904 against 0.1980 ms at 16384 rows, 0.631 against 0.649 at
+// 65536; 0.0742 against 0.0684 at 4096, where 6 groups of 768 rows leave SMs idle; the crossover is at 6144).
+constexpr int kLpNTBig = 384, kLpOCCBig = 1;
+constexpr long long kLpBigBatch = 6144;
 constexpr long long kLpMinBatch = 1024;   // below this the CTA-per-particle kernel fills the machine better
 constexpr long long kPdMinBatch = 16384;  // PhenomD-form: from here k_pd_lp is faster than k_bins (measured: 35.9 vs 34.6 M evals/s at 16384, 44.5 vs 35.9 at 65536)
 
@@ -194,12 +199,12 @@ int ensure_partial(ns_handle* h, size_t n) {
 }
 
 // cbs [B][CB_SIZE]; rows_dev (optional, device) overrides the row count of the task lists (B is then the capacity).
-template <int NDET>
-int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
+template <int NDET, int NT, int OCC>
+int launch_bins_lp_g(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
   using AL = AccLayout<1, NDET>;
-  constexpr int NT = kLpNT, PP = kLpPP;
+  constexpr int PP = kLpPP;
   const long long ngroups = (B + NT * PP - 1) / (NT * PP);
-  const long long grid_max = (long long)h->n_sm * kLpOCC;
+  const long long grid_max = (long long)h->n_sm * OCC;
   // bins per task (multiple of the unroll, 32..256): the value that minimises rounds x (bins per task + per-task overhead) x
   // slow-down from sharing the SM, rounds = ceil(tasks / resident CTAs) -- large tiles amortise the per-task set-up, small ones
   // balance the last round; one CTA alone on an SM already runs at ~85 % of the FP64 pipe, so co-resident CTAs divide it
@@ -210,7 +215,7 @@ int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows
     for (int c = 32; c <= kLpKR; c += kLpUNR) {
       const int nr = (h->cfg.n_freq + c - 1) / c;
       const long long nt = ngroups * nr;
-      const long long per_sm = std::min<long long>(kLpOCC, (nt + h->n_sm - 1) / h->n_sm);
+      const long long per_sm = std::min<long long>(OCC, (nt + h->n_sm - 1) / h->n_sm);
       const double cost = (double)((nt + grid_max - 1) / grid_max) * (c + 8) * std::max(1.0, 0.85 * per_sm) + 0.25 * nr;
       if (cost < best - 1e-9) { best = cost; kr = c; }
     }
@@ -225,8 +230,9 @@ int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, cbs, B, rows_dev, kr, nranges, ntasks,
-                                                                              h->d_partial);
+  CU_CHECK(h, cudaFuncSetAttribute(k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, OCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem));
+  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, OCC><<<(unsigned)grid, NT, kLpDynSmem, s>>>(h->d_cfg, h->tb, cbs, B, rows_dev, kr, nranges, ntasks,
+                                                                                    h->d_partial);
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
   if (rows_dev) {
@@ -237,6 +243,12 @@ int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows
   }
   LAUNCH_CHECK(h);
   return 0;
+}
+// (B is the row capacity when rows_dev is given: the geometry, like the range length, is a function of the call, not of the round)
+template <int NDET>
+int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
+  if (B >= kLpBigBatch) return launch_bins_lp_g<NDET, kLpNTBig, kLpOCCBig>(h, cbs, B, rows_dev, logl, parts, s);
+  return launch_bins_lp_g<NDET, kLpNT, kLpOCC>(h, cbs, B, rows_dev, logl, parts, s);
 }
 
 // Launch with programmatic stream serialization: the kernel may become resident while the kernel before it on the stream still runs;
@@ -716,9 +728,10 @@ int ns_init(ns_handle** out, const ns_config* cfg, const double* live_u_dev, con
                                                           h->d_tab + 8 * nf, h->d_tab + 9 * nf, h->d_wd, h->d_ws);
     g_launches.fetch_add(1);
     static_assert(sizeof(MathTables) % sizeof(double2) == 0, "the 512-entry table follows the struct, 16-byte aligned");
-    INIT_CHECK(cudaMalloc(&h->d_mtab, sizeof(MathTables) + sizeof(double2) * kSc9N), -2);
+    INIT_CHECK(cudaMalloc(&h->d_mtab, sizeof(MathTables) + sizeof(double2) * (kSc9N + kSc11N)), -2);
     double2* sc9 = reinterpret_cast<double2*>(reinterpret_cast<char*>(h->d_mtab) + sizeof(MathTables));
-    k_math_tables<<<1, 256, 0, s>>>(h->d_mtab, sc9);
+    h->tb.sc11 = sc9 + kSc9N;
+    k_math_tables<<<1, 256, 0, s>>>(h->d_mtab, sc9, sc9 + kSc9N);
     g_launches.fetch_add(1);
     h->tb.mt = h->d_mtab;
     h->tb.sc9 = sc9;
@@ -1270,6 +1283,19 @@ int occ_of(K kern, int threads, size_t smem, long long grid, int n_sm, double* f
   if (ctas) *ctas = per_sm;
   return 0;
 }
+template <int NDET>
+int occ_lp(long long rows, int n_sm, double* frac, int32_t* ctas) {
+  if (rows >= kLpBigBatch) {
+    auto kern = k_bins_lp<NDET, kLpNTBig, kLpKR, kLpPP, kLpUNR, kLpOCCBig>;
+    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem);
+    const long long grid = std::min<long long>((rows + kLpNTBig * kLpPP - 1) / (kLpNTBig * kLpPP) * 16, (long long)n_sm * kLpOCCBig);
+    return occ_of(kern, kLpNTBig, kLpDynSmem, grid, n_sm, frac, ctas);
+  }
+  auto kern = k_bins_lp<NDET, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>;
+  cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem);
+  const long long grid = std::min<long long>((rows + kLpNT * kLpPP - 1) / (kLpNT * kLpPP) * 16, (long long)n_sm * kLpOCC);
+  return occ_of(kern, kLpNT, kLpDynSmem, grid, n_sm, frac, ctas);
+}
 }  // namespace
 
 extern "C" {
@@ -1280,10 +1306,9 @@ int nsgw_sweep_occupancy(ns_handle* h, int64_t rows, double* warps_active_host, 
   const int nd = h->cfg.n_det, n_sm = h->n_sm;
   const bool tf2 = h->cfg.like_kind == NSGW_LIKE_GW_TAYLORF2;
   if (tf2 && rows >= kLpMinBatch && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 12000))) {
-    const long long grid = std::min<long long>((rows + kLpNT * kLpPP - 1) / (kLpNT * kLpPP) * 16, (long long)n_sm * kLpOCC);
-    if (nd == 1) return occ_of(k_bins_lp<1, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
-    if (nd == 2) return occ_of(k_bins_lp<2, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
-    return occ_of(k_bins_lp<3, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>, kLpNT, 0, grid, n_sm, warps_active_host, ctas_per_sm_host);
+    if (nd == 1) return occ_lp<1>(rows, n_sm, warps_active_host, ctas_per_sm_host);
+    if (nd == 2) return occ_lp<2>(rows, n_sm, warps_active_host, ctas_per_sm_host);
+    return occ_lp<3>(rows, n_sm, warps_active_host, ctas_per_sm_host);
   }
   if (!tf2 && (h->opt_walk_kernel == 3 || (h->opt_walk_kernel == 0 && rows >= 12000))) {
     const int kr = h->wl_kr > 0 ? h->wl_kr : std::max(kPdKT, (h->cfg.n_freq / 32 + kPdKT - 1) / kPdKT * kPdKT);
@@ -1414,7 +1439,8 @@ int na_launch(ns_handle* h, const double* theta_dev, long long B, double* logl, 
     k_setup<1><<<gs, 128, 0, s>>>(h->d_cfg, theta_dev, B, cbs);
     LAUNCH_CHECK(h);
     // every (range, sum, row < B) entry of `partial` the finishing pass reads is written by this launch: nothing to clear
-    k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, 0, s>>>(h->d_cfg, h->tb, cbs, B, nullptr, kNaKr, nranges, ntasks, partial);
+    CU_CHECK(h, cudaFuncSetAttribute(k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem));
+    k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, kLpOCC><<<(unsigned)grid, NT, kLpDynSmem, s>>>(h->d_cfg, h->tb, cbs, B, nullptr, kNaKr, nranges, ntasks, partial);
     LAUNCH_CHECK(h);
     k_finish<1, NDET><<<gs, 128, 0, s>>>(h->d_cfg, cbs, partial, nranges, B, logl, nullptr);
     LAUNCH_CHECK(h);

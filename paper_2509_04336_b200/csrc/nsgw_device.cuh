@@ -50,6 +50,7 @@ struct Tables {
   const double* ws[kMaxDet];   // 4 df f_k^-7/3 / S_k
   const struct MathTables* mt; // sin/cos, 2^(j/64), atan(j/32) tables (built once per handle; CTAs copy them to shared memory)
   const double2* sc9;          // exp(2 pi i k / 512), the lane-per-row kernels' sin/cos table (sincos_lut9)
+  const double2* sc11;         // exp(2 pi i k / 2048) (sincos_lut11)
 };
 
 // ------------------------------------------------------------------------------------------------------
@@ -222,6 +223,28 @@ __device__ __forceinline__ void sincos_lut9(double u, const double2* sc9, double
   double pc = fma(z, kLut9C[3], kLut9C[2]);
   ps *= r;
   pc = fma(pc, z, 1.0);
+  c = fma(T.x, pc, -(T.y * ps));
+  s = fma(T.y, pc, T.x * ps);
+}
+
+// The same with 2048 entries and the angle in units of 1/2048 turn (u = 512 q): |alpha| <= pi/2048, sin alpha = alpha - alpha^3/6
+// (7e-17), cos alpha = 1 - alpha^2/2 (2.3e-13): 8 FP64 instructions, 32 KB of shared memory.
+constexpr int kSc11N = 2048;
+__constant__ double kLut11C[3] = {0.0030679615757712824594, -4.8128075711894501273e-9, -4.7061941152045052618e-6};
+__device__ __forceinline__ void build_sc11(double2* sc, int tid, int nthreads) {
+  for (int i = tid; i < kSc11N; i += nthreads) {
+    double s, c;
+    sincos_qt(i * (1.0 / 512.0), s, c);
+    sc[i] = make_double2(c, s);
+  }
+}
+__device__ __forceinline__ void sincos_lut11(double u, const double2* sc, double& s, double& c) {
+  const int ki = __double2int_rn(u);
+  const double r = u - (double)ki;
+  const double z = r * r;
+  const double2 T = sc[ki & (kSc11N - 1)];
+  const double ps = fma(z, kLut11C[1], kLut11C[0]) * r;
+  const double pc = fma(z, kLut11C[2], 1.0);
   c = fma(T.x, pc, -(T.y * ps));
   s = fma(T.y, pc, T.x * ps);
 }
