@@ -287,7 +287,7 @@ def run_ours(args):
         # `ncu --set full` capture of this same command (profiles/r01ad_k_bins_lp_ncu_full.txt); only valid for the default batch
         traffic, traffic_file = traffic_from_profile("k_bins_lp") if (B == 65536 and n_freq == 4017) else (None, None)
         roof = {"bound": "alu", "achieved": ach, "peak": fp64_burst, "unit": "TFLOP/s", "frac": ach / fp64_burst,
-                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, one CTA of 384 thr x 2 particles per SM from 6144 rows, three of 128 below; 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
+                "traffic": traffic, "traffic_unit": "bytes per launch (ncu dram read+write) from %s; algorithmic 96 B x B = %d" % (traffic_file, 96 * B), "kernel": "k_bins_lp<2det> (lane per particle, one CTA of 512 threads x 2 particles per SM from 6144 rows, three of 128 below; 256-bin tiles)", "kernel_ms": kern_ms / kern_n,
                 "flops_per_particle_bin": alg_flops_per_bin(n_det),
                 "model_note": "the flop model follows the kernel's formulation down: 53 per particle-bin (2 detectors) since k_bins_lp takes sin/cos "
                               "from a 2048-entry table (three FMAs fewer), 59 before; on the 59-flop yardstick of BENCH_r01 this run is at %.3f"

@@ -176,14 +176,19 @@ int pick_p(long long B) { return B >= 4096 ? 2 : 1; }
 #ifndef NSGW_LP_NT
 #define NSGW_LP_NT 128
 #define NSGW_LP_PP 2
-#define NSGW_LP_UNR 4
+#define NSGW_LP_UNR 2
 #define NSGW_LP_OCC 3
 #endif
 constexpr int kLpNT = NSGW_LP_NT, kLpKR = 256, kLpPP = NSGW_LP_PP, kLpUNR = NSGW_LP_UNR, kLpOCC = NSGW_LP_OCC;
-// From kLpBigBatch rows on: ONE CTA of 384 threads per SM instead of three of 128 -- the SM then holds one copy of the 32 KB sin/cos
-// table instead of three and a tile serves 768 rows (measured, config 2: 0.1904 against 0.1980 ms at 16384 rows, 0.631 against 0.649 at
-// 65536; 0.0742 against 0.0684 at 4096, where 6 groups of 768 rows leave SMs idle; the crossover is at 6144).
-constexpr int kLpNTBig = 384, kLpOCCBig = 1;
+// From kLpBigBatch rows on: ONE CTA of 512 threads per SM instead of three of 128 -- the SM then holds one copy of the 32 KB sin/cos
+// table instead of three, a tile serves 1024 rows, and at 124 registers 16 warps are resident instead of 12 (measured, config 2, kernel
+// time at 65536 rows: 3 x 128 threads 0.649 ms, 1 x 384 0.631, 1 x 512 0.621, with the loop unrolled by 2 instead of 4 0.616; 448 or 416
+// threads -- warps not a multiple of the four sub-partitions -- 0.69 / 0.76; 640 / 768 threads spill: 0.66 / 0.72; 2 x 256 0.630).
+#ifndef NSGW_LP_NT_BIG
+#define NSGW_LP_NT_BIG 512
+#define NSGW_LP_OCC_BIG 1
+#endif
+constexpr int kLpNTBig = NSGW_LP_NT_BIG, kLpOCCBig = NSGW_LP_OCC_BIG;
 constexpr long long kLpBigBatch = 6144;
 constexpr long long kLpMinBatch = 1024;   // below this the CTA-per-particle kernel fills the machine better
 constexpr long long kPdMinBatch = 16384;  // PhenomD-form: from here k_pd_lp is faster than k_bins (measured: 35.9 vs 34.6 M evals/s at 16384, 44.5 vs 35.9 at 65536)
