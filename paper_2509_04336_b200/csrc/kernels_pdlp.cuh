@@ -30,7 +30,10 @@
 #ifndef NSGW_PD_KT
 #define NSGW_PD_KT 128
 #endif
-constexpr int kPdNT = 128;            // threads per CTA
+#ifndef NSGW_PD_NT
+#define NSGW_PD_NT 128
+#endif
+constexpr int kPdNT = NSGW_PD_NT;     // threads per CTA
 constexpr int kPdPP = NSGW_PD_PP;     // rows per thread
 constexpr int kPdKT = NSGW_PD_KT;     // bins per shared-memory tile
 constexpr int kPdOCC = NSGW_PD_OCC;   // CTAs per SM

@@ -249,10 +249,11 @@ int launch_bins_lp_g(ns_handle* h, const double* cbs, long long B, const int* ro
   LAUNCH_CHECK(h);
   return 0;
 }
-// (B is the row capacity when rows_dev is given: the geometry, like the range length, is a function of the call, not of the round)
+// (with rows_dev, B is the row CAPACITY of a round of the worklist walk and the rows are several times fewer: the small geometry's
+// finer tasks -- measured on `extras.walk`, 16384 walkers: 27.2 against 22.2 M evaluations/s)
 template <int NDET>
 int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
-  if (B >= kLpBigBatch) return launch_bins_lp_g<NDET, kLpNTBig, kLpOCCBig>(h, cbs, B, rows_dev, logl, parts, s);
+  if (B >= kLpBigBatch && !rows_dev) return launch_bins_lp_g<NDET, kLpNTBig, kLpOCCBig>(h, cbs, B, rows_dev, logl, parts, s);
   return launch_bins_lp_g<NDET, kLpNT, kLpOCC>(h, cbs, B, rows_dev, logl, parts, s);
 }
 
@@ -1289,13 +1290,7 @@ int occ_of(K kern, int threads, size_t smem, long long grid, int n_sm, double* f
   return 0;
 }
 template <int NDET>
-int occ_lp(long long rows, int n_sm, double* frac, int32_t* ctas) {
-  if (rows >= kLpBigBatch) {
-    auto kern = k_bins_lp<NDET, kLpNTBig, kLpKR, kLpPP, kLpUNR, kLpOCCBig>;
-    cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem);
-    const long long grid = std::min<long long>((rows + kLpNTBig * kLpPP - 1) / (kLpNTBig * kLpPP) * 16, (long long)n_sm * kLpOCCBig);
-    return occ_of(kern, kLpNTBig, kLpDynSmem, grid, n_sm, frac, ctas);
-  }
+int occ_lp(long long rows, int n_sm, double* frac, int32_t* ctas) {   // the walk's rounds are swept with the small geometry
   auto kern = k_bins_lp<NDET, kLpNT, kLpKR, kLpPP, kLpUNR, kLpOCC>;
   cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem);
   const long long grid = std::min<long long>((rows + kLpNT * kLpPP - 1) / (kLpNT * kLpPP) * 16, (long long)n_sm * kLpOCC);
