@@ -397,16 +397,19 @@ __global__ void __launch_bounds__(NT, OCC) k_bins_lp(const DevCfg* __restrict__ 
                                                      stays the stride of `partial`*/, int kr /*bins per range, <= KR, multiple of UNR*/,
                                                      int nranges, long long ntasks_host, double* __restrict__ partial) {
   using AL = AccLayout<1, NDET>;
-  const long long B = B_dev ? (long long)*B_dev : B_host;
-  const long long ntasks = B_dev ? (B + NT * PP - 1) / (NT * PP) * nranges : ntasks_host;
-  if (blockIdx.x >= ntasks) return;
   constexpr int ND1 = NDET - 1, ND1s = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) LpSmem<NDET, KR> sm;
   extern __shared__ __align__(16) double2 sc11[];          // kSc11N entries (dynamic: with the tile it is past the 48 KB static limit)
   const DevCfg& cfg = *cfgp;
   const int tid = threadIdx.x;
   const int nf = cfg.n_freq;
+  // the table is the handle's (ns_init): its copy runs under the tail of the kernel before this one (k_setup, k_wl_head) when the launch is a
+  // programmatic dependent one; the coefficient blocks and the row count are that kernel's output
   for (int i = tid; i < 2 * kSc11N; i += NT) reinterpret_cast<double*>(sc11)[i] = __ldg(reinterpret_cast<const double*>(tb.sc11) + i);
+  pdl_wait();
+  const long long B = B_dev ? (long long)*B_dev : B_host;
+  const long long ntasks = B_dev ? (B + NT * PP - 1) / (NT * PP) * nranges : ntasks_host;
+  if (blockIdx.x >= ntasks) return;
   for (long long task = blockIdx.x; task < ntasks; task += gridDim.x) {
     const long long grp = task / nranges;
     const int rng = (int)(task % nranges);
@@ -505,6 +508,7 @@ template <int MODEL, int NDET>
 __global__ void k_finish(const DevCfg* __restrict__ cfgp, const double* __restrict__ cbs_g, const double* __restrict__ partial, int nchunks,
                          long long B, double* logl, double* parts) {
   using AL = AccLayout<MODEL, NDET>;
+  pdl_wait();   // (launched as a programmatic dependent of the sweep)
   long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (p >= B) return;
   double sums[AL::N];

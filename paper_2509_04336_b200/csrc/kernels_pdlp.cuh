@@ -363,6 +363,7 @@ __global__ void __launch_bounds__(kPdNT, kPdOCC) k_pd_lp(const DevCfg* __restric
 template <int MODEL, int NDET>
 __global__ void k_finish_rows(const DevCfg* __restrict__ cfgp, const double* __restrict__ cbs_g, const double* __restrict__ partial, int nslots,
                               long long n_rows, const int* __restrict__ n_rows_dev, long long stride, double* logl, double* parts) {
+  pdl_wait();   // (launched as a programmatic dependent of the sweep)
   using AL = AccLayout<MODEL, NDET>;
   const long long B = n_rows_dev ? (long long)*n_rows_dev : n_rows;
   for (long long p = blockIdx.x * (long long)blockDim.x + threadIdx.x; p < B; p += (long long)gridDim.x * blockDim.x) {

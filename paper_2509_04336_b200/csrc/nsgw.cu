@@ -203,6 +203,19 @@ int ensure_partial(ns_handle* h, size_t n) {
   return 0;
 }
 
+// Launch with programmatic stream serialization: the kernel may become resident while the kernel before it on the stream still runs;
+// it calls pdl_wait() before it reads what that kernel wrote.
+template <class... KArgs, class... Args>
+cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s, Args... args) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(grid); lc.blockDim = dim3(block); lc.dynamicSmemBytes = smem; lc.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  return cudaLaunchKernelEx(&lc, kern, KArgs(args)...);
+}
+
 // cbs [B][CB_SIZE]; rows_dev (optional, device) overrides the row count of the task lists (B is then the capacity).
 template <int NDET, int NT, int OCC>
 int launch_bins_lp_g(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
@@ -236,15 +249,18 @@ int launch_bins_lp_g(ns_handle* h, const double* cbs, long long B, const int* ro
     cudaEventRecord(e0, s);
   }
   CU_CHECK(h, cudaFuncSetAttribute(k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, OCC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kLpDynSmem));
-  k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, OCC><<<(unsigned)grid, NT, kLpDynSmem, s>>>(h->d_cfg, h->tb, cbs, B, rows_dev, kr, nranges, ntasks,
-                                                                                    h->d_partial);
+  // programmatic dependent launches: the sweep behind k_setup / k_wl_head (its table copy runs under their tail), the finish behind the sweep
+  CU_CHECK(h, launch_pdl(k_bins_lp<NDET, NT, kLpKR, PP, kLpUNR, OCC>, (unsigned)grid, NT, kLpDynSmem, s, (const DevCfg*)h->d_cfg, h->tb, cbs,
+                         (long long)B, rows_dev, kr, nranges, (long long)ntasks, h->d_partial));
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
   if (rows_dev) {
     const long long gfin = std::min<long long>((B + 127) / 128, (long long)h->n_sm * 8);
-    k_finish_rows<1, NDET><<<(unsigned)gfin, 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges, B, rows_dev, B, logl, parts);
+    CU_CHECK(h, launch_pdl(k_finish_rows<1, NDET>, (unsigned)gfin, 128, 0, s, (const DevCfg*)h->d_cfg, cbs, (const double*)h->d_partial, nranges,
+                           (long long)B, rows_dev, (long long)B, logl, parts));
   } else {
-    k_finish<1, NDET><<<(unsigned)((B + 127) / 128), 128, 0, s>>>(h->d_cfg, cbs, h->d_partial, nranges, B, logl, parts);
+    CU_CHECK(h, launch_pdl(k_finish<1, NDET>, (unsigned)((B + 127) / 128), 128, 0, s, (const DevCfg*)h->d_cfg, cbs, (const double*)h->d_partial,
+                           nranges, (long long)B, logl, parts));
   }
   LAUNCH_CHECK(h);
   return 0;
@@ -255,19 +271,6 @@ template <int NDET>
 int launch_bins_lp(ns_handle* h, const double* cbs, long long B, const int* rows_dev, double* logl, double* parts, cudaStream_t s) {
   if (B >= kLpBigBatch && !rows_dev) return launch_bins_lp_g<NDET, kLpNTBig, kLpOCCBig>(h, cbs, B, rows_dev, logl, parts, s);
   return launch_bins_lp_g<NDET, kLpNT, kLpOCC>(h, cbs, B, rows_dev, logl, parts, s);
-}
-
-// Launch with programmatic stream serialization: the kernel may become resident while the kernel before it on the stream still runs;
-// it calls pdl_wait() before it reads what that kernel wrote.
-template <class... KArgs, class... Args>
-cudaError_t launch_pdl(void (*kern)(KArgs...), unsigned grid, unsigned block, size_t smem, cudaStream_t s, Args... args) {
-  cudaLaunchConfig_t lc = {};
-  lc.gridDim = dim3(grid); lc.blockDim = dim3(block); lc.dynamicSmemBytes = smem; lc.stream = s;
-  cudaLaunchAttribute at[1];
-  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = 1;
-  lc.attrs = at; lc.numAttrs = 1;
-  return cudaLaunchKernelEx(&lc, kern, KArgs(args)...);
 }
 
 // Bins per range of k_pd_lp for `rows` rows (multiple of the tile length): the value that minimises rounds x (range + per-task
