@@ -338,8 +338,6 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
                                                            long long B_host, const int* __restrict__ B_dev /*overrides B_host*/,
                                                            double* logl, double* parts) {
   using AL = AccLayout<MODEL, NDET>;
-  const long long B = B_dev ? (long long)*B_dev : B_host;
-  if ((long long)blockIdx.x * P >= B) return;     // the worklist walk sizes the grid for its row capacity
   constexpr int NT = kBinsThreads, NW = NT / 32, NV = P * AL::N, ND1 = NDET > 1 ? NDET - 1 : 1;
   __shared__ __align__(16) double cbs[P * CB_SIZE];
   __shared__ double2 tabL[P * ND1 * 32], tabW[P * ND1 * NW], step[P * ND1];
@@ -348,8 +346,15 @@ __global__ void __launch_bounds__(kBinsThreads, 2) k_bins(const DevCfg* __restri
   __shared__ bool active[P];
   __shared__ int slot[P];
   const DevCfg& cfg = *cfgp;
-  const long long p0 = (long long)blockIdx.x * P;
+  // The coefficient blocks and the device-side row count are the output of the kernel before this one (see pdl_wait); the tables are the
+  // handle's.  A batch copies them under that kernel's tail; a round of the worklist walk, whose grid is sized for the row capacity, first
+  // lets the surplus CTAs go.
+  if (B_dev) pdl_wait();
+  const long long B = B_dev ? (long long)*B_dev : B_host;
+  if ((long long)blockIdx.x * P >= B) return;
   load_math_tables(&mtab, tb.mt, threadIdx.x, NT);
+  if (!B_dev) pdl_wait();
+  const long long p0 = (long long)blockIdx.x * P;
   if (threadIdx.x < P) slot[threadIdx.x] = threadIdx.x;
   for (int e = threadIdx.x; e < P * CB_SIZE; e += NT) {
     long long p = p0 + e / CB_SIZE;

@@ -325,11 +325,8 @@ int launch_pd_lp(ns_handle* h, const double* cbs, long long rows, const int* row
     cudaEventCreate(&e0); cudaEventCreate(&e1);
     cudaEventRecord(e0, s);
   }
-  if (rows_dev) {   // a round of the worklist walk: programmatic dependent launch behind k_wl_head (kernels_wl.cuh)
-    CU_CHECK(h, launch_pdl(k_pd_lp<NDET>, (unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s, (const DevCfg*)h->d_cfg, h->tb, a));
-  } else {
-    k_pd_lp<NDET><<<(unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s>>>(h->d_cfg, h->tb, a);
-  }
+  // programmatic dependent launch behind k_wl_head (a round of the worklist walk) or k_setup (a batch): the tables are copied under its tail
+  CU_CHECK(h, launch_pdl(k_pd_lp<NDET>, (unsigned)grid, kPdNT, pd_mix_bytes<kPdPP>(), s, (const DevCfg*)h->d_cfg, h->tb, a));
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
   return 0;
@@ -348,9 +345,11 @@ int launch_bins_nd(ns_handle* h, long long B, double* logl, double* parts, cudaS
     cudaEventRecord(e0, s);
   }
   if (P == 2) {
-    k_bins<MODEL, NDET, 2><<<(unsigned)((B + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, nullptr, logl, parts);
+    CU_CHECK(h, launch_pdl(k_bins<MODEL, NDET, 2>, (unsigned)((B + 1) / 2), kBinsThreads, 0, s, (const DevCfg*)h->d_cfg, h->tb, (const double*)h->d_cb,
+                           (long long)B, (const int*)nullptr, logl, parts));
   } else {
-    k_bins<MODEL, NDET, 1><<<(unsigned)B, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, h->d_cb, B, nullptr, logl, parts);
+    CU_CHECK(h, launch_pdl(k_bins<MODEL, NDET, 1>, (unsigned)B, kBinsThreads, 0, s, (const DevCfg*)h->d_cfg, h->tb, (const double*)h->d_cb, (long long)B,
+                           (const int*)nullptr, logl, parts));
   }
   if (e0) { cudaEventRecord(e1, s); h->prof_ev.emplace_back(e0, e1); }
   LAUNCH_CHECK(h);
@@ -511,8 +510,12 @@ template <int MODEL, int NDET>
 int sweep_rows(ns_handle* h, const double* cbs, long long R, const int* rows_dev, bool lane, double* logl, cudaStream_t s) {
   if (MODEL == 2 && lane) return launch_pd_lp<NDET>(h, cbs, R, rows_dev, h->wl_kr, logl, nullptr, s);
   if (MODEL == 1 && lane && R >= kLpMinBatch) return launch_bins_lp<NDET>(h, cbs, R, rows_dev, logl, nullptr, s);
-  if (R >= 4096) k_bins<MODEL, NDET, 2><<<(unsigned)((R + 1) / 2), kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
-  else k_bins<MODEL, NDET, 1><<<(unsigned)R, kBinsThreads, 0, s>>>(h->d_cfg, h->tb, cbs, R, rows_dev, logl, nullptr);
+  if (R >= 4096)
+    CU_CHECK(h, launch_pdl(k_bins<MODEL, NDET, 2>, (unsigned)((R + 1) / 2), kBinsThreads, 0, s, (const DevCfg*)h->d_cfg, h->tb, cbs, (long long)R, rows_dev,
+                           logl, (double*)nullptr));
+  else
+    CU_CHECK(h, launch_pdl(k_bins<MODEL, NDET, 1>, (unsigned)R, kBinsThreads, 0, s, (const DevCfg*)h->d_cfg, h->tb, cbs, (long long)R, rows_dev, logl,
+                           (double*)nullptr));
   LAUNCH_CHECK(h);
   return 0;
 }
