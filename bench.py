@@ -302,7 +302,10 @@ def run_ours(args):
                            "l2": "flushed between timed iterations (256 MiB write)", "parallelism": f"rows sharded x{world}, no collective"},
                 "clocks": clocks,
                 "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": B * 11 * 8, "d2h_bytes_per_step": B * 8,
-                        "max_abs_dlogl_vs_device_call": e2e_diff},
+                        "max_abs_dlogl_vs_device_call": e2e_diff,
+                        "how": "gw_loglike_batch_host on pinned host buffers: the set-up kernel fetches theta over the host link, the finishing code "
+                               "stores logL into the host buffer (the same bytes cross the link as with copies; nsgw_set_option(NSGW_OPT_HOST_ZERO_COPY, 0) "
+                               "restores cudaMemcpyAsync H2D / D2H around the kernels)"},
                 "gpu_launches": int(launches), "roofline": roof}
         bs = []
         for b in sweep_B:

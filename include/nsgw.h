@@ -91,9 +91,9 @@ const char* ns_last_error(const ns_handle* h); /* h may be NULL: message of the 
  * <d,h>_det, <h,h>_det interleaved. */
 int gw_loglike_batch(ns_handle* h, const double* theta_dev, int64_t B, double* logl_dev, double* parts_dev, void* stream);
 
-/* Same with HOST buffers (the end-to-end entry point bench.py's `e2e` leg times): theta_host [B, 11] -> H2D into handle-owned
- * scratch -> the same kernels -> D2H into logl_host [B].  Pinned host memory makes the copies asynchronous; pageable works too.
- * Synchronises before returning. */
+/* Same with HOST buffers (the end-to-end entry point bench.py's `e2e` leg times).  Pinned (device-accessible) buffers are used in
+ * place: the set-up kernel fetches theta_host [B, 11] over the host link while it computes, the finishing code stores into
+ * logl_host [B].  Pageable buffers go H2D into handle-owned scratch -> the same kernels -> D2H.  Synchronises before returning. */
 int gw_loglike_batch_host(ns_handle* h, const double* theta_host, int64_t B, double* logl_host, void* stream);
 
 /* gw_loglike_batch for callers that cannot allocate (CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc):
@@ -283,6 +283,9 @@ int nsgw_profile_read(ns_handle* h, double* total_ms_host, int64_t* launches_hos
  * traces and end points are identical for every chunk length and batch composition; between values the kernels sum a row's bins
  * in different fixed orders, so logL agrees to rounding (1e-12) and a decision can differ only where logL is that close to logL*. */
 #define NSGW_OPT_WALK_KERNEL 6
+/* key NSGW_OPT_HOST_ZERO_COPY: 1 (default) = gw_loglike_batch_host reads theta and writes logL in place when both buffers are pinned
+ * (device-accessible) host memory, with no copy in the stream; 0 = always copy through handle-owned device scratch.  Same results. */
+#define NSGW_OPT_HOST_ZERO_COPY 7
 int nsgw_set_option(ns_handle* h, int32_t key, int32_t value);
 
 /* Number of kernels launched by this library since process start (for bench.py's gpu_launches). */

@@ -34,6 +34,23 @@ __global__ void k_math_tables(MathTables* mt, double2* sc9, double2* sc11) {
   build_sc11(sc11, threadIdx.x, blockDim.x);
 }
 
+// k_setup for theta in MAPPED HOST memory (gw_loglike_batch_host with pinned buffers): the CTA's rows are one contiguous block, fetched
+// over the host link with coalesced loads into shared memory (a thread reading its own 11 doubles at an 88-byte stride would touch every
+// 128-byte line eleven times), then set up one row per thread as k_setup does -- same arithmetic, same coefficient blocks.
+template <int MODEL>
+__global__ void __launch_bounds__(128) k_setup_staged(const DevCfg* __restrict__ cfg, const double* theta, long long B, double* cbs) {
+  __shared__ double th_s[128 * 11];
+  const long long r0 = blockIdx.x * 128LL;
+  const int n = (int)min(128LL, B - r0);
+  for (int i = threadIdx.x; i < n * 11; i += 128) th_s[i] = theta[r0 * 11 + i];
+  __syncthreads();
+  if ((int)threadIdx.x >= n) return;
+  double th[11];
+#pragma unroll
+  for (int d = 0; d < 11; ++d) th[d] = th_s[threadIdx.x * 11 + d];
+  setup_particle<MODEL>(*cfg, th, cbs + (r0 + threadIdx.x) * CB_SIZE);
+}
+
 // I_{7/3} per detector: deterministic single-CTA tree sum.
 __global__ void k_i73(DevCfg* cfg, const double* __restrict__ ws) {
   __shared__ double sh[256];

@@ -54,7 +54,7 @@ EXPORTS = ["ns_init", "ns_free", "ns_last_error", "gw_loglike_batch", "gw_loglik
 
 # nsgw_set_option keys (include/nsgw.h)
 NOALLOC_MAX_ROWS, NOALLOC_MAX_BINS = 4096, 16384     # gw_loglike_batch_noalloc (include/nsgw.h)
-OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS, OPT_WALK_STAGE, OPT_WALK_KERNEL = 0, 1, 2, 3, 4, 5, 6
+OPT_BINS_KERNEL, OPT_WALK_SPEC, OPT_LIKELIHOOD, OPT_INNER_KERNEL, OPT_SLICE_STEPS, OPT_WALK_STAGE, OPT_WALK_KERNEL, OPT_HOST_ZERO_COPY = 0, 1, 2, 3, 4, 5, 6, 7
 
 _lib = None
 

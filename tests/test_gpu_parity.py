@@ -98,6 +98,30 @@ def test_taylorf2_injection_and_unphysical(nsgw, c2):
     assert h.gw_loglike_batch(dev(np.zeros((0, 11)))).numel() == 0     # empty batch
 
 
+@pytest.mark.parametrize("model", ["taylorf2", "phenomd"])
+def test_host_entry_paths_agree(nsgw, c2, c3, model):
+    # gw_loglike_batch_host: pinned buffers used in place (theta fetched over the host link by the set-up kernel, logL stored into the
+    # caller's buffer), the same with the copies forced, and pageable buffers -- all bit for bit the device call
+    spec = c2 if model == "taylorf2" else c3[0]
+    h = nsgw.Handle(spec)
+    for B in (1, 700, 5000):
+        u = W.uniforms(B, 11, 300 + B)
+        th = h.prior_transform_batch(dev(u))
+        th[B // 2, 1] = 1.5                                   # an unphysical row: -inf
+        ref = h.gw_loglike_batch(th).cpu()
+        th_pin, out_pin = th.cpu().pin_memory(), torch.full((B,), float("nan"), dtype=torch.float64).pin_memory()
+        h.gw_loglike_batch_host(th_pin, out_pin)
+        assert torch.equal(out_pin, ref)
+        h.set_option(nsgw.OPT_HOST_ZERO_COPY, 0)
+        out2 = torch.full((B,), float("nan"), dtype=torch.float64).pin_memory()
+        h.gw_loglike_batch_host(th_pin, out2)
+        h.set_option(nsgw.OPT_HOST_ZERO_COPY, 1)
+        assert torch.equal(out2, ref)
+        out3 = torch.full((B,), float("nan"), dtype=torch.float64)          # pageable
+        h.gw_loglike_batch_host(th.cpu(), out3)
+        assert torch.equal(out3, ref)
+
+
 @pytest.mark.parametrize("kern", KERNELS)
 @pytest.mark.parametrize("B", [3, 515, 4101])
 def test_phenomd_loglike_parity_config3_shape(nsgw, c3, B, kern):
